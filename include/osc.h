@@ -1,0 +1,159 @@
+/*
+ * osc.h -- C ABI of libosc_b200: per-event three-flavour neutrino oscillation probability through
+ * constant-density matter, event reweighting and binned-PDF filling on one NVIDIA B200 (sm_100a).
+ *
+ * The calls follow the paper's statement of the problem (arXiv:1311.7579; line numbers are those of
+ * PAPER.md) and BASELINE.json:north_star:
+ *   - the oscillation-parameter set of Table 1 goes in through osc_set_params;
+ *     everything that depends only on the parameters is computed once on the host and handed to the
+ *     kernels ("computed on the CPU and then copied to the GPU");
+ *   - an array of true energies in, one oscillation weight per element out, double precision
+ *     (Listing 1)                                                  -> osc_prob[_all];
+ *   - each Monte Carlo event weighted by its oscillation probability and binned into a histogram, the
+ *     PDF, with the energy-scale systematic applied by "simply scaling the ...
+ *     reconstructed energy"                                          -> osc_reweight_bin;
+ *   - one PDF rebuild per proposed parameter set                    -> osc_reweight_bin_batch.
+ *
+ * Conventions (DESIGN.md "Readings of the paper" A1..A16):
+ *   - phase m^2 L / 2E = OSC_K_PHASE * m^2[eV^2] * L[km] / E[GeV];
+ *     matter term A = OSC_K_MATTER * OSC_Y_E * rho[g/cm^3] * E[GeV] (eV^2), sign flipped for antineutrinos;
+ *   - PMNS matrix in the PDG parametrisation, input angles as sin^2(theta_ij); antineutrinos use U*;
+ *   - m^2 = (0, dm2_21, dm2_31), dm2_31 = hierarchy * |dm2_32| + dm2_21;
+ *   - P(alpha -> beta) = |S_{beta alpha}|^2, S = exp(-i H L), flavour index 0 = e, 1 = mu, 2 = tau.
+ *
+ * Memory: every array argument marked DEVICE is caller-owned device memory on the current CUDA device
+ * (for PyTorch: tensor.data_ptr()); the library neither frees nor keeps caller pointers beyond the work
+ * it enqueues.  HOST arguments are read before the call returns.  fp64 arrays must be 8-byte aligned.
+ *
+ * Asynchrony: osc_prob*, osc_reweight_bin* enqueue work on `stream` (a cudaStream_t passed as void*;
+ * NULL = the legacy default stream) and return without synchronising; results are valid once the caller
+ * has synchronised the stream.  osc_set_params is host-synchronous and affects only calls made after it
+ * returns: each launch carries its own copy of the parameter block (kernel-parameter constant bank), so
+ * changing parameters never races with work already enqueued.
+ *
+ * Errors: every call returns an osc_status (0 = OK, negative = error) and never throws or aborts;
+ * osc_last_error() gives the message of the calling thread's most recent failure.  Per-event data
+ * faults cannot be reported synchronously and have defined data semantics instead (A11): an event whose
+ * E_true is not finite or <= 0 yields NaN from osc_prob[_all] and is skipped by osc_reweight_bin*; so is
+ * an event whose channel code is outside [0, n_channels).
+ */
+#ifndef OSC_B200_H
+#define OSC_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define OSC_K_PHASE 2.5338653580781979     /* rad per (eV^2 km / GeV): 1e3 / (2e9 hbar c [eV m])        */
+#define OSC_K_MATTER 1.5264932449499478e-4 /* eV^2 per (GeV g/cm^3): 2 sqrt2 G_F (hbar c)^3 N_A 1e18    */
+#define OSC_Y_E 0.5                        /* electrons per nucleon                                      */
+
+typedef enum {
+    OSC_OK = 0,
+    OSC_ERR_INVALID_ARG = -1,    /* null pointer with n > 0, flavour/hierarchy/range violation, non-finite scalar */
+    OSC_ERR_NOT_CONFIGURED = -2, /* osc_set_params has not been called successfully                               */
+    OSC_ERR_CUDA = -3,           /* a CUDA runtime call failed (message in osc_last_error)                        */
+    OSC_ERR_ALIGNMENT = -4       /* an fp64 array pointer is not 8-byte aligned                                   */
+} osc_status;
+
+enum { OSC_NU_E = 0, OSC_NU_MU = 1, OSC_NU_TAU = 2 }; /* flavour index */
+enum { OSC_NORMAL = 1, OSC_INVERTED = -1 };           /* mass hierarchy */
+
+/* Number of reweighting channels and their meaning (BASELINE.json configs[2]):
+ * channel 0: nu_mu -> nu_mu, 1: nu_mu -> nu_e, 2: nubar_mu -> nubar_mu, 3: nubar_mu -> nubar_e. */
+#define OSC_N_CHANNELS 4
+
+/* One oscillation-parameter set; same fields and order as osc_set_params. */
+typedef struct {
+    double sin2_th12, sin2_th23, sin2_th13; /* sin^2(theta_ij), each in [0, 1]            */
+    double dm2_32;                          /* |Delta m^2_32| in eV^2, > 0                 */
+    double dm2_21;                          /* Delta m^2_21 in eV^2, >= 0                  */
+    double delta_cp;                        /* radians                                     */
+    double rho_g_cm3;                       /* matter density in g/cm^3, >= 0              */
+    double L_km;                            /* baseline in km, >= 0                        */
+    int hierarchy;                          /* OSC_NORMAL or OSC_INVERTED                  */
+} osc_params;
+
+/* Host-side per-parameter-set precompute.
+ * Stores the parameter block that later calls hand to their kernels.  Thread-safe; host only.
+ * Returns OSC_ERR_INVALID_ARG (state unchanged) if any value is outside the ranges listed above. */
+int osc_set_params(double sin2_th12, double sin2_th23, double sin2_th13, double dm2_32, double dm2_21,
+                   double delta_cp, double rho_g_cm3, double L_km, int hierarchy);
+
+/* Per-event probability (rows a2a-a2f, kernel calculateOscProb of Listing 1).
+ *   E_true  DEVICE [n]  true neutrino energies in GeV
+ *   P_out   DEVICE [n]  P(flavour_in -> flavour_out) for (anti)neutrinos; NaN where E_true is unusable
+ * n == 0 is a no-op returning OSC_OK. */
+int osc_prob(const double *E_true, size_t n, int flavour_in, int flavour_out, int antinu, double *P_out,
+             void *stream);
+
+/* All nine transitions from one eigen-solve per event (BASELINE.json configs[1]).
+ *   P_out   DEVICE [9][n] row-major; row 3*beta + alpha holds P(alpha -> beta). */
+int osc_prob_all(const double *E_true, size_t n, int antinu, double *P_out, void *stream);
+
+/* Fused reweight + histogram (rows a3a-a3c).  For every event j with usable
+ * E_true[j] and channel[j] in [0, OSC_N_CHANNELS):
+ *     x = fl64(energy_scale * E_reco[j])                      (one rounded fp64 multiply)
+ *     b = the unique i with bin_edges[i] <= x < bin_edges[i+1] (fp64 compares); no such i -> event dropped
+ *     hist_out[channel[j]][b] += w0[j] * P_channel(E_true[j])
+ *   E_true, E_reco, w0  DEVICE [n] fp64;   channel  DEVICE [n] int8
+ *   bin_edges           DEVICE [n_bins + 1] fp64, strictly increasing (not checked: device data)
+ *   hist_out            DEVICE [OSC_N_CHANNELS][n_bins] fp64 row-major, OVERWRITTEN (zeroed when n == 0)
+ * No per-event weight array is written to memory.  The result is bit-reproducible from run to run for
+ * fixed inputs (fixed event -> thread map, fixed-order merges, no floating-point atomics). */
+int osc_reweight_bin(const double *E_true, const double *E_reco, const double *w0, const int8_t *channel,
+                     size_t n, double energy_scale, const double *bin_edges, int n_bins, double *hist_out,
+                     void *stream);
+
+/* Batched parameter sets (row a4; BASELINE.json configs[3]): slice p of hist_out equals
+ * osc_reweight_bin run with points[p].  Independent of the state set by osc_set_params.
+ *   points    HOST [n_points]; validated and copied before the call returns
+ *   hist_out  DEVICE [n_points][OSC_N_CHANNELS][n_bins] fp64, OVERWRITTEN */
+int osc_reweight_bin_batch(const osc_params *points, int n_points, const double *E_true,
+                           const double *E_reco, const double *w0, const int8_t *channel, size_t n,
+                           double energy_scale, const double *bin_edges, int n_bins, double *hist_out,
+                           void *stream);
+
+/* Debug/verification export of the integer binning decision of osc_reweight_bin (row a3c):
+ *   bin_out  DEVICE [n] int32: the bin index b of event j, or -1 if the event is dropped. */
+int osc_bin_index(const double *E_true, const double *E_reco, const int8_t *channel, size_t n,
+                  double energy_scale, const double *bin_edges, int n_bins, int32_t *bin_out, void *stream);
+
+/* Same as the osc_prob / osc_reweight_bin pair but with HOST buffers: copies the inputs to the device,
+ * runs the kernels, copies the result back and synchronises.  This is the flow of the paper's Listing 1
+ * and what bench.py times as "e2e". */
+int osc_prob_host(const double *E_true_host, size_t n, int flavour_in, int flavour_out, int antinu,
+                  double *P_out_host);
+int osc_reweight_bin_host(const double *E_true_host, const double *E_reco_host, const double *w0_host,
+                          const int8_t *channel_host, size_t n, double energy_scale,
+                          const double *bin_edges_host, int n_bins, double *hist_out_host);
+
+/* Message of the calling thread's most recent error ("" if none).  Never NULL. */
+const char *osc_last_error(void);
+
+/* Number of kernel launches this library has enqueued since it was loaded (for bench.py's gpu_launches). */
+unsigned long long osc_launch_count(void);
+
+/* Library version string, e.g. "osc_b200 0.1 (sm_100a)". */
+const char *osc_version(void);
+
+/* The library works on the calling thread's current CUDA device.  These two wrap cudaSetDevice /
+ * cudaGetDevice of the library's own (statically linked) CUDA runtime so that a caller which picked its
+ * device through another runtime instance (PyTorch) can check and align the two. */
+int osc_set_device(int device);
+int osc_get_device(int *device /* HOST, out */);
+
+/* Measurement helper, not part of the hot path: enqueues one launch of a register-only chain of
+ * independent fp64 fused multiply-adds on every SM (blocks_per_sm blocks of 256 threads each, 8 chains
+ * per thread, `iters` DFMAs per chain) and reports in *flops_per_launch (HOST, out, may be NULL) the
+ * floating-point operations of that launch (2 per DFMA).  bench.py times it with CUDA events to obtain
+ * the measured fp64 peak that roofline fractions are quoted against. */
+int osc_fp64_peak_probe(int iters, int blocks_per_sm, double *flops_per_launch, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OSC_B200_H */

@@ -1,0 +1,11 @@
+"""osc-b200: per-event three-flavour neutrino oscillation reweighting on one NVIDIA B200 (sm_100a, fp64).
+
+The product is the C-ABI library ``libosc_b200.so`` (include/osc.h, sources under ``csrc/``); this
+package is its thin Python binding (``binding.py``), its build step (``build.py``) and the seeded
+synthetic input generators (``workloads.py``).  See DESIGN.md.
+"""
+from .binding import (  # noqa: F401
+    N_CHANNELS, OscError, osc_bin_index, osc_fp64_peak_probe, osc_get_device, osc_last_error, osc_launch_count,
+    osc_params, osc_prob, osc_prob_all, osc_prob_host, osc_reweight_bin, osc_reweight_bin_batch,
+    osc_reweight_bin_host, osc_set_device, osc_set_params, osc_version,
+)

@@ -1,0 +1,271 @@
+"""Thin ctypes binding of libosc_b200.so (include/osc.h): argument marshalling only.
+
+Every function has the name of the C entry point it calls; all arithmetic of the path runs in the
+CUDA kernels behind that call.  PyTorch supplies device memory (``tensor.data_ptr()``) and the stream
+(``torch.cuda.current_stream()``) and nothing else.  There is no CPU fallback: if the shared library
+is missing or a call fails, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Mapping, Optional, Sequence
+
+import numpy as np
+
+from . import build as _build
+
+_dp = ctypes.c_void_p
+_lib: Optional[ctypes.CDLL] = None
+
+N_CHANNELS = 4  # OSC_N_CHANNELS
+PARAM_FIELDS = ("sin2_th12", "sin2_th23", "sin2_th13", "dm2_32", "dm2_21", "delta_cp", "rho_g_cm3",
+                "L_km", "hierarchy")
+
+# every symbol include/osc.h declares (tests/test_abi.py checks the header against this list)
+EXPORTS = ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_batch",
+           "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_last_error", "osc_launch_count",
+           "osc_version", "osc_set_device", "osc_get_device", "osc_fp64_peak_probe")
+
+
+class OscError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"libosc_b200 status {status}: {message}")
+        self.status = status
+
+
+class osc_params(ctypes.Structure):
+    """Mirror of ``osc_params`` in include/osc.h."""
+    _fields_ = [("sin2_th12", ctypes.c_double), ("sin2_th23", ctypes.c_double), ("sin2_th13", ctypes.c_double),
+                ("dm2_32", ctypes.c_double), ("dm2_21", ctypes.c_double), ("delta_cp", ctypes.c_double),
+                ("rho_g_cm3", ctypes.c_double), ("L_km", ctypes.c_double), ("hierarchy", ctypes.c_int)]
+
+
+def lib() -> ctypes.CDLL:
+    """Load libosc_b200.so (built in-tree by paper_1311_7579_b200.build).  Fails loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB_PATH
+    if not os.path.exists(path):
+        raise OscError(-100, f"{path} is missing: run `python -m paper_1311_7579_b200.build` "
+                             "(there is no CPU fallback)")
+    L = ctypes.CDLL(path)
+    d, i, sz, vp = ctypes.c_double, ctypes.c_int, ctypes.c_size_t, ctypes.c_void_p
+    L.osc_set_params.argtypes = [d, d, d, d, d, d, d, d, i]
+    L.osc_prob.argtypes = [_dp, sz, i, i, i, _dp, vp]
+    L.osc_prob_all.argtypes = [_dp, sz, i, _dp, vp]
+    L.osc_reweight_bin.argtypes = [_dp, _dp, _dp, _dp, sz, d, _dp, i, _dp, vp]
+    L.osc_reweight_bin_batch.argtypes = [ctypes.POINTER(osc_params), i, _dp, _dp, _dp, _dp, sz, d, _dp, i, _dp, vp]
+    L.osc_bin_index.argtypes = [_dp, _dp, _dp, sz, d, _dp, i, _dp, vp]
+    L.osc_prob_host.argtypes = [_dp, sz, i, i, i, _dp]
+    L.osc_reweight_bin_host.argtypes = [_dp, _dp, _dp, _dp, sz, d, _dp, i, _dp]
+    L.osc_set_device.argtypes = [i]
+    L.osc_get_device.argtypes = [ctypes.POINTER(i)]
+    L.osc_fp64_peak_probe.argtypes = [i, i, ctypes.POINTER(d), vp]
+    for name in ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_batch",
+                 "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_set_device", "osc_get_device",
+                 "osc_fp64_peak_probe"):
+        getattr(L, name).restype = i
+    L.osc_last_error.restype = ctypes.c_char_p
+    L.osc_version.restype = ctypes.c_char_p
+    L.osc_launch_count.restype = ctypes.c_ulonglong
+    _lib = L
+    return L
+
+
+def _check(rc: int) -> None:
+    if rc != 0:
+        raise OscError(rc, lib().osc_last_error().decode())
+
+
+def _stream(stream) -> int:
+    import torch
+
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _dev(t, dtype, what: str) -> int:
+    """Device pointer of a contiguous CUDA tensor of the given dtype."""
+    if not t.is_cuda:
+        raise TypeError(f"{what} must be a CUDA tensor")
+    if t.dtype != dtype:
+        raise TypeError(f"{what} must have dtype {dtype}, got {t.dtype}")
+    if not t.is_contiguous():
+        raise TypeError(f"{what} must be contiguous")
+    _sync_device(t.device.index)
+    return t.data_ptr()
+
+
+_cur_dev = None
+
+
+def _sync_device(index: Optional[int]) -> None:
+    """Align the library's (statically linked) CUDA runtime with the device of the tensors."""
+    global _cur_dev
+    if index is None:
+        index = 0
+    if _cur_dev != index:
+        _check(lib().osc_set_device(int(index)))
+        _cur_dev = index
+
+
+def _host(a: np.ndarray, dtype, what: str) -> int:
+    if not isinstance(a, np.ndarray) or a.dtype != dtype or not a.flags["C_CONTIGUOUS"]:
+        raise TypeError(f"{what} must be a C-contiguous numpy array of dtype {np.dtype(dtype)}")
+    return a.ctypes.data
+
+
+def make_params(p) -> osc_params:
+    if isinstance(p, osc_params):
+        return p
+    if isinstance(p, Mapping):
+        return osc_params(*[p[f] if f != "hierarchy" else int(p[f]) for f in PARAM_FIELDS])
+    return osc_params(*[getattr(p, f) if f != "hierarchy" else int(getattr(p, f)) for f in PARAM_FIELDS])
+
+
+# ---------------------------------------------------------------------------------------------------
+# entry points (same names and argument order as include/osc.h)
+# ---------------------------------------------------------------------------------------------------
+
+def osc_set_params(sin2_th12: float, sin2_th23: float, sin2_th13: float, dm2_32: float, dm2_21: float,
+                   delta_cp: float, rho_g_cm3: float, L_km: float, hierarchy: int = 1) -> None:
+    _check(lib().osc_set_params(sin2_th12, sin2_th23, sin2_th13, dm2_32, dm2_21, delta_cp, rho_g_cm3, L_km,
+                                int(hierarchy)))
+
+
+def osc_prob(E_true, flavour_in: int, flavour_out: int, antinu: int, P_out=None, stream=None):
+    import torch
+
+    n = E_true.numel()
+    if P_out is None:
+        P_out = torch.empty_like(E_true)
+    _check(lib().osc_prob(_dev(E_true, torch.float64, "E_true"), n, flavour_in, flavour_out, int(antinu),
+                          _dev(P_out, torch.float64, "P_out"), _stream(stream)))
+    return P_out
+
+
+def osc_prob_all(E_true, antinu: int, P_out=None, stream=None):
+    """[9, n] tensor, row 3*beta + alpha = P(alpha -> beta)."""
+    import torch
+
+    n = E_true.numel()
+    if P_out is None:
+        P_out = torch.empty((9, n), dtype=torch.float64, device=E_true.device)
+    if P_out.numel() != 9 * n:
+        raise ValueError("P_out must hold 9 * n values")
+    _check(lib().osc_prob_all(_dev(E_true, torch.float64, "E_true"), n, int(antinu),
+                              _dev(P_out, torch.float64, "P_out"), _stream(stream)))
+    return P_out
+
+
+def _event_ptrs(E_true, E_reco, w0, channel):
+    import torch
+
+    n = E_true.numel()
+    if E_reco.numel() != n or channel.numel() != n or (w0 is not None and w0.numel() != n):
+        raise ValueError("event arrays differ in length")
+    return (n, _dev(E_true, torch.float64, "E_true"), _dev(E_reco, torch.float64, "E_reco"),
+            _dev(w0, torch.float64, "w0") if w0 is not None else None, _dev(channel, torch.int8, "channel"))
+
+
+def osc_reweight_bin(E_true, E_reco, w0, channel, energy_scale: float, bin_edges, hist_out=None, stream=None):
+    """[N_CHANNELS, n_bins] histogram tensor (overwritten)."""
+    import torch
+
+    n, pt, pr, pw, pc = _event_ptrs(E_true, E_reco, w0, channel)
+    nb = bin_edges.numel() - 1
+    if hist_out is None:
+        hist_out = torch.empty((N_CHANNELS, nb), dtype=torch.float64, device=E_true.device)
+    if hist_out.numel() != N_CHANNELS * nb:
+        raise ValueError("hist_out must hold N_CHANNELS * n_bins values")
+    _check(lib().osc_reweight_bin(pt, pr, pw, pc, n, float(energy_scale), _dev(bin_edges, torch.float64, "bin_edges"),
+                                  nb, _dev(hist_out, torch.float64, "hist_out"), _stream(stream)))
+    return hist_out
+
+
+def osc_reweight_bin_batch(points: Sequence, E_true, E_reco, w0, channel, energy_scale: float, bin_edges,
+                           hist_out=None, stream=None):
+    """[n_points, N_CHANNELS, n_bins] histograms, one slice per parameter set, in one call."""
+    import torch
+
+    n, pt, pr, pw, pc = _event_ptrs(E_true, E_reco, w0, channel)
+    nb = bin_edges.numel() - 1
+    npts = len(points)
+    arr = (osc_params * max(npts, 1))(*[make_params(q) for q in points])
+    if hist_out is None:
+        hist_out = torch.empty((npts, N_CHANNELS, nb), dtype=torch.float64, device=E_true.device)
+    if hist_out.numel() != npts * N_CHANNELS * nb:
+        raise ValueError("hist_out must hold n_points * N_CHANNELS * n_bins values")
+    _check(lib().osc_reweight_bin_batch(arr, npts, pt, pr, pw, pc, n, float(energy_scale),
+                                        _dev(bin_edges, torch.float64, "bin_edges"), nb,
+                                        _dev(hist_out, torch.float64, "hist_out"), _stream(stream)))
+    return hist_out
+
+
+def osc_bin_index(E_true, E_reco, channel, energy_scale: float, bin_edges, bin_out=None, stream=None):
+    import torch
+
+    n, pt, pr, _, pc = _event_ptrs(E_true, E_reco, None, channel)
+    nb = bin_edges.numel() - 1
+    if bin_out is None:
+        bin_out = torch.empty(n, dtype=torch.int32, device=E_true.device)
+    _check(lib().osc_bin_index(pt, pr, pc, n, float(energy_scale), _dev(bin_edges, torch.float64, "bin_edges"), nb,
+                               _dev(bin_out, torch.int32, "bin_out"), _stream(stream)))
+    return bin_out
+
+
+def osc_prob_host(E_true: np.ndarray, flavour_in: int, flavour_out: int, antinu: int,
+                  P_out: Optional[np.ndarray] = None) -> np.ndarray:
+    """Host buffers in and out (the flow of the paper's Listing 1): H2D, kernel, D2H, synchronise."""
+    if P_out is None:
+        P_out = np.empty_like(E_true)
+    _check(lib().osc_prob_host(_host(E_true, np.float64, "E_true"), E_true.size, flavour_in, flavour_out,
+                               int(antinu), _host(P_out, np.float64, "P_out")))
+    return P_out
+
+
+def osc_reweight_bin_host(E_true: np.ndarray, E_reco: np.ndarray, w0: np.ndarray, channel: np.ndarray,
+                          energy_scale: float, bin_edges: np.ndarray,
+                          hist_out: Optional[np.ndarray] = None) -> np.ndarray:
+    nb = bin_edges.size - 1
+    if hist_out is None:
+        hist_out = np.empty((N_CHANNELS, nb), dtype=np.float64)
+    _check(lib().osc_reweight_bin_host(_host(E_true, np.float64, "E_true"), _host(E_reco, np.float64, "E_reco"),
+                                       _host(w0, np.float64, "w0"), _host(channel, np.int8, "channel"), E_true.size,
+                                       float(energy_scale), _host(bin_edges, np.float64, "bin_edges"), nb,
+                                       _host(hist_out, np.float64, "hist_out")))
+    return hist_out
+
+
+def osc_last_error() -> str:
+    return lib().osc_last_error().decode()
+
+
+def osc_launch_count() -> int:
+    return int(lib().osc_launch_count())
+
+
+def osc_version() -> str:
+    return lib().osc_version().decode()
+
+
+def osc_set_device(device: int) -> None:
+    global _cur_dev
+    _check(lib().osc_set_device(int(device)))
+    _cur_dev = int(device)
+
+
+def osc_get_device() -> int:
+    v = ctypes.c_int(-1)
+    _check(lib().osc_get_device(ctypes.byref(v)))
+    return v.value
+
+
+def osc_fp64_peak_probe(iters: int, blocks_per_sm: int = 4, stream=None) -> float:
+    """Enqueue one DFMA-probe launch; returns its floating-point operation count."""
+    flops = ctypes.c_double(0.0)
+    _check(lib().osc_fp64_peak_probe(int(iters), int(blocks_per_sm), ctypes.byref(flops), _stream(stream)))
+    return flops.value

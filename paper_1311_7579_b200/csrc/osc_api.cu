@@ -1,0 +1,416 @@
+// osc_api.cu -- the C ABI of libosc_b200 (include/osc.h): argument checks, host precompute, launches.
+// No torch types, no exceptions across the boundary; every failure sets the thread's error message.
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <vector>
+
+#include "../../include/osc.h"
+#include "osc_kernels.cuh"
+#include "osc_precompute.h"
+
+using namespace oscb;
+
+namespace {
+
+thread_local char t_err[512] = "";
+std::mutex g_mu;
+HostSet g_state;
+bool g_configured = false;
+std::atomic<unsigned long long> g_launches{0};
+
+int fail(int code, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(t_err, sizeof(t_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                                   \
+    do {                                                                                                 \
+        cudaError_t e_ = (expr);                                                                         \
+        if (e_ != cudaSuccess) return fail(OSC_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_));        \
+    } while (0)
+
+bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+int sm_count(int* out)
+{
+    static int cached[64] = {0};
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return fail(OSC_ERR_CUDA, "device index %d out of range", dev);
+    if (cached[dev] == 0) {
+        int v = 0;
+        CUDA_TRY(cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev));
+        cached[dev] = v;
+    }
+    *out = cached[dev];
+    return OSC_OK;
+}
+
+int snapshot(HostSet& h)
+{
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!g_configured) return fail(OSC_ERR_NOT_CONFIGURED, "osc_set_params has not been called");
+    h = g_state;
+    return OSC_OK;
+}
+
+int check_flavour(int f, const char* what)
+{
+    if (f < 0 || f > 2) return fail(OSC_ERR_INVALID_ARG, "%s = %d is not a flavour index (0, 1, 2)", what, f);
+    return OSC_OK;
+}
+
+// Blocks per SM the persistent kernels are sized for (register budget: see DESIGN.md "Kernels").
+constexpr int kBlocksPerSM = 4;
+
+int grid_for(size_t work_items, int* grid)
+{
+    int sms = 0;
+    int rc = sm_count(&sms);
+    if (rc) return rc;
+    size_t g = (size_t)sms * kBlocksPerSM;
+    if (work_items < g) g = work_items;
+    if (g < 1) g = 1;
+    *grid = (int)g;
+    return OSC_OK;
+}
+
+int post_launch(const char* what)
+{
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(OSC_ERR_CUDA, "%s launch failed: %s", what, cudaGetErrorString(e));
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return OSC_OK;
+}
+
+size_t bin_smem_bytes(int nb)
+{
+    return sizeof(unsigned long long) * (size_t)(nb + 1) + sizeof(double) * kTransFields * kChannels +
+           sizeof(double) * (size_t)kWarps * kChannels * (size_t)nb;
+}
+
+constexpr int kMaxBins = 768; // 8 warps x 4 channels x 768 bins x 8 B = 196 KB of per-warp histograms
+
+int check_bin_args(const double* E_true, const double* E_reco, const double* w0, const int8_t* channel, size_t n,
+                   double energy_scale, const double* bin_edges, int n_bins, const void* out)
+{
+    if (n_bins < 1 || n_bins > kMaxBins)
+        return fail(OSC_ERR_INVALID_ARG, "n_bins = %d outside [1, %d]", n_bins, kMaxBins);
+    if (!(energy_scale > 0.0) || !std::isfinite(energy_scale))
+        return fail(OSC_ERR_INVALID_ARG, "energy_scale must be finite and > 0");
+    if (!bin_edges || !out) return fail(OSC_ERR_INVALID_ARG, "null bin_edges or output pointer");
+    if (n > 0 && (!E_true || !E_reco || !channel)) return fail(OSC_ERR_INVALID_ARG, "null event array with n > 0");
+    (void)w0;
+    if (!aligned(E_true, 8) || !aligned(E_reco, 8) || !aligned(w0, 8) || !aligned(bin_edges, 8))
+        return fail(OSC_ERR_ALIGNMENT, "fp64 array not 8-byte aligned");
+    return OSC_OK;
+}
+
+// Enqueue k2 for one parameter block.  hist_out is overwritten.
+int launch_reweight(const BinArgs& args, const double* E_true, const double* E_reco, const double* w0,
+                    const int8_t* channel, size_t n, double energy_scale, const double* bin_edges, int n_bins,
+                    double* hist_out, cudaStream_t st)
+{
+    const size_t nh = (size_t)kChannels * n_bins;
+    if (n == 0) {
+        CUDA_TRY(cudaMemsetAsync(hist_out, 0, nh * sizeof(double), st));
+        return OSC_OK;
+    }
+    const size_t ntiles = (n + 2 * kBlock - 1) / (2 * kBlock);
+    int grid = 1;
+    int rc = grid_for(ntiles, &grid);
+    if (rc) return rc;
+    const size_t smem = bin_smem_bytes(n_bins);
+    // fewer resident blocks when the per-warp histograms are large
+    if (smem > 48 * 1024) {
+        int sms = 0;
+        rc = sm_count(&sms);
+        if (rc) return rc;
+        size_t per_sm = (size_t)(220 * 1024) / smem;
+        if (per_sm < 1) per_sm = 1;
+        if (per_sm > (size_t)kBlocksPerSM) per_sm = kBlocksPerSM;
+        size_t g = (size_t)sms * per_sm;
+        if ((size_t)grid > g) grid = (int)g;
+    }
+    const int ngroups = (grid + kGroup - 1) / kGroup;
+    const size_t bytes_partial = (size_t)grid * nh * sizeof(double);
+    const size_t bytes_gpartial = (size_t)ngroups * nh * sizeof(double);
+    const size_t bytes_counters = (size_t)(ngroups + 1) * sizeof(unsigned int);
+    char* scratch = nullptr;
+    CUDA_TRY(cudaMallocAsync((void**)&scratch, bytes_partial + bytes_gpartial + bytes_counters, st));
+    MergeScratch ms;
+    ms.partial = reinterpret_cast<double*>(scratch);
+    ms.gpartial = reinterpret_cast<double*>(scratch + bytes_partial);
+    ms.counters = reinterpret_cast<unsigned int*>(scratch + bytes_partial + bytes_gpartial);
+    ms.ngroups = ngroups;
+    cudaError_t e = cudaMemsetAsync(ms.counters, 0, bytes_counters, st);
+    if (e == cudaSuccess) {
+        const bool vec = aligned(E_true, 16) && aligned(E_reco, 16) && aligned(w0, 16) && aligned(channel, 2);
+        if (vec) {
+            if (smem > 48 * 1024)
+                e = cudaFuncSetAttribute(reweight_bin_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e == cudaSuccess)
+                reweight_bin_kernel<true><<<grid, kBlock, smem, st>>>(args, E_true, E_reco, w0, channel, n, energy_scale,
+                                                                    bin_edges, n_bins, ms, hist_out);
+        } else {
+            if (smem > 48 * 1024)
+                e = cudaFuncSetAttribute(reweight_bin_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e == cudaSuccess)
+                reweight_bin_kernel<false><<<grid, kBlock, smem, st>>>(args, E_true, E_reco, w0, channel, n,
+                                                                     energy_scale, bin_edges, n_bins, ms, hist_out);
+        }
+        if (e == cudaSuccess) e = cudaGetLastError();
+        if (e == cudaSuccess) g_launches.fetch_add(1, std::memory_order_relaxed);
+    }
+    cudaError_t e2 = cudaFreeAsync(scratch, st);
+    if (e != cudaSuccess) return fail(OSC_ERR_CUDA, "osc_reweight_bin launch failed: %s", cudaGetErrorString(e));
+    if (e2 != cudaSuccess) return fail(OSC_ERR_CUDA, "cudaFreeAsync: %s", cudaGetErrorString(e2));
+    return OSC_OK;
+}
+
+// Device staging buffers of the *_host entry points (grown on demand, reused between calls).
+struct HostPath {
+    std::mutex mu;
+    cudaStream_t stream = nullptr;
+    char* buf = nullptr;
+    size_t cap = 0;
+    int ensure(size_t bytes)
+    {
+        if (!stream) CUDA_TRY(cudaStreamCreateWithFlags(&stream, cudaStreamNonBlocking));
+        if (bytes > cap) {
+            if (buf) CUDA_TRY(cudaFree(buf));
+            buf = nullptr;
+            cap = 0;
+            CUDA_TRY(cudaMalloc((void**)&buf, bytes));
+            cap = bytes;
+        }
+        return OSC_OK;
+    }
+};
+HostPath g_host;
+
+size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+} // namespace
+
+extern "C" {
+
+int osc_set_params(double sin2_th12, double sin2_th23, double sin2_th13, double dm2_32, double dm2_21,
+                   double delta_cp, double rho_g_cm3, double L_km, int hierarchy)
+{
+    osc_params p;
+    p.sin2_th12 = sin2_th12;
+    p.sin2_th23 = sin2_th23;
+    p.sin2_th13 = sin2_th13;
+    p.dm2_32 = dm2_32;
+    p.dm2_21 = dm2_21;
+    p.delta_cp = delta_cp;
+    p.rho_g_cm3 = rho_g_cm3;
+    p.L_km = L_km;
+    p.hierarchy = hierarchy;
+    if (const char* msg = check_params(p)) return fail(OSC_ERR_INVALID_ARG, "osc_set_params: %s", msg);
+    HostSet h;
+    precompute(p, h);
+    std::lock_guard<std::mutex> lk(g_mu);
+    g_state = h;
+    g_configured = true;
+    return OSC_OK;
+}
+
+int osc_prob(const double* E_true, size_t n, int flavour_in, int flavour_out, int antinu, double* P_out, void* stream)
+{
+    int rc;
+    if ((rc = check_flavour(flavour_in, "flavour_in")) || (rc = check_flavour(flavour_out, "flavour_out"))) return rc;
+    if (antinu != 0 && antinu != 1) return fail(OSC_ERR_INVALID_ARG, "antinu must be 0 or 1");
+    HostSet h;
+    if ((rc = snapshot(h))) return rc;
+    if (n == 0) return OSC_OK;
+    if (!E_true || !P_out) return fail(OSC_ERR_INVALID_ARG, "null array with n > 0");
+    if (!aligned(E_true, 8) || !aligned(P_out, 8)) return fail(OSC_ERR_ALIGNMENT, "fp64 array not 8-byte aligned");
+    ProbArgs a;
+    a.set = h.set;
+    a.tr = make_trans(h, flavour_in, flavour_out, antinu);
+    const size_t npairs = (n + 1) / 2;
+    int grid = 1;
+    if ((rc = grid_for((npairs + kBlock - 1) / kBlock, &grid))) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (aligned(E_true, 16) && aligned(P_out, 16))
+        prob_kernel<true><<<grid, kBlock, 0, st>>>(a, E_true, n, P_out);
+    else
+        prob_kernel<false><<<grid, kBlock, 0, st>>>(a, E_true, n, P_out);
+    return post_launch("osc_prob");
+}
+
+int osc_prob_all(const double* E_true, size_t n, int antinu, double* P_out, void* stream)
+{
+    int rc;
+    if (antinu != 0 && antinu != 1) return fail(OSC_ERR_INVALID_ARG, "antinu must be 0 or 1");
+    HostSet h;
+    if ((rc = snapshot(h))) return rc;
+    if (n == 0) return OSC_OK;
+    if (!E_true || !P_out) return fail(OSC_ERR_INVALID_ARG, "null array with n > 0");
+    if (!aligned(E_true, 8) || !aligned(P_out, 8)) return fail(OSC_ERR_ALIGNMENT, "fp64 array not 8-byte aligned");
+    ProbAllArgs a;
+    a.set = h.set;
+    for (int beta = 0; beta < 2; ++beta)
+        for (int alpha = 0; alpha < 2; ++alpha) a.tr[2 * beta + alpha] = make_trans(h, alpha, beta, antinu);
+    int grid = 1;
+    if ((rc = grid_for((n + 2 * kBlock - 1) / (2 * kBlock), &grid))) return rc;
+    prob_all_kernel<<<grid, kBlock, 0, static_cast<cudaStream_t>(stream)>>>(a, E_true, n, P_out);
+    return post_launch("osc_prob_all");
+}
+
+int osc_reweight_bin(const double* E_true, const double* E_reco, const double* w0, const int8_t* channel, size_t n,
+                     double energy_scale, const double* bin_edges, int n_bins, double* hist_out, void* stream)
+{
+    int rc = check_bin_args(E_true, E_reco, w0, channel, n, energy_scale, bin_edges, n_bins, hist_out);
+    if (rc) return rc;
+    if (n > 0 && !w0) return fail(OSC_ERR_INVALID_ARG, "null w0 with n > 0");
+    if (!aligned(hist_out, 8)) return fail(OSC_ERR_ALIGNMENT, "hist_out not 8-byte aligned");
+    HostSet h;
+    if ((rc = snapshot(h))) return rc;
+    BinArgs args;
+    make_bin_args(h, args);
+    return launch_reweight(args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges, n_bins, hist_out,
+                           static_cast<cudaStream_t>(stream));
+}
+
+int osc_reweight_bin_batch(const osc_params* points, int n_points, const double* E_true, const double* E_reco,
+                           const double* w0, const int8_t* channel, size_t n, double energy_scale,
+                           const double* bin_edges, int n_bins, double* hist_out, void* stream)
+{
+    if (n_points < 0) return fail(OSC_ERR_INVALID_ARG, "n_points < 0");
+    if (n_points == 0) return OSC_OK;
+    if (!points) return fail(OSC_ERR_INVALID_ARG, "null points with n_points > 0");
+    int rc = check_bin_args(E_true, E_reco, w0, channel, n, energy_scale, bin_edges, n_bins, hist_out);
+    if (rc) return rc;
+    if (n > 0 && !w0) return fail(OSC_ERR_INVALID_ARG, "null w0 with n > 0");
+    if (!aligned(hist_out, 8)) return fail(OSC_ERR_ALIGNMENT, "hist_out not 8-byte aligned");
+    for (int p = 0; p < n_points; ++p)
+        if (const char* msg = check_params(points[p]))
+            return fail(OSC_ERR_INVALID_ARG, "osc_reweight_bin_batch: point %d: %s", p, msg);
+    const size_t nh = (size_t)kChannels * n_bins;
+    for (int p = 0; p < n_points; ++p) {
+        HostSet h;
+        precompute(points[p], h);
+        BinArgs args;
+        make_bin_args(h, args);
+        rc = launch_reweight(args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges, n_bins,
+                             hist_out + (size_t)p * nh, static_cast<cudaStream_t>(stream));
+        if (rc) return rc;
+    }
+    return OSC_OK;
+}
+
+int osc_bin_index(const double* E_true, const double* E_reco, const int8_t* channel, size_t n, double energy_scale,
+                  const double* bin_edges, int n_bins, int32_t* bin_out, void* stream)
+{
+    int rc = check_bin_args(E_true, E_reco, E_true, channel, n, energy_scale, bin_edges, n_bins, bin_out);
+    if (rc) return rc;
+    if (n == 0) return OSC_OK;
+    int grid = 1;
+    if ((rc = grid_for((n + kBlock - 1) / kBlock, &grid))) return rc;
+    const size_t smem = sizeof(unsigned long long) * (size_t)(n_bins + 1);
+    bin_index_kernel<<<grid, kBlock, smem, static_cast<cudaStream_t>(stream)>>>(E_true, E_reco, channel, n, energy_scale,
+                                                                              bin_edges, n_bins, bin_out);
+    return post_launch("osc_bin_index");
+}
+
+int osc_prob_host(const double* E_true_host, size_t n, int flavour_in, int flavour_out, int antinu,
+                  double* P_out_host)
+{
+    if (n > 0 && (!E_true_host || !P_out_host)) return fail(OSC_ERR_INVALID_ARG, "null host array with n > 0");
+    std::lock_guard<std::mutex> lk(g_host.mu);
+    const size_t bytes = round_up(n * sizeof(double), 256);
+    int rc = g_host.ensure(2 * bytes + 256);
+    if (rc) return rc;
+    double* dE = reinterpret_cast<double*>(g_host.buf);
+    double* dP = reinterpret_cast<double*>(g_host.buf + bytes);
+    if (n) CUDA_TRY(cudaMemcpyAsync(dE, E_true_host, n * sizeof(double), cudaMemcpyHostToDevice, g_host.stream));
+    rc = osc_prob(dE, n, flavour_in, flavour_out, antinu, dP, g_host.stream);
+    if (rc) return rc;
+    if (n) CUDA_TRY(cudaMemcpyAsync(P_out_host, dP, n * sizeof(double), cudaMemcpyDeviceToHost, g_host.stream));
+    CUDA_TRY(cudaStreamSynchronize(g_host.stream));
+    return OSC_OK;
+}
+
+int osc_reweight_bin_host(const double* E_true_host, const double* E_reco_host, const double* w0_host,
+                          const int8_t* channel_host, size_t n, double energy_scale, const double* bin_edges_host,
+                          int n_bins, double* hist_out_host)
+{
+    if (n_bins < 1 || n_bins > kMaxBins) return fail(OSC_ERR_INVALID_ARG, "n_bins = %d outside [1, %d]", n_bins, kMaxBins);
+    if (!bin_edges_host || !hist_out_host) return fail(OSC_ERR_INVALID_ARG, "null bin_edges or hist_out");
+    if (n > 0 && (!E_true_host || !E_reco_host || !w0_host || !channel_host))
+        return fail(OSC_ERR_INVALID_ARG, "null host array with n > 0");
+    std::lock_guard<std::mutex> lk(g_host.mu);
+    const size_t b8 = round_up(n * sizeof(double), 256);
+    const size_t b1 = round_up(n, 256);
+    const size_t be = round_up((size_t)(n_bins + 1) * sizeof(double), 256);
+    const size_t bh = round_up((size_t)kChannels * n_bins * sizeof(double), 256);
+    int rc = g_host.ensure(3 * b8 + b1 + be + bh + 256);
+    if (rc) return rc;
+    char* p = g_host.buf;
+    double* dEt = reinterpret_cast<double*>(p);
+    double* dEr = reinterpret_cast<double*>(p + b8);
+    double* dW = reinterpret_cast<double*>(p + 2 * b8);
+    int8_t* dC = reinterpret_cast<int8_t*>(p + 3 * b8);
+    double* dEdges = reinterpret_cast<double*>(p + 3 * b8 + b1);
+    double* dH = reinterpret_cast<double*>(p + 3 * b8 + b1 + be);
+    cudaStream_t st = g_host.stream;
+    if (n) {
+        CUDA_TRY(cudaMemcpyAsync(dEt, E_true_host, n * sizeof(double), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(cudaMemcpyAsync(dEr, E_reco_host, n * sizeof(double), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(cudaMemcpyAsync(dW, w0_host, n * sizeof(double), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(cudaMemcpyAsync(dC, channel_host, n, cudaMemcpyHostToDevice, st));
+    }
+    CUDA_TRY(cudaMemcpyAsync(dEdges, bin_edges_host, (size_t)(n_bins + 1) * sizeof(double), cudaMemcpyHostToDevice, st));
+    rc = osc_reweight_bin(dEt, dEr, dW, dC, n, energy_scale, dEdges, n_bins, dH, st);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpyAsync(hist_out_host, dH, (size_t)kChannels * n_bins * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return OSC_OK;
+}
+
+const char* osc_last_error(void) { return t_err; }
+
+unsigned long long osc_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+const char* osc_version(void) { return "osc_b200 0.1 (sm_100a)"; }
+
+int osc_set_device(int device)
+{
+    CUDA_TRY(cudaSetDevice(device));
+    return OSC_OK;
+}
+
+int osc_get_device(int* device)
+{
+    if (!device) return fail(OSC_ERR_INVALID_ARG, "null device pointer");
+    CUDA_TRY(cudaGetDevice(device));
+    return OSC_OK;
+}
+
+int osc_fp64_peak_probe(int iters, int blocks_per_sm, double* flops_per_launch, void* stream)
+{
+    if (iters < 1 || blocks_per_sm < 1 || blocks_per_sm > 8) return fail(OSC_ERR_INVALID_ARG, "bad probe arguments");
+    int sms = 0;
+    int rc = sm_count(&sms);
+    if (rc) return rc;
+    static double* sink = nullptr;
+    if (!sink) CUDA_TRY(cudaMalloc((void**)&sink, 64));
+    const int grid = sms * blocks_per_sm;
+    dfma_probe_kernel<<<grid, kBlock, 0, static_cast<cudaStream_t>(stream)>>>(sink, iters, 1.0);
+    if (flops_per_launch) *flops_per_launch = 2.0 * 8.0 * (double)iters * (double)kBlock * (double)grid;
+    return post_launch("osc_fp64_peak_probe");
+}
+
+} // extern "C"

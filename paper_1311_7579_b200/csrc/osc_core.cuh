@@ -1,0 +1,137 @@
+// osc_core.cuh -- the per-event closed form shared by all kernels (rows a2a-a2f of SURVEY.md 8(a)).
+//
+// Matter Hamiltonian in the flavour basis (eV^2): T = M + A e e^dagger, M = U diag(m^2) U^dagger,
+// A = +-K_MATTER Y_E rho E (A3, A6).  With eigenvalues lam0 >= lam1 >= lam2 and
+// the global phase exp(-i lam0 x) dropped (x = K_PHASE L / E),
+//
+//     S' = E1 I - a P0 + b P2,   E1 = exp(i g01 x),  a = E1 - 1,  b = exp(i g02 x) - E1,
+//     P0 = (T - lam1)(T - lam2) / (g01 g02),          P2 = (T - lam0)(T - lam1) / (g02 g12),
+//
+// g_ij = lam_i - lam_j >= 0.  a/g01 and b/g12 are sinc-like and finite when a gap closes, so nothing
+// here divides by a small gap.  Dropping one more common phase,
+//
+//     Z = delta e^{i h1} - i kap0 N0 + i kap2 e^{i h02} N2,     P(alpha -> beta) = |Z_{beta alpha}|^2,
+//     h1 = g01 x / 2, h12 = g12 x / 2, h02 = h1 + h12,
+//     kap0 = 2 sin(h1) / (g01 g02),  kap2 = 2 sin(h12) / (g12 g02),
+//     N0 = T^2 - (lam1 + lam2) T + lam1 lam2 I,  N2 = T^2 - (lam0 + lam1) T + lam0 lam1 I.
+//
+// The eigenvalues come from the trigonometric solution of the characteristic cubic
+// lam^3 - c2 lam^2 + c1 lam - c0 (BASELINE.json:north_star item 2): lam_k = c2/3 + (2/3) R tau_k with
+// R^2 = c2^2 - 3 c1 and tau the roots of 4 tau^3 - 3 tau = u, u = (2 c2^3 - 9 c2 c1 + 27 c0)/(2 R^3).
+// Only |u| is solved (largest root t, osc_math.cuh); for u < 0 the roots are negated and reversed.
+#pragma once
+#include "osc_math.cuh"
+#include "osc_types.h"
+
+namespace oscb {
+
+struct OscEig {
+    double c1h, s1h;       // cos, sin of h1
+    double c02, s02;       // cos, sin of h02
+    double kap0, kap2;
+    double sum12, prod12;  // lam1 + lam2, lam1 lam2
+    double sum01, prod01;  // lam0 + lam1, lam0 lam1
+};
+
+__device__ __forceinline__ double select_d(bool c, double a, double b) { return c ? a : b; }
+
+// Rows a2a-a2d: eigenvalues, gap phases and the two sinc-like factors for matter term A at 1/E.
+__device__ __forceinline__ void eig_solve(const OscSet& ps, double A, double invE, OscEig& o)
+{
+    const double SQ3 = 1.7320508075688772;
+    const double HALF_SQ3 = 0.8660254037844386;
+
+    // a2b characteristic polynomial
+    double c2 = A + ps.tr;
+    double c1 = fma(A, ps.k1, ps.dd);
+    double c0_27 = A * ps.k0_27;
+    double c1_3 = 3.0 * c1;
+    double R2 = fma(c2, c2, -c1_3);
+    R2 = fmax(R2, 1e-60);                       // T proportional to I cannot be solved; keep finite
+    double tq = fma(2.0, R2, -c1_3);            // 2 c2^2 - 9 c1
+    double q = fma(c2, tq, c0_27);              // 2 c2^3 - 9 c2 c1 + 27 c0
+
+    // a2c trigonometric cubic
+    double rinv = rsqrt_pos(R2);
+    double rinv2 = rinv * rinv;
+    double U2 = (q * rinv) * rinv2;             // 2 u = 2 cos(3 phi)
+    bool neg = __double2hiint(U2) < 0;
+    double t, rh;
+    cos_third_acos(fabs(U2), t, rh);            // t = cos(phi'), rh = 1 / (24 t^2 - 6)
+    double om = 1.0 - t;
+    double w = fma(om, t, om);                  // 1 - t^2 = sin^2(phi')
+    w = fmax(w, 1e-30);
+    double y = rsqrt_pos(w);
+    double s = w * y;                           // sin(phi')
+    double ga = fma(-HALF_SQ3, s, 1.5 * t);     // gaps in units of (2/3) R:  ga >= gb, ga + gb = largest gap
+    double gb = SQ3 * s;
+    double m = fma(HALF_SQ3, s, 0.5 * t);
+    double tau0 = select_d(neg, m, t);
+    double tau2 = select_d(neg, -t, -m);
+
+    double R = R2 * rinv;
+    double Rs = R * (2.0 / 3.0);
+    double c2_3 = c2 * (1.0 / 3.0);
+    double lam0 = fma(Rs, tau0, c2_3);
+    double lam2 = fma(Rs, tau2, c2_3);
+    o.sum12 = c2 - lam0;
+    o.prod12 = fma(-lam0, o.sum12, c1);
+    o.sum01 = c2 - lam2;
+    o.prod01 = fma(-lam2, o.sum01, c1);
+
+    // 1/(g_small_pair g02) and 1/(g_big_pair g02): ga (ga + gb) = 3 t^2 - 3/4 = (24 t^2 - 6) / 8
+    double rr = rh * rinv2;
+    double ka = 36.0 * rr;                                  // 2 / (Rs^2 ga gc)
+    double kb = (rr * (36.0 / SQ3)) * (ga * y);             // 2 / (Rs^2 gb gc)
+
+    // a2d gap phases in quarter turns
+    double RX = R * (ps.xq23 * invE);
+    double hqa = ga * RX, hqb = gb * RX;
+    double hq1 = select_d(neg, hqb, hqa);
+    double hq12 = select_d(neg, hqa, hqb);
+    double s1, c1c, s12, c12;
+    sincos_quarter(hq1, s1, c1c);
+    sincos_quarter(hq12, s12, c12);
+    o.s1h = s1;
+    o.c1h = c1c;
+    o.c02 = fma(c1c, c12, -(s1 * s12));
+    o.s02 = fma(s1, c12, c1c * s12);
+    o.kap0 = s1 * select_d(neg, kb, ka);
+    o.kap2 = s12 * select_d(neg, ka, kb);
+}
+
+// Rows a2e-a2f: |Z_{beta alpha}|^2 for one transition.
+__device__ __forceinline__ double assemble(const OscEig& e, double A, const OscTrans& tr)
+{
+    double Tr = fma(A, tr.ee, tr.Tr0);
+    double Ti = tr.Ti0;
+    double T2r = fma(A, fma(A, tr.ee, tr.T2r1), tr.T2r0);
+    double T2i = fma(A, tr.T2i1, tr.T2i0);
+    double N0r = fma(e.prod12, tr.delta, fma(-e.sum12, Tr, T2r));
+    double N0i = fma(-e.sum12, Ti, T2i);
+    double N2r = fma(e.prod01, tr.delta, fma(-e.sum01, Tr, T2r));
+    double N2i = fma(-e.sum01, Ti, T2i);
+    double Wr = fma(e.c02, N2r, -(e.s02 * N2i));
+    double Wi = fma(e.s02, N2r, e.c02 * N2i);
+    double Zr = fma(tr.delta, e.c1h, fma(e.kap0, N0i, -(e.kap2 * Wi)));
+    double Zi = fma(tr.delta, e.s1h, fma(e.kap2, Wr, -(e.kap0 * N0r)));
+    return fma(Zr, Zr, Zi * Zi);
+}
+
+// A11: usable energy <=> finite and > 0 <=> 0 < bits < 0x7FF0000000000000 (integer pipe).
+__device__ __forceinline__ bool energy_ok(double E)
+{
+    unsigned long long b = (unsigned long long)__double_as_longlong(E);
+    return (b - 1ull) < 0x7FEFFFFFFFFFFFFFull;
+}
+
+__device__ __forceinline__ double prob_one(const OscSet& ps, const OscTrans& tr, double E)
+{
+    double invE = rcp_pos(E);
+    double A = tr.sa * E;
+    OscEig e;
+    eig_solve(ps, A, invE, e);
+    return assemble(e, A, tr);
+}
+
+} // namespace oscb

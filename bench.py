@@ -1,0 +1,350 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the oscillation-reweighting hot path on B200 (contract: see DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--events n]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+Workload (BASELINE.json configs[2], the one the metric "oscillation-reweighted events/s" is quoted on): per GPU
+1e7 synthetic events (E_true, E_reco, w0 fp64 + channel int8, 250 MB > L2) in 4 channels, Table 1 parameters; one
+STEP = osc_set_params (row a1) followed by osc_reweight_bin (rows a2a-a3c fused) for each of the three energy-scale
+values {0.97, 1.00, 1.03}, i.e. three full reweight-and-histogram passes over the events.  value = event
+reweightings per second = N_gpus * n * 3 * K / time.  With N > 1 every rank holds its own n events (weak scaling) and
+the partial histograms are summed with one NCCL all-reduce per step.
+
+rank 0 prints ONE JSON line.  --impl reference times the CPU oracle (test infrastructure) on a bounded sample of the
+same workload; it is a deliberately slow program and its number is a reported baseline, not a target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1311_7579_b200 import workloads as wl  # noqa: E402  (no method arithmetic in there)
+
+METRIC = "fp64 oscillation-reweighted events/sec"
+UNIT = "events/s"
+N_EVENTS = 10_000_000
+SCALES = wl.ENERGY_SCALES
+BYTES_PER_EVENT = 25          # E_true + E_reco + w0 (fp64) + channel (int8): SURVEY.md 8(d), DESIGN.md "k2"
+# fp64 operations the closed form executes per event in k2 (DFMA = 2, DADD/DMUL = 1), counted from the SASS of the
+# shipped kernel's event loop: DESIGN.md "k2: operation budget".
+FLOP_PER_EVENT = 201.0
+FP64_LANES_PER_SM_CLK = 64    # B200 (sm_100): 4 sub-partitions x 16 fp64 lanes; DESIGN.md "fp64 roofline"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--events", type=int, default=N_EVENTS, help="events per GPU (default: configs[2], 1e7)")
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons during the timed region (B200_PROFILING.md 'clocks line')."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, reasons, power = [], [], set(), []
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        rows = [r for (t, r) in self.rows if t0 - 0.05 <= t <= t1 + 0.15] or [r for (_, r) in self.rows]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                smax.append(float(f[1]))
+                power.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_rate(n_target_seconds: float = 15.0):
+    """Oracle (as it stands) on a bounded sample of the configs[2] workload; events/s over all host cores."""
+    import oracle
+
+    oracle.build()
+    par = oracle.Params(**wl.table1())
+    edges = wl.bin_edges()
+    cores = oracle.threads()
+    probe_n = 20_000
+    ev = wl.events(probe_n, seed=2)
+    t = time.perf_counter()
+    oracle.reweight_bin(par, *ev, 1.0, edges)
+    rate = probe_n / max(time.perf_counter() - t, 1e-9)
+    n = int(min(max(rate * n_target_seconds / len(SCALES), 10_000), 2_000_000))
+    ev = wl.events(n, seed=2)
+    t = time.perf_counter()
+    for s in SCALES:
+        oracle.reweight_bin(par, *ev, s, edges)
+    dt = time.perf_counter() - t
+    return {"value": n * len(SCALES) / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {n} events of the configs[2] arrays (seed 2) x {len(SCALES)} energy scales, "
+                      f"long-double Jacobi oracle, OpenMP over events, {dt:.1f} s"}, n, dt
+
+
+def run_reference(args):
+    """The oracle timed on the host cores: K steps, each a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+
+    oracle.build()
+    par = oracle.Params(**wl.table1())
+    edges = wl.bin_edges()
+    cores = oracle.threads()
+    ev = wl.events(20_000, seed=2)
+    t = time.perf_counter()
+    oracle.reweight_bin(par, *ev, 1.0, edges)
+    rate = 20_000 / max(time.perf_counter() - t, 1e-9)
+    total_steps = max(args.steps + args.warmup, 1)
+    n = int(min(max(rate * 60.0 / (len(SCALES) * total_steps), 2_000), 1_000_000))   # whole run ~1 minute
+    ev = wl.events(n, seed=2)
+    for _ in range(args.warmup):
+        for s in SCALES:
+            oracle.reweight_bin(par, *ev, s, edges)
+    t = time.perf_counter()
+    for _ in range(args.steps):
+        for s in SCALES:
+            oracle.reweight_bin(par, *ev, s, edges)
+    dt = time.perf_counter() - t
+    value = n * len(SCALES) * args.steps / dt
+    sample = (f"each step = first {n} events of the configs[2] arrays (seed 2) x {len(SCALES)} energy scales; "
+              f"long-double Jacobi oracle with OpenMP over events")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64 (long double inside the oracle)", "data": "synthetic",
+        "config": {"workload": "configs[2] bounded sample: 4 channels, 50 bins, 3 energy scales, Table 1 parameters",
+                   "events_per_step": n, "passes_per_step": len(SCALES)},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_1311_7579_b200 as osc   # raises if libosc_b200.so is missing: no fallback
+    from paper_1311_7579_b200 import build as _build
+
+    _build.build_library()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        if world == 1 and args.gpus > 1:
+            raise SystemExit("launch with torch.distributed.run --nproc-per-node N for --gpus N")
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    osc.osc_set_device(local)
+    device = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+
+    n = args.events
+    par = wl.table1()
+    et, er, w0, ch = wl.events(n, seed=2 + 1000 * rank)          # each rank its own shard (weak scaling)
+    edges = wl.bin_edges()
+    # pinned host copies (e2e leg) and device-resident copies (value leg)
+    h_et, h_er, h_w0, h_ch = (torch.from_numpy(a).pin_memory() for a in (et, er, w0, ch))
+    d_et, d_er, d_w0, d_ch = (t.to(device) for t in (h_et, h_er, h_w0, h_ch))
+    d_edges = torch.from_numpy(edges).to(device)
+    hist = torch.zeros((len(SCALES), osc.N_CHANNELS, wl.N_BINS), dtype=torch.float64, device=device)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        osc.osc_set_params(**par)                                                           # a1
+        for k, s in enumerate(SCALES):
+            osc.osc_reweight_bin(d_et, d_er, d_w0, d_ch, s, d_edges, hist_out=hist[k])      # a2a-a3c
+        if world > 1:
+            dist.all_reduce(hist)                                                           # 8(e)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+
+    # ---- timed region: device-resident inputs -----------------------------------------------------------------
+    sampler = ClockSampler(local) if rank == 0 else None
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = osc.osc_launch_count()
+    barrier()
+    t_wall0 = time.time()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    barrier()
+    t_wall1 = time.time()
+    launches = osc.osc_launch_count() - launches0
+    ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+    t_ms = torch.tensor([ms], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
+    ms = float(t_ms.item())
+    value = world * n * len(SCALES) * args.steps / (ms * 1e-3)
+
+    # ---- dominant kernel alone (k2), CUDA events per launch, for the roofline ----------------------------------
+    osc.osc_set_params(**par)
+    reps = 30
+    ks, ke = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ks.record(stream)
+    for i in range(reps):
+        osc.osc_reweight_bin(d_et, d_er, d_w0, d_ch, SCALES[i % 3], d_edges, hist_out=hist[i % 3])
+    ke.record(stream)
+    torch.cuda.synchronize()
+    k_ms = ks.elapsed_time(ke) / reps
+
+    # ---- fp64 peak probe in the same run (DFMA-only, register resident) ----------------------------------------
+    probe_flops = osc.osc_fp64_peak_probe(1 << 14, 4)
+    torch.cuda.synchronize()
+    ps, pe = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ps.record(stream)
+    for _ in range(5):
+        osc.osc_fp64_peak_probe(1 << 14, 4)
+    pe.record(stream)
+    torch.cuda.synchronize()
+    fp64_peak_tflops = 5 * probe_flops / (ps.elapsed_time(pe) * 1e-3) / 1e12
+
+    # ---- e2e: same step through the C ABI with HOST buffers (H2D and D2H inside the timed region) ---------------
+    e2e = None
+    if not args.no_e2e:
+        np_in = [t.numpy() for t in (h_et, h_er, h_w0, h_ch)]
+        h_hist = torch.zeros((len(SCALES), osc.N_CHANNELS, wl.N_BINS), dtype=torch.float64).pin_memory()
+        np_hist = h_hist.numpy()
+
+        def step_host():
+            osc.osc_set_params(**par)
+            for k, s in enumerate(SCALES):
+                osc.osc_reweight_bin_host(*np_in, s, edges, hist_out=np_hist[k])
+
+        for _ in range(2):
+            step_host()
+        barrier()
+        e_steps = max(2, min(args.steps, 5))
+        t0 = time.perf_counter()
+        for _ in range(e_steps):
+            step_host()
+        barrier()
+        e_dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=device)
+        if world > 1:
+            dist.all_reduce(e_dt, op=dist.ReduceOp.MAX)
+        h2d = len(SCALES) * (n * BYTES_PER_EVENT + edges.nbytes)
+        d2h = len(SCALES) * osc.N_CHANNELS * wl.N_BINS * 8
+        e2e = {"value": world * n * len(SCALES) * e_steps / float(e_dt.item()), "unit": UNIT,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e_steps,
+               "api": "osc_reweight_bin_host (pinned host buffers, one call per energy scale)"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    hbm_peak, peak_src = peaks()
+    sm_count = torch.cuda.get_device_properties(device).multi_processor_count
+    sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
+    nominal_tflops = sm_count * FP64_LANES_PER_SM_CLK * 2 * sm_max * 1e6 / 1e12
+    achieved_tflops = n * FLOP_PER_EVENT / (k_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "achieved": achieved_tflops, "peak": fp64_peak_tflops, "unit": "TFLOP/s",
+                "frac": achieved_tflops / fp64_peak_tflops, "traffic": None,
+                "kernel": "reweight_bin_kernel (k2)", "kernel_ms": k_ms,
+                "flop_per_event": FLOP_PER_EVENT,
+                "peak_source": "DFMA-only probe kernel measured in this run (osc_fp64_peak_probe)",
+                "nominal_peak": nominal_tflops,
+                "hbm": {"achieved": n * BYTES_PER_EVENT / (k_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                        "frac": n * BYTES_PER_EVENT / (k_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": peak_src}}
+
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        cpu, _, _ = oracle_rate()
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[2]: 1e7 events/GPU x 4 channels, 50-bin E_reco histograms over 0-5 GeV, "
+                               "energy scales {0.97,1.00,1.03}, Table 1 parameters (normal hierarchy)",
+                   "events_per_gpu": n, "passes_per_step": len(SCALES), "n_bins": wl.N_BINS,
+                   "l2": "inputs (250 MB per pass) larger than L2 (126 MB); no explicit flush",
+                   "parallelism": f"events sharded over {world} GPU(s); histogram all-reduce" if world > 1 else "1 GPU"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+    }
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -39,9 +39,10 @@ __global__ void __launch_bounds__(kBlock)
 prob_kernel(const __grid_constant__ ProbArgs a, const double* __restrict__ E_true, size_t n,
             double* __restrict__ P_out)
 {
-    const size_t npairs = (n + 1) / 2;
+    // VEC: slot i holds events (2i, 2i+1); otherwise tile i / kBlock holds events j0 and j0 + kBlock
+    const size_t nslots = VEC ? (n + 1) / 2 : ((n + 2 * kBlock - 1) / (2 * kBlock)) * kBlock;
     const size_t stride = (size_t)gridDim.x * kBlock;
-    for (size_t i = (size_t)blockIdx.x * kBlock + threadIdx.x; i < npairs; i += stride) {
+    for (size_t i = (size_t)blockIdx.x * kBlock + threadIdx.x; i < nslots; i += stride) {
         const size_t j0 = VEC ? 2 * i : (i / kBlock) * (2 * kBlock) + (i % kBlock);
         const size_t j1 = VEC ? j0 + 1 : j0 + kBlock;
         const bool has1 = j1 < n;

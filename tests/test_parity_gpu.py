@@ -1,0 +1,477 @@
+"""GPU-vs-oracle parity (SURVEY.md section 4 tier T2/T3/T4), through the C ABI, on a B200.
+
+Bars (BASELINE.json:north_star): every fp64 probability within 1e-10 absolute of the oracle, every
+fp64 histogram bin within 1e-9 relative, integer bin indices bit-exact.  Inputs are the seeded arrays
+of paper_1311_7579_b200.workloads, handed byte-identical to both sides.  No expected value here comes
+from the CUDA path.
+"""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1311_7579_b200 import workloads as wl
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+P_ABS = 1e-10     # north_star: absolute, per probability
+H_REL = 1e-9      # north_star: relative, per histogram bin
+H_ZERO = 1e-25    # see assert_hist_close
+
+
+@pytest.fixture(scope="module")
+def osc():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1311_7579_b200 import build
+
+    build.build_library()
+    import paper_1311_7579_b200 as m
+
+    torch.cuda.set_device(0)
+    m.osc_set_device(0)
+    return m
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def host(t):
+    return t.cpu().numpy()
+
+
+def assert_prob_close(got, ref, what=""):
+    assert got.shape == ref.shape
+    assert np.array_equal(np.isnan(got), np.isnan(ref)), f"{what}: NaN pattern differs"
+    m = ~np.isnan(ref)
+    err = float(np.max(np.abs(got[m] - ref[m]))) if m.any() else 0.0
+    assert err <= P_ABS, f"{what}: max |dP| = {err:.3e} > {P_ABS}"
+    return err
+
+
+def assert_hist_close(got, ref, what=""):
+    """1e-9 relative on every bin.  Bins no event falls into are exactly 0.0 on both sides.  H_ZERO keeps the
+    relative bar meaningful where the probability itself is a computed zero (e.g. P(numu->nue) at L = 0: the
+    oracle's long-double rounding leaves ~1e-39 where the closed form gives exactly 0): it is 25 orders below
+    any event weight of these workloads."""
+    assert got.shape == ref.shape
+    assert np.all(got[ref == 0.0] == 0.0), f"{what}: a bin the oracle leaves empty is not 0.0"
+    assert np.all(np.isfinite(got)), f"{what}: non-finite bin"
+    err = np.abs(got - ref)
+    bad = err > H_REL * np.abs(ref) + H_ZERO
+    nz = np.abs(ref) > H_ZERO
+    rel = float(np.max(err[nz] / np.abs(ref[nz]))) if nz.any() else 0.0
+    assert not bad.any(), f"{what}: max rel bin error {rel:.3e} > {H_REL}"
+    return rel
+
+
+def set_params(osc, par):
+    osc.osc_set_params(**par)
+    return oracle.Params(**par)
+
+
+# ------------------------------------------------------------------------------------------------
+# configs[0]: 1e5 events, Table 1, P(numu->numu) and P(numu->nue)
+# ------------------------------------------------------------------------------------------------
+def test_config0(osc):
+    E = wl.e_true(100_000, seed=0)
+    op = set_params(osc, wl.table1())
+    dE = dev(E)
+    for fin, fout in ((1, 1), (1, 0)):
+        got = host(osc.osc_prob(dE, fin, fout, 0))
+        assert_prob_close(got, oracle.prob(op, E, fin, fout, 0), f"config0 {fin}->{fout}")
+
+
+# ------------------------------------------------------------------------------------------------
+# configs[1] at a size the oracle finishes in seconds: all 9 transitions x nu/nubar, 4 delta draws x
+# both hierarchies; several tiles and a ragged tail
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("run", range(8))
+def test_config1_all_transitions(osc, run):
+    par = wl.config1_runs()[run]
+    n = 40_000 + 2 * 256 * 3 + 131
+    E = wl.e_true(n, seed=1)
+    op = set_params(osc, par)
+    dE = dev(E)
+    for anti in (0, 1):
+        got = host(osc.osc_prob_all(dE, anti))
+        assert_prob_close(got, oracle.prob_all(op, E, anti), f"config1 run {run} anti {anti}")
+        s = got.reshape(3, 3, n)
+        assert np.max(np.abs(s.sum(axis=0) - 1.0)) < 1e-12   # unitarity of what was written
+        assert np.max(np.abs(s.sum(axis=1) - 1.0)) < 1e-12
+        assert got.min() >= 0.0
+
+
+def test_single_transition_equals_all(osc):
+    par = wl.config1_runs()[3]
+    E = wl.e_true(6_001, seed=11)
+    op = set_params(osc, par)
+    dE = dev(E)
+    for anti in (0, 1):
+        ref = oracle.prob_all(op, E, anti)
+        for a in range(3):
+            for b in range(3):
+                got = host(osc.osc_prob(dE, a, b, anti))
+                assert_prob_close(got, ref[3 * b + a], f"{a}->{b} anti {anti}")
+
+
+# ------------------------------------------------------------------------------------------------
+# configs[4] parameter settings: rho x L x hierarchy, and harder corners (degenerate spectra, L = 0,
+# large density, resonance)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("k", range(12))
+def test_sweep_settings_prob(osc, k):
+    par = wl.sweep_settings()[k]
+    E = wl.e_true(20_000, seed=40 + k)
+    op = set_params(osc, par)
+    dE = dev(E)
+    for anti in (0, 1):
+        assert_prob_close(host(osc.osc_prob_all(dE, anti)), oracle.prob_all(op, E, anti), f"sweep {k} anti {anti}")
+
+
+CORNERS = [
+    dict(rho_g_cm3=0.0, dm2_21=0.0, sin2_th13=0.0),               # exactly degenerate pair in vacuum (P3)
+    dict(rho_g_cm3=2.6, dm2_21=0.0, sin2_th13=0.0),               # degenerate pair in matter
+    dict(rho_g_cm3=2.6, dm2_21=0.0),                              # one mass scale (P7)
+    dict(rho_g_cm3=2.6, sin2_th13=0.0),                           # solar sector only (P8)
+    dict(L_km=0.0),                                               # P = delta (P5)
+    dict(rho_g_cm3=50.0, L_km=1300.0),                            # large density
+    dict(rho_g_cm3=100.0, L_km=2000.0, hierarchy=-1),
+    dict(rho_g_cm3=12.0, L_km=1300.0, delta_cp=1.3),              # atmospheric resonance inside 0.1-10 GeV
+    dict(sin2_th12=0.0, sin2_th13=0.0, sin2_th23=0.0),            # U = 1
+    dict(sin2_th12=1.0, sin2_th13=1.0, sin2_th23=1.0, delta_cp=-2.0),
+    dict(sin2_th23=0.3, delta_cp=-math.pi / 2, hierarchy=-1, L_km=1300.0),
+    dict(dm2_32=1e-3, dm2_21=9.9e-4, delta_cp=2.5),               # comparable splittings
+    dict(dm2_32=2.4e-3, dm2_21=2.4e-3, hierarchy=-1),             # inverted: dm2_31 = 0 -> m1 = m3 degenerate
+]
+
+
+@pytest.mark.parametrize("k", range(len(CORNERS)))
+def test_corner_parameters(osc, k):
+    par = wl.table1(**CORNERS[k])
+    E = np.concatenate([wl.e_true(5_000, seed=60 + k), np.geomspace(0.1, 10.0, 1_237)])
+    op = set_params(osc, par)
+    dE = dev(E)
+    for anti in (0, 1):
+        assert_prob_close(host(osc.osc_prob_all(dE, anti)), oracle.prob_all(op, E, anti), f"corner {k} anti {anti}")
+        for fin, fout in ((1, 1), (1, 0), (0, 0), (2, 1)):
+            assert_prob_close(host(osc.osc_prob(dE, fin, fout, anti)), oracle.prob(op, E, fin, fout, anti),
+                              f"corner {k} {fin}->{fout} anti {anti}")
+
+
+def test_random_parameter_sets(osc):
+    rng = np.random.Generator(np.random.PCG64(77))
+    E = np.concatenate([wl.e_true(1_500, seed=78), np.geomspace(0.1, 10.0, 500)])
+    dE = dev(E)
+    worst = 0.0
+    for _ in range(60):
+        par = dict(sin2_th12=rng.uniform(0, 1), sin2_th23=rng.uniform(0, 1), sin2_th13=rng.uniform(0, 1),
+                   dm2_32=10 ** rng.uniform(-4, -2), dm2_21=10 ** rng.uniform(-6, -3),
+                   delta_cp=rng.uniform(-math.pi, math.pi), rho_g_cm3=rng.uniform(0, 15),
+                   L_km=rng.uniform(0, 2000), hierarchy=int(rng.choice([1, -1])))
+        op = set_params(osc, par)
+        for anti in (0, 1):
+            worst = max(worst, assert_prob_close(host(osc.osc_prob_all(dE, anti)), oracle.prob_all(op, E, anti),
+                                                 f"random {par} anti {anti}"))
+    print(f"random parameter sets: worst |dP| = {worst:.3e}")
+
+
+# ------------------------------------------------------------------------------------------------
+# A11: unusable energies, ragged sizes, unaligned slices
+# ------------------------------------------------------------------------------------------------
+def test_bad_energies_give_nan(osc):
+    op = set_params(osc, wl.table1())
+    E = wl.e_true(1_031, seed=5)
+    E[[0, 7, 512, 513, 1030]] = [0.0, -1.0, np.nan, np.inf, -np.inf]
+    E[100] = -0.0
+    dE = dev(E)
+    assert_prob_close(host(osc.osc_prob(dE, 1, 0, 0)), oracle.prob(op, E, 1, 0, 0), "bad energies")
+    assert_prob_close(host(osc.osc_prob_all(dE, 1)), oracle.prob_all(op, E, 1), "bad energies all")
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 31, 32, 33, 255, 256, 257, 511, 512, 513, 1023, 1025, 4097])
+def test_ragged_sizes(osc, n):
+    op = set_params(osc, wl.table1(delta_cp=0.7))
+    E = wl.e_true(n + 1, seed=n)
+    d = dev(E)
+    for off in (0, 1):                      # off = 1: 8-byte aligned only -> scalar path
+        Es = E[off:off + n]
+        o0 = 2 - off                        # off = 0: output 16-byte aligned too -> 128-bit path
+        out = torch.full((n + 4,), -7.0, dtype=torch.float64, device="cuda")
+        osc.osc_prob(d[off:off + n], 1, 1, 0, P_out=out[o0:o0 + n])
+        o = host(out)
+        assert np.all(o[:o0] == -7.0) and np.all(o[o0 + n:] == -7.0), "wrote outside P_out"
+        assert_prob_close(o[o0:o0 + n], oracle.prob(op, Es, 1, 1, 0), f"ragged n={n} off={off}")
+        pa = torch.full((9 * n + 2,), -7.0, dtype=torch.float64, device="cuda")
+        osc.osc_prob_all(d[off:off + n], 0, P_out=pa[1:1 + 9 * n])
+        o = host(pa)
+        assert o[0] == -7.0 and o[-1] == -7.0
+        assert_prob_close(o[1:1 + 9 * n].reshape(9, n), oracle.prob_all(op, Es, 0), f"ragged all n={n}")
+
+
+def test_n_zero(osc):
+    set_params(osc, wl.table1())
+    e = torch.empty(0, dtype=torch.float64, device="cuda")
+    assert osc.osc_prob(e, 1, 1, 0).numel() == 0
+    assert osc.osc_prob_all(e, 0).numel() == 0
+    edges = dev(wl.bin_edges())
+    h = torch.full((4, 50), 3.0, dtype=torch.float64, device="cuda")
+    osc.osc_reweight_bin(e, e, e, torch.empty(0, dtype=torch.int8, device="cuda"), 1.0, edges, hist_out=h)
+    assert float(h.abs().sum()) == 0.0      # overwritten (zeroed) even with no events
+    hb = torch.full((2, 4, 50), 3.0, dtype=torch.float64, device="cuda")
+    osc.osc_reweight_bin_batch([wl.table1(), wl.table1()], e, e, e, torch.empty(0, dtype=torch.int8, device="cuda"),
+                               1.0, edges, hist_out=hb)
+    assert float(hb.abs().sum()) == 0.0
+
+
+# ------------------------------------------------------------------------------------------------
+# configs[2]: fused reweight + histogram; bin indices bit-exact
+# ------------------------------------------------------------------------------------------------
+def test_config2_histograms(osc):
+    n = 300_000 + 2 * 256 * 5 + 77
+    et, er, w0, ch = wl.events(n, seed=2)
+    edges = wl.bin_edges()
+    op = set_params(osc, wl.table1())
+    d = [dev(a) for a in (et, er, w0, ch)]
+    de = dev(edges)
+    for s in wl.ENERGY_SCALES:
+        got = host(osc.osc_reweight_bin(*d, s, de))
+        ref = oracle.reweight_bin(op, et, er, w0, ch, s, edges)
+        assert_hist_close(got, ref, f"config2 s={s}")
+        bi = host(osc.osc_bin_index(d[0], d[1], d[3], s, de))
+        assert np.array_equal(bi, oracle.bin_index(et, er, ch, s, edges)), f"bin indices differ at s={s}"
+
+
+@pytest.mark.parametrize("k", range(12))
+def test_sweep_settings_histograms(osc, k):
+    par = wl.sweep_settings()[k]
+    n = 50_000 + k
+    et, er, w0, ch = wl.events(n, seed=100 + k)
+    edges = wl.bin_edges()
+    op = set_params(osc, par)
+    got = host(osc.osc_reweight_bin(dev(et), dev(er), dev(w0), dev(ch), 1.0, dev(edges)))
+    assert_hist_close(got, oracle.reweight_bin(op, et, er, w0, ch, 1.0, edges), f"sweep hist {k}")
+
+
+def test_bin_index_bit_exact_large_and_edges(osc):
+    n = 1_000_000
+    et, er, w0, ch = wl.events(n, seed=7)
+    edges = wl.bin_edges()
+    # events exactly on edges (upper bin), just below, on the last edge (dropped), negative, NaN, -0.0
+    er[:51] = edges
+    er[51:102] = np.nextafter(edges, -np.inf)
+    er[102:153] = np.nextafter(edges, np.inf)
+    er[153:158] = [np.nan, -0.0, np.inf, -np.inf, -1e-300]
+    et[200:204] = [0.0, -3.0, np.nan, np.inf]
+    ch[300:304] = [-1, 4, 127, -128]
+    set_params(osc, wl.table1())
+    d_et, d_er, d_ch, de = dev(et), dev(er), dev(ch), dev(edges)
+    for s in (0.97, 1.0, 1.03, 1.0 / 3.0, 7.123456789):
+        bi = host(osc.osc_bin_index(d_et, d_er, d_ch, s, de))
+        assert np.array_equal(bi, oracle.bin_index(et, er, ch, s, edges)), f"s={s}"
+
+
+def test_dropped_and_bad_events_are_skipped(osc):
+    n = 20_011
+    et, er, w0, ch = wl.events(n, seed=8)
+    edges = wl.bin_edges()
+    er[:51] = edges
+    er[60:63] = [np.nan, -1.0, 1e9]
+    et[100:104] = [0.0, -3.0, np.nan, np.inf]
+    ch[300:304] = [-1, 4, 127, -128]
+    w0[500] = 0.0
+    op = set_params(osc, wl.table1(delta_cp=-1.0))
+    got = host(osc.osc_reweight_bin(dev(et), dev(er), dev(w0), dev(ch), 1.0, dev(edges)))
+    assert_hist_close(got, oracle.reweight_bin(op, et, er, w0, ch, 1.0, edges), "bad events")
+
+
+@pytest.mark.parametrize("nb,kind", [(1, "uniform"), (2, "uniform"), (3, "log"), (7, "random"), (50, "random"),
+                                     (64, "uniform"), (200, "log"), (768, "uniform")])
+def test_bin_layouts(osc, nb, kind):
+    n = 30_007
+    et, er, w0, ch = wl.events(n, seed=9)
+    rng = np.random.Generator(np.random.PCG64(nb))
+    if kind == "uniform":
+        edges = wl.bin_edges(nb, 5.0)
+    elif kind == "log":
+        edges = np.geomspace(0.05, 6.0, nb + 1)
+    else:
+        edges = np.sort(rng.uniform(-0.5, 5.0, nb + 1))
+        assert np.all(np.diff(edges) > 0)
+    op = set_params(osc, wl.table1())
+    d_et, d_er, d_w, d_ch, de = dev(et), dev(er), dev(w0), dev(ch), dev(edges)
+    got = host(osc.osc_reweight_bin(d_et, d_er, d_w, d_ch, 1.03, de))
+    assert_hist_close(got, oracle.reweight_bin(op, et, er, w0, ch, 1.03, edges), f"nb={nb} {kind}")
+    assert np.array_equal(host(osc.osc_bin_index(d_et, d_er, d_ch, 1.03, de)),
+                          oracle.bin_index(et, er, ch, 1.03, edges))
+
+
+@pytest.mark.parametrize("n", [1, 2, 31, 33, 511, 513, 1025, 5000])
+def test_histogram_ragged_and_unaligned(osc, n):
+    et, er, w0, ch = wl.events(n + 1, seed=300 + n)
+    edges = wl.bin_edges()
+    op = set_params(osc, wl.table1())
+    d = [dev(a) for a in (et, er, w0, ch)]
+    de = dev(edges)
+    for off in (0, 1):
+        got = host(osc.osc_reweight_bin(*[t[off:off + n] for t in d], 1.0, de))
+        ref = oracle.reweight_bin(op, *[a[off:off + n] for a in (et, er, w0, ch)], 1.0, edges)
+        assert_hist_close(got, ref, f"n={n} off={off}")
+
+
+def test_histogram_is_bit_reproducible(osc):
+    n = 400_003
+    et, er, w0, ch = wl.events(n, seed=10)
+    set_params(osc, wl.table1())
+    d = [dev(a) for a in (et, er, w0, ch)]
+    de = dev(wl.bin_edges())
+    a = host(osc.osc_reweight_bin(*d, 1.0, de))
+    for _ in range(3):
+        assert np.array_equal(a, host(osc.osc_reweight_bin(*d, 1.0, de)))
+
+
+# ------------------------------------------------------------------------------------------------
+# configs[3]: batched parameter scan
+# ------------------------------------------------------------------------------------------------
+def test_config3_full_grid_small_sample(osc):
+    pts = wl.scan_points()
+    assert len(pts) == 1024
+    n = 2_003
+    et, er, w0, ch = wl.events(n, seed=3)
+    edges = wl.bin_edges()
+    got = host(osc.osc_reweight_bin_batch(pts, dev(et), dev(er), dev(w0), dev(ch), 1.0, dev(edges)))
+    ref = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 1.0, edges)
+    assert got.shape == (1024, 4, 50)
+    assert_hist_close(got, ref, "config3 grid")
+
+
+def test_config3_diagonal_more_events(osc):
+    pts = wl.scan_points()[::33][:16]
+    n = 60_000 + 19
+    et, er, w0, ch = wl.events(n, seed=3)
+    edges = wl.bin_edges()
+    d = [dev(a) for a in (et, er, w0, ch)]
+    de = dev(edges)
+    got = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, de))
+    ref = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 1.0, edges)
+    assert_hist_close(got, ref, "config3 diagonal")
+
+
+def test_batch_point_count_edge_cases(osc):
+    n = 5_003
+    et, er, w0, ch = wl.events(n, seed=12)
+    edges = wl.bin_edges(13, 4.0)
+    d = [dev(a) for a in (et, er, w0, ch)]
+    de = dev(edges)
+    mixed = [wl.table1(), wl.table1(hierarchy=-1, rho_g_cm3=0.0), wl.table1(L_km=1300.0, delta_cp=2.0),
+             wl.table1(sin2_th13=0.0, dm2_21=0.0), wl.table1(L_km=0.0)]
+    for npts in (1, 2, 5):
+        pts = mixed[:npts]
+        got = host(osc.osc_reweight_bin_batch(pts, *d, 0.97, de))
+        ref = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 0.97, edges)
+        assert_hist_close(got, ref, f"batch npts={npts}")
+    # the batched call does not depend on, and does not change, the osc_set_params state
+    op = set_params(osc, wl.table1(delta_cp=0.4))
+    osc.osc_reweight_bin_batch(mixed, *d, 1.0, de)
+    got = host(osc.osc_reweight_bin(*d, 1.0, de))
+    assert_hist_close(got, oracle.reweight_bin(op, et, er, w0, ch, 1.0, edges), "state after batch")
+
+
+# ------------------------------------------------------------------------------------------------
+# asynchrony: parameters are captured at enqueue time; work runs on the caller's stream
+# ------------------------------------------------------------------------------------------------
+def test_params_captured_at_enqueue_on_side_stream(osc):
+    n = 2_000_000
+    E = wl.e_true(n, seed=13)
+    dE = dev(E)
+    pa, pb = wl.table1(), wl.table1(delta_cp=1.0, hierarchy=-1)
+    st = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(st):
+        osc.osc_set_params(**pa)
+        out_a = osc.osc_prob(dE, 1, 0, 0, stream=st)
+        osc.osc_set_params(**pb)              # must not disturb the launch already enqueued
+        out_b = osc.osc_prob(dE, 1, 0, 0, stream=st)
+    st.synchronize()
+    idx = np.arange(0, n, 997)
+    assert_prob_close(host(out_a)[idx], oracle.prob(oracle.Params(**pa), E[idx], 1, 0, 0), "first launch")
+    assert_prob_close(host(out_b)[idx], oracle.prob(oracle.Params(**pb), E[idx], 1, 0, 0), "second launch")
+
+
+def test_host_entry_points(osc):
+    n = 50_001
+    et, er, w0, ch = wl.events(n, seed=14)
+    edges = wl.bin_edges()
+    op = set_params(osc, wl.table1())
+    assert_prob_close(osc.osc_prob_host(et, 1, 0, 1), oracle.prob(op, et, 1, 0, 1), "osc_prob_host")
+    assert_hist_close(osc.osc_reweight_bin_host(et, er, w0, ch, 1.03, edges),
+                      oracle.reweight_bin(op, et, er, w0, ch, 1.03, edges), "osc_reweight_bin_host")
+
+
+# ------------------------------------------------------------------------------------------------
+# BASELINE.json full sizes, in the launch configuration bench.py times: sampled outputs the oracle
+# computes one by one, plus properties that hold at any size
+# ------------------------------------------------------------------------------------------------
+def test_config1_full_size_sampled(osc):
+    n = 10_000_000
+    E = wl.e_true(n, seed=1)
+    par = wl.config1_runs()[5]
+    op = set_params(osc, par)
+    dE = dev(E)
+    idx = np.random.Generator(np.random.PCG64(1)).choice(n, 30_000, replace=False)
+    idx[:4] = [0, 1, n - 2, n - 1]
+    out = torch.empty((9, n), dtype=torch.float64, device="cuda")
+    for anti in (0, 1):
+        osc.osc_prob_all(dE, anti, P_out=out)
+        s = out.view(3, 3, n)
+        assert float((s.sum(0) - 1).abs().max()) < 1e-12 and float((s.sum(1) - 1).abs().max()) < 1e-12
+        assert_prob_close(host(out[:, torch.from_numpy(idx).cuda()]), oracle.prob_all(op, E[idx], anti),
+                          f"config1 full anti {anti}")
+
+
+def test_config2_full_size(osc):
+    n = 10_000_000
+    et, er, w0, ch = wl.events(n, seed=2)
+    edges = wl.bin_edges()
+    op = set_params(osc, wl.table1())
+    d = [dev(a) for a in (et, er, w0, ch)]
+    de = dev(edges)
+    full = {s: host(osc.osc_reweight_bin(*d, s, de)) for s in wl.ENERGY_SCALES}
+    # (a) additivity over chunks (any size): chunk histograms sum to the full one
+    m = 2_500_000
+    for s in wl.ENERGY_SCALES:
+        parts = sum(host(osc.osc_reweight_bin(*[t[i:i + m] for t in d], s, de)) for i in range(0, n, m))
+        assert np.max(np.abs(parts - full[s]) / np.maximum(full[s], 1e-300) * (full[s] > 0)) < 1e-12
+    # (b) the oracle on one 1e6-event chunk of the same arrays
+    c = slice(3_000_000, 4_000_000)
+    got = host(osc.osc_reweight_bin(*[t[c] for t in d], 1.03, de))
+    assert_hist_close(got, oracle.reweight_bin(op, et[c], er[c], w0[c], ch[c], 1.03, edges), "config2 chunk")
+    # (c) bin indices bit-exact on all 1e7 events
+    for s in wl.ENERGY_SCALES:
+        assert np.array_equal(host(osc.osc_bin_index(d[0], d[1], d[3], s, de)), oracle.bin_index(et, er, ch, s, edges))
+    # (d) sum of bins == sum of w0 * P over in-range events, with P sampled from the oracle
+    idx = np.arange(0, n, 500)
+    b = oracle.bin_index(et[idx], er[idx], ch[idx], 1.0, edges)
+    sub = host(osc.osc_reweight_bin(*[t[torch.from_numpy(idx).cuda()] for t in d], 1.0, de))
+    ref = oracle.reweight_bin(op, et[idx], er[idx], w0[idx], ch[idx], 1.0, edges)
+    assert (b >= 0).sum() > 0
+    assert_hist_close(sub, ref, "config2 strided sample")
+
+
+def test_paper_validation_replay(osc):
+    """1e7 energies uniform in 0-30 GeV, residuals ~1e-12 in fp64 (A12: floored at 1e-3 GeV)."""
+    n = 10_000_000
+    E = wl.validation_energies(n, seed=4)
+    op = set_params(osc, wl.table1())
+    dE = dev(E)
+    idx = np.random.Generator(np.random.PCG64(4)).choice(n, 40_000, replace=False)
+    idx[:64] = np.argsort(E)[:64]          # the lowest energies = the largest phases
+    for fin, fout, anti in ((1, 1, 0), (1, 0, 0), (1, 0, 1)):
+        got = host(osc.osc_prob(dE, fin, fout, anti))
+        err = assert_prob_close(got[idx], oracle.prob(op, E[idx], fin, fout, anti), "validation replay")
+        print(f"validation replay {fin}->{fout} anti={anti}: max |dP| = {err:.2e}")

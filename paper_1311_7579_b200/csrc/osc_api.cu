@@ -5,8 +5,11 @@
 #include <atomic>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
+#include <map>
 #include <mutex>
+#include <utility>
 #include <vector>
 
 #include "../../include/osc.h"
@@ -92,13 +95,16 @@ int post_launch(const char* what)
     return OSC_OK;
 }
 
-size_t bin_smem_bytes(int nb)
-{
-    return sizeof(unsigned long long) * (size_t)(nb + 1) + sizeof(double) * kTransFields * kChannels +
-           sizeof(double) * (size_t)kWarps * kChannels * (size_t)nb;
-}
+constexpr int kMaxBins = 768; // 4 warps x 2 slots x 4 channels x 768 bins x 8 B = 196 KB of sub-histograms
+constexpr size_t kSmemBudget = 220 * 1024;
 
-constexpr int kMaxBins = 768; // 8 warps x 4 channels x 768 bins x 8 B = 196 KB of per-warp histograms
+size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+size_t k2_smem_bytes(int nb, int threads, int n_sub)
+{
+    return sizeof(double) * kBinArgsDoubles + bin_table_bytes(nb) +
+           sizeof(double) * (size_t)(threads / 32) * kSlots * n_sub * kChannels * (size_t)nb;
+}
 
 int check_bin_args(const double* E_true, const double* E_reco, const double* w0, const int8_t* channel, size_t n,
                    double energy_scale, const double* bin_edges, int n_bins, const void* out)
@@ -115,7 +121,73 @@ int check_bin_args(const double* E_true, const double* E_reco, const double* w0,
     return OSC_OK;
 }
 
-// Enqueue k2 for one parameter block.  hist_out is overwritten.
+// Stream-ordered scratch of one call; freed (stream-ordered) when it goes out of scope.
+struct Scratch {
+    char* p = nullptr;
+    cudaStream_t st = nullptr;
+    int alloc(size_t bytes, cudaStream_t s)
+    {
+        st = s;
+        CUDA_TRY(cudaMallocAsync((void**)&p, bytes, s));
+        return OSC_OK;
+    }
+    ~Scratch()
+    {
+        if (p) cudaFreeAsync(p, st);
+    }
+};
+
+// Device scratch the library keeps per (device, stream) for osc_reweight_bin: merge tickets (kept at zero
+// between kernels by the kernels themselves) and the per-block partial histograms.  Work on one stream is
+// ordered, so consecutive calls can share the buffer; it is allocated, zeroed and (when it has to grow)
+// freed in stream order.
+constexpr size_t kCounterBytes = 4096;
+struct StreamScratch {
+    char* buf = nullptr;
+    size_t cap = 0;
+};
+std::mutex g_scratch_mu;
+std::map<std::pair<int, cudaStream_t>, StreamScratch> g_scratch;
+
+int stream_scratch(size_t bytes, cudaStream_t st, char** out)
+{
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lk(g_scratch_mu);
+    StreamScratch& s = g_scratch[std::make_pair(dev, st)];
+    if (s.cap < bytes) {
+        if (s.buf) CUDA_TRY(cudaFreeAsync(s.buf, st));
+        s.buf = nullptr;
+        s.cap = 0;
+        const size_t cap = round_up(bytes + bytes / 2, 1 << 16);
+        char* p = nullptr;
+        CUDA_TRY(cudaMallocAsync((void**)&p, cap, st));
+        cudaError_t e = cudaMemsetAsync(p, 0, kCounterBytes, st);
+        if (e != cudaSuccess) {
+            cudaFreeAsync(p, st);
+            return fail(OSC_ERR_CUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e));
+        }
+        s.buf = p;
+        s.cap = cap;
+    }
+    *out = s.buf;
+    return OSC_OK;
+}
+
+template <bool VEC, int THREADS>
+int launch_k2(int grid, size_t smem, cudaStream_t st, const BinArgs& args, const double* E_true, const double* E_reco,
+              const double* w0, const int8_t* channel, size_t n, double energy_scale, const double* bin_edges,
+              int n_bins, int n_sub, const MergeScratch& ms, double* hist_out)
+{
+    if (smem > 48 * 1024)
+        CUDA_TRY(cudaFuncSetAttribute(reweight_bin_kernel<VEC, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)smem));
+    reweight_bin_kernel<VEC, THREADS><<<grid, THREADS, smem, st>>>(args, E_true, E_reco, w0, channel, n, energy_scale,
+                                                                  bin_edges, n_bins, n_sub, ms, hist_out);
+    return post_launch("osc_reweight_bin");
+}
+
+// Enqueue bin_setup + k2 for one parameter block.  hist_out is overwritten.
 int launch_reweight(const BinArgs& args, const double* E_true, const double* E_reco, const double* w0,
                     const int8_t* channel, size_t n, double energy_scale, const double* bin_edges, int n_bins,
                     double* hist_out, cudaStream_t st)
@@ -125,56 +197,48 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
         CUDA_TRY(cudaMemsetAsync(hist_out, 0, nh * sizeof(double), st));
         return OSC_OK;
     }
-    const size_t ntiles = (n + 2 * kBlock - 1) / (2 * kBlock);
-    int grid = 1;
-    int rc = grid_for(ntiles, &grid);
+    int sms = 0;
+    int rc = sm_count(&sms);
     if (rc) return rc;
-    const size_t smem = bin_smem_bytes(n_bins);
-    // fewer resident blocks when the per-warp histograms are large
-    if (smem > 48 * 1024) {
-        int sms = 0;
-        rc = sm_count(&sms);
-        if (rc) return rc;
-        size_t per_sm = (size_t)(220 * 1024) / smem;
-        if (per_sm < 1) per_sm = 1;
-        if (per_sm > (size_t)kBlocksPerSM) per_sm = kBlocksPerSM;
-        size_t g = (size_t)sms * per_sm;
-        if ((size_t)grid > g) grid = (int)g;
-    }
+    const int threads = k2_smem_bytes(n_bins, 256, 1) <= kSmemBudget ? 256 : 128;
+    // two sub-histograms per slot halve the collisions inside a warp; taken when at least 3 blocks still fit
+    const int n_sub = (threads == 256 && 3 * (k2_smem_bytes(n_bins, 256, 2) + 1024) <= kSmemBudget) ? 2 : 1;
+    int n_sub_t = n_sub;
+    if (const char* e = getenv("OSC_TUNE_NSUB")) n_sub_t = atoi(e);
+    const size_t smem = k2_smem_bytes(n_bins, threads, n_sub_t);
+    size_t per_sm = kSmemBudget / (smem + 1024);
+    if (const char* e = getenv("OSC_TUNE_BPS")) per_sm = (size_t)atoi(e);
+    if (per_sm < 1) per_sm = 1;
+    const size_t max_per_sm = threads == 256 ? kBlocksPerSM : 2 * kBlocksPerSM;
+    if (per_sm > max_per_sm && !getenv("OSC_TUNE_BPS")) per_sm = max_per_sm;
+    const size_t ntiles = (n + 2 * threads - 1) / (2 * (size_t)threads);
+    size_t g = (size_t)sms * per_sm;
+    if (ntiles < g) g = ntiles;
+    const int grid = (int)g;
+
     const int ngroups = (grid + kGroup - 1) / kGroup;
+    if ((size_t)(ngroups + 1) * sizeof(unsigned int) > kCounterBytes)
+        return fail(OSC_ERR_CUDA, "merge ticket area too small for %d groups", ngroups);
     const size_t bytes_partial = (size_t)grid * nh * sizeof(double);
     const size_t bytes_gpartial = (size_t)ngroups * nh * sizeof(double);
-    const size_t bytes_counters = (size_t)(ngroups + 1) * sizeof(unsigned int);
     char* scratch = nullptr;
-    CUDA_TRY(cudaMallocAsync((void**)&scratch, bytes_partial + bytes_gpartial + bytes_counters, st));
+    if ((rc = stream_scratch(kCounterBytes + bytes_partial + bytes_gpartial, st, &scratch))) return rc;
     MergeScratch ms;
-    ms.partial = reinterpret_cast<double*>(scratch);
-    ms.gpartial = reinterpret_cast<double*>(scratch + bytes_partial);
-    ms.counters = reinterpret_cast<unsigned int*>(scratch + bytes_partial + bytes_gpartial);
+    ms.counters = reinterpret_cast<unsigned int*>(scratch);
+    ms.partial = reinterpret_cast<double*>(scratch + kCounterBytes);
+    ms.gpartial = reinterpret_cast<double*>(scratch + kCounterBytes + bytes_partial);
     ms.ngroups = ngroups;
-    cudaError_t e = cudaMemsetAsync(ms.counters, 0, bytes_counters, st);
-    if (e == cudaSuccess) {
-        const bool vec = aligned(E_true, 16) && aligned(E_reco, 16) && aligned(w0, 16) && aligned(channel, 2);
-        if (vec) {
-            if (smem > 48 * 1024)
-                e = cudaFuncSetAttribute(reweight_bin_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e == cudaSuccess)
-                reweight_bin_kernel<true><<<grid, kBlock, smem, st>>>(args, E_true, E_reco, w0, channel, n, energy_scale,
-                                                                    bin_edges, n_bins, ms, hist_out);
-        } else {
-            if (smem > 48 * 1024)
-                e = cudaFuncSetAttribute(reweight_bin_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e == cudaSuccess)
-                reweight_bin_kernel<false><<<grid, kBlock, smem, st>>>(args, E_true, E_reco, w0, channel, n,
-                                                                     energy_scale, bin_edges, n_bins, ms, hist_out);
-        }
-        if (e == cudaSuccess) e = cudaGetLastError();
-        if (e == cudaSuccess) g_launches.fetch_add(1, std::memory_order_relaxed);
-    }
-    cudaError_t e2 = cudaFreeAsync(scratch, st);
-    if (e != cudaSuccess) return fail(OSC_ERR_CUDA, "osc_reweight_bin launch failed: %s", cudaGetErrorString(e));
-    if (e2 != cudaSuccess) return fail(OSC_ERR_CUDA, "cudaFreeAsync: %s", cudaGetErrorString(e2));
-    return OSC_OK;
+
+    const bool vec = aligned(E_true, 16) && aligned(E_reco, 16) && aligned(w0, 16) && aligned(channel, 2);
+    if (threads == 256)
+        return vec ? launch_k2<true, 256>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
+                                          n_bins, n_sub_t, ms, hist_out)
+                   : launch_k2<false, 256>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
+                                           n_bins, n_sub, ms, hist_out);
+    return vec ? launch_k2<true, 128>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
+                                      n_bins, n_sub_t, ms, hist_out)
+               : launch_k2<false, 128>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
+                                       n_bins, n_sub, ms, hist_out);
 }
 
 // Device staging buffers of the *_host entry points (grown on demand, reused between calls).
@@ -197,8 +261,6 @@ struct HostPath {
     }
 };
 HostPath g_host;
-
-size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 } // namespace
 
@@ -299,16 +361,65 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
         if (const char* msg = check_params(points[p]))
             return fail(OSC_ERR_INVALID_ARG, "osc_reweight_bin_batch: point %d: %s", p, msg);
     const size_t nh = (size_t)kChannels * n_bins;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (n == 0) {
+        CUDA_TRY(cudaMemsetAsync(hist_out, 0, (size_t)n_points * nh * sizeof(double), st));
+        return OSC_OK;
+    }
+    // a1 for every point (host), packed as BinArgs
+    std::vector<BinArgs> blocks((size_t)n_points);
     for (int p = 0; p < n_points; ++p) {
         HostSet h;
         precompute(points[p], h);
-        BinArgs args;
-        make_bin_args(h, args);
-        rc = launch_reweight(args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges, n_bins,
-                             hist_out + (size_t)p * nh, static_cast<cudaStream_t>(stream));
-        if (rc) return rc;
+        make_bin_args(h, blocks[(size_t)p]);
     }
-    return OSC_OK;
+    int sms = 0;
+    if ((rc = sm_count(&sms))) return rc;
+
+    // geometry: 1 block per SM (shared-memory bound); blocks = nchunks x ngroups ~ 4 waves
+    const size_t hist1 = sizeof(double) * (kBatchThreads / 32) * kSlots * nh;
+    const int n_sub = (2 * hist1 <= 64 * 1024) ? 2 : 1;
+    const size_t fixed = sizeof(double) * kBinArgsDoubles + bin_table_bytes(n_bins) + n_sub * hist1;
+    if (fixed + 18 * 2 * kBatchThreads > kSmemBudget)
+        return fail(OSC_ERR_INVALID_ARG, "osc_reweight_bin_batch: n_bins = %d needs more shared memory than one SM has "
+                                         "(limit for the batched call: about 380 bins)", n_bins);
+    const int tile_quant = 2 * kBatchThreads;
+    int te = (int)((kSmemBudget - fixed) / 18 / tile_quant * tile_quant);
+    if (te > 8192) te = 8192;
+    BatchGeom geo;
+    const int target_blocks = 4 * sms;
+    int ngroups = n_points < 16 ? n_points : 16;
+    size_t max_chunks = (n + tile_quant - 1) / tile_quant;          // at least one thread-pair row per chunk
+    size_t nchunks = (size_t)(target_blocks + ngroups - 1) / ngroups;
+    if (nchunks > max_chunks) {
+        nchunks = max_chunks;
+        // few events: spread the points over more groups instead
+        size_t want = ((size_t)target_blocks + nchunks - 1) / nchunks;
+        ngroups = (int)(want < (size_t)n_points ? want : (size_t)n_points);
+    }
+    geo.chunk_events = round_up((n + nchunks - 1) / nchunks, 2);
+    nchunks = (n + geo.chunk_events - 1) / geo.chunk_events;
+    geo.nchunks = (int)nchunks;
+    geo.pts_per_group = (n_points + ngroups - 1) / ngroups;
+    ngroups = (n_points + geo.pts_per_group - 1) / geo.pts_per_group;
+    if ((size_t)te > round_up(geo.chunk_events, tile_quant)) te = (int)round_up(geo.chunk_events, tile_quant);
+    geo.te = te;
+    const size_t smem = fixed + (size_t)18 * te;
+
+    const size_t bytes_points = round_up((size_t)n_points * sizeof(BinArgs), 256);
+    const size_t bytes_partial = (size_t)n_points * nchunks * nh * sizeof(double);
+    Scratch sc;
+    if ((rc = sc.alloc(bytes_points + bytes_partial, st))) return rc;
+    double* d_points = reinterpret_cast<double*>(sc.p);
+    double* partial = reinterpret_cast<double*>(sc.p + bytes_points);
+    // pageable source: the copy is staged before the call returns, so `blocks` may go out of scope
+    CUDA_TRY(cudaMemcpyAsync(d_points, blocks.data(), (size_t)n_points * sizeof(BinArgs), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaFuncSetAttribute(reweight_batch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    reweight_batch_kernel<<<dim3((unsigned)nchunks, (unsigned)ngroups), kBatchThreads, smem, st>>>(
+        d_points, n_points, E_true, E_reco, w0, channel, n, geo, energy_scale, bin_edges, n_bins, n_sub, partial);
+    if ((rc = post_launch("osc_reweight_bin_batch"))) return rc;
+    merge_chunks_kernel<<<n_points, 256, 0, st>>>(partial, (int)nchunks, (int)nh, hist_out);
+    return post_launch("osc_reweight_bin_batch merge");
 }
 
 int osc_bin_index(const double* E_true, const double* E_reco, const int8_t* channel, size_t n, double energy_scale,
@@ -319,9 +430,9 @@ int osc_bin_index(const double* E_true, const double* E_reco, const int8_t* chan
     if (n == 0) return OSC_OK;
     int grid = 1;
     if ((rc = grid_for((n + kBlock - 1) / kBlock, &grid))) return rc;
-    const size_t smem = sizeof(unsigned long long) * (size_t)(n_bins + 1);
-    bin_index_kernel<<<grid, kBlock, smem, static_cast<cudaStream_t>(stream)>>>(E_true, E_reco, channel, n, energy_scale,
-                                                                              bin_edges, n_bins, bin_out);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    bin_index_kernel<<<grid, kBlock, bin_table_bytes(n_bins), st>>>(E_true, E_reco, channel, n, energy_scale, bin_edges,
+                                                                   n_bins, bin_out);
     return post_launch("osc_bin_index");
 }
 

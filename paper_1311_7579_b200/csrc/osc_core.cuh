@@ -46,8 +46,8 @@ __device__ __forceinline__ void eig_solve(const OscSet& ps, double A, double inv
     double c1 = fma(A, ps.k1, ps.dd);
     double c0_27 = A * ps.k0_27;
     double c1_3 = 3.0 * c1;
-    double R2 = fma(c2, c2, -c1_3);
-    R2 = fmax(R2, 1e-60);                       // T proportional to I cannot be solved; keep finite
+    double R2 = fma(c2, c2, -c1_3);             // (1/2) sum of squared gaps: > 0 for every valid parameter set
+    R2 = floor_at_pow2(R2, 0x03000000);         // (DESIGN.md "R2 > 0"); the floor 2^-975 only keeps NaN out
     double tq = fma(2.0, R2, -c1_3);            // 2 c2^2 - 9 c1
     double q = fma(c2, tq, c0_27);              // 2 c2^3 - 9 c2 c1 + 27 c0
 
@@ -60,7 +60,7 @@ __device__ __forceinline__ void eig_solve(const OscSet& ps, double A, double inv
     cos_third_acos(fabs(U2), t, rh);            // t = cos(phi'), rh = 1 / (24 t^2 - 6)
     double om = 1.0 - t;
     double w = fma(om, t, om);                  // 1 - t^2 = sin^2(phi')
-    w = fmax(w, 1e-30);
+    w = floor_at_pow2(w, 0x39B00000);           // >= 2^-100: a closed gap stays finite (sinc form below)
     double y = rsqrt_pos(w);
     double s = w * y;                           // sin(phi')
     double ga = fma(-HALF_SQ3, s, 1.5 * t);     // gaps in units of (2/3) R:  ga >= gb, ga + gb = largest gap
@@ -84,14 +84,13 @@ __device__ __forceinline__ void eig_solve(const OscSet& ps, double A, double inv
     double ka = 36.0 * rr;                                  // 2 / (Rs^2 ga gc)
     double kb = (rr * (36.0 / SQ3)) * (ga * y);             // 2 / (Rs^2 gb gc)
 
-    // a2d gap phases in quarter turns
+    // a2d gap phases in quarter turns: g R xq23 / E
     double RX = R * (ps.xq23 * invE);
-    double hqa = ga * RX, hqb = gb * RX;
-    double hq1 = select_d(neg, hqb, hqa);
-    double hq12 = select_d(neg, hqa, hqb);
+    double ha = select_d(neg, gb, ga);
+    double hb = select_d(neg, ga, gb);
     double s1, c1c, s12, c12;
-    sincos_quarter(hq1, s1, c1c);
-    sincos_quarter(hq12, s12, c12);
+    sincos_quarter_mul(ha, RX, s1, c1c);
+    sincos_quarter_mul(hb, RX, s12, c12);
     o.s1h = s1;
     o.c1h = c1c;
     o.c02 = fma(c1c, c12, -(s1 * s12));

@@ -1,0 +1,119 @@
+// osc_hist.cuh -- deterministic shared-memory histogram accumulation.
+//
+// sm_100a has no native fp64 shared-memory atomic add (atomicAdd(double*) on shared memory lowers to an
+// ATOMS.CAST.SPIN loop whose order of additions is not defined).  Instead every warp owns private
+// sub-histograms and resolves the collisions inside the warp itself:
+//
+//   * each lane carries two events (slot 0 and slot 1); slot s of the lanes with (lane mod n_sub) = u adds
+//     into sub-histogram (s, u) of the warp, so the two slots never collide with each other and only
+//     32 / n_sub lanes can collide at all (n_sub = 2 when shared memory allows, else 1);
+//   * lanes that hit the same word are found with MATCH.ANY on the word's address; a lane's rank is the
+//     number of lower lanes with the same address;
+//   * phase r = 0, 1, ... lets exactly the lanes of rank r do a plain read-modify-write: inside a phase
+//     all addresses are distinct, and for one address the additions happen in lane order.
+//
+// Block result = sub-histograms summed in (warp, slot, u) order; blocks are merged in two fixed-order
+// levels by the last block to arrive (tickets), so every histogram is a deterministic function of the
+// inputs.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "osc_smem.cuh"
+
+namespace oscb {
+
+constexpr int kSlots = 2; // events per lane per iteration
+
+// Shared-window byte addresses of this lane's two sub-histograms (loop invariant).
+struct LaneHist {
+    uint32_t h0, h1;
+};
+
+__device__ __forceinline__ LaneHist lane_hist(const double* hist, int nh, int n_sub, unsigned warp, unsigned lane)
+{
+    const unsigned u = lane & (unsigned)(n_sub - 1);
+    const uint32_t wbase = smem_u32(hist) + 8u * (warp * (unsigned)(kSlots * n_sub * nh));
+    LaneHist lh;
+    lh.h0 = wbase + 8u * (u * (unsigned)nh);
+    lh.h1 = wbase + 8u * (((unsigned)n_sub + u) * (unsigned)nh);
+    return lh;
+}
+
+// cell0 / cell1: histogram cell of the lane's slot-0 / slot-1 event, or -1 for a dropped event.
+__device__ __forceinline__ void warp_hist_add2(const LaneHist& lh, int cell0, double w0, int cell1, double w1,
+                                               unsigned lt_mask)
+{
+    const unsigned FULL = 0xffffffffu;
+    const uint32_t a0 = cell0 >= 0 ? lh.h0 + 8u * (unsigned)cell0 : 0xFFFFFFFFu;
+    const uint32_t a1 = cell1 >= 0 ? lh.h1 + 8u * (unsigned)cell1 : 0xFFFFFFFFu;
+    const unsigned p0 = __match_any_sync(FULL, a0);
+    const unsigned p1 = __match_any_sync(FULL, a1);
+    const int r0 = cell0 >= 0 ? __popc(p0 & lt_mask) : -1;
+    const int r1 = cell1 >= 0 ? __popc(p1 & lt_mask) : -1;
+    const int rmax = __reduce_max_sync(FULL, max(r0, r1));
+#pragma unroll 1
+    for (int ph = 0; ph <= rmax; ++ph) {
+        if (r0 == ph) sts_f64_volatile(a0, lds_f64_volatile(a0) + w0);
+        if (r1 == ph) sts_f64_volatile(a1, lds_f64_volatile(a1) + w1);
+        __syncwarp();
+    }
+}
+
+// Scratch of one call: counters[ngroups + 1] | partial[grid][nh] | gpartial[ngroups][nh].  It lives in a
+// buffer the library keeps per (device, stream); calls on one stream are ordered, so they can share it.
+// The counters are zero when a kernel starts and the blocks that consume them set them back to zero.
+struct MergeScratch {
+    double* partial;
+    double* gpartial;
+    unsigned int* counters;
+    int ngroups;
+};
+
+constexpr int kGroup = 16; // blocks per first-level merge group
+
+// hist: [n_sub][nh] sub-histograms of this block in shared memory (n_sub = warps * kSlots).
+// Writes the block's sum to ms.partial, then the last block of each group sums the group and the last
+// group sums the groups into out[nh].  Must be called by all threads of the block.
+__device__ __forceinline__ void block_merge(const double* hist, int n_sub, int nh, const MergeScratch& ms,
+                                            double* __restrict__ out, unsigned int* s_ticket)
+{
+    __syncthreads();
+    double* my_partial = ms.partial + (size_t)blockIdx.x * nh;
+    for (int i = threadIdx.x; i < nh; i += blockDim.x) {
+        double s = hist[i];
+        for (int w = 1; w < n_sub; ++w) s += hist[(size_t)w * nh + i];
+        my_partial[i] = s;
+    }
+    __threadfence();
+    __syncthreads();
+
+    const int group = blockIdx.x / kGroup;
+    const int gfirst = group * kGroup;
+    const int gsize = min(kGroup, (int)gridDim.x - gfirst);
+    if (threadIdx.x == 0) *s_ticket = atomicAdd(ms.counters + group, 1u);
+    __syncthreads();
+    if (*s_ticket != (unsigned)(gsize - 1)) return;
+    if (threadIdx.x == 0) ms.counters[group] = 0u;          // last of the group: nobody else reads it again
+    __threadfence();
+    for (int i = threadIdx.x; i < nh; i += blockDim.x) {
+        const double* src = ms.partial + (size_t)gfirst * nh + i;
+        double s = __ldcg(src);
+        for (int b = 1; b < gsize; ++b) s += __ldcg(src + (size_t)b * nh);
+        ms.gpartial[(size_t)group * nh + i] = s;
+    }
+    __threadfence();
+    __syncthreads();
+
+    if (threadIdx.x == 0) *s_ticket = atomicAdd(ms.counters + ms.ngroups, 1u);
+    __syncthreads();
+    if (*s_ticket != (unsigned)(ms.ngroups - 1)) return;
+    if (threadIdx.x == 0) ms.counters[ms.ngroups] = 0u;
+    __threadfence();
+    for (int i = threadIdx.x; i < nh; i += blockDim.x) {
+        double s = __ldcg(ms.gpartial + i);
+        for (int g = 1; g < ms.ngroups; ++g) s += __ldcg(ms.gpartial + (size_t)g * nh + i);
+        out[i] = s;
+    }
+}
+
+} // namespace oscb

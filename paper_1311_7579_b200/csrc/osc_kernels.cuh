@@ -1,24 +1,27 @@
 // osc_kernels.cuh -- sm_100a kernels of libosc_b200.
 //
-//   prob_kernel          k1   one transition per event                       (osc_prob)
-//   prob_all_kernel      k1b  nine transitions from one eigen-solve          (osc_prob_all)
-//   reweight_bin_kernel  k2   fused probability -> weight -> bin -> histogram (osc_reweight_bin)
-//   bin_index_kernel          the integer binning decision of k2, exported    (osc_bin_index)
+//   prob_kernel            k1   one transition per event                        (osc_prob)
+//   prob_all_kernel        k1b  nine transitions from one eigen-solve           (osc_prob_all)
+//   reweight_bin_kernel    k2   fused probability -> weight -> bin -> histogram  (osc_reweight_bin)
+//   reweight_batch_kernel  k3   event tiles resident in shared memory, reused across many
+//                               parameter sets                                   (osc_reweight_bin_batch)
+//   merge_chunks_kernel         fixed-order sum of k3's per-chunk histograms
+//   bin_index_kernel            the integer binning decision of k2/k3, exported  (osc_bin_index)
 //
-// All are persistent grid-stride kernels sized from the SM count; every thread carries two events
-// per iteration (two independent fp64 dependency chains) and the parameter block arrives as a
+// k1, k1b and k2 are persistent grid-stride kernels sized from the SM count; every thread carries two
+// events per iteration (two independent fp64 dependency chains) and the parameter block arrives as a
 // __grid_constant__ kernel parameter.  DESIGN.md "Kernels" has the per-event operation budget and
 // the roofline that bounds each of them.
 #pragma once
 #include <cstdint>
 
+#include "osc_bins.cuh"
 #include "osc_core.cuh"
+#include "osc_hist.cuh"
 
 namespace oscb {
 
-constexpr int kBlock = 256;          // threads per block (8 warps)
-constexpr int kWarps = kBlock / 32;
-constexpr int kGroup = 16;           // blocks per merge group in k2's two-level histogram merge
+constexpr int kBlock = 256;          // threads per block of k1 / k1b (8 warps)
 
 // Streaming loads/stores: every event byte is touched once (evict-first, no L1 allocation).
 __device__ __forceinline__ double ld_stream(const double* p) { return __ldcs(p); }
@@ -124,187 +127,113 @@ prob_all_kernel(const __grid_constant__ ProbAllArgs a, const double* __restrict_
 }
 
 // ------------------------------------------------------------------------------------------------
-// Binning (row a3c).  The decision "edges[i] <= x < edges[i+1]" is taken on order-preserving integer
-// images of the doubles (IEEE-754 total order with -0 folded onto +0 and NaN excluded), so it is
-// bit-identical to the fp64 comparisons and costs no fp64-pipe instructions.
+// Debug export of the binning decision (osc_bin_index): bin of every event, -1 if dropped (A8, A11).
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ unsigned long long order_key(double v)
-{
-    unsigned long long b = (unsigned long long)__double_as_longlong(v);
-    if (b == 0x8000000000000000ull) b = 0ull;                           // -0.0 == +0.0
-    return (b & 0x8000000000000000ull) ? ~b : (b | 0x8000000000000000ull);
-}
-
-__device__ __forceinline__ bool is_nan_bits(double v)
-{
-    return ((unsigned long long)__double_as_longlong(v) & 0x7FFFFFFFFFFFFFFFull) > 0x7FF0000000000000ull;
-}
-
-// ekey[0..nb] = order_key(edges[i]) in shared memory; top_step = largest power of two <= nb.
-// Returns the unique i with edges[i] <= x < edges[i+1], or -1.
-__device__ __forceinline__ int find_bin(const unsigned long long* ekey, int nb, int top_step, double x)
-{
-    const unsigned long long kx = order_key(x);
-    int lo = 0;
-    for (int step = top_step; step > 0; step >>= 1) {
-        const int mid = lo + step;
-        if (mid <= nb && ekey[mid] <= kx) lo = mid;
-    }
-    const bool inside = !is_nan_bits(x) && ekey[0] <= kx && lo < nb;
-    return inside ? lo : -1;
-}
-
-__device__ __forceinline__ void load_edge_keys(unsigned long long* ekey, const double* __restrict__ edges, int nb)
-{
-    for (int i = threadIdx.x; i <= nb; i += blockDim.x) ekey[i] = order_key(edges[i]);
-}
-
-__device__ __forceinline__ int pow2_floor(int v)
-{
-    return 1 << (31 - __clz(v));
-}
-
-// Debug export of the binning decision (osc_bin_index).
 __global__ void __launch_bounds__(kBlock)
 bin_index_kernel(const double* __restrict__ E_true, const double* __restrict__ E_reco,
                  const int8_t* __restrict__ channel, size_t n, double energy_scale,
                  const double* __restrict__ edges, int nb, int32_t* __restrict__ bin_out)
 {
-    extern __shared__ unsigned long long smem_u64[];
-    unsigned long long* ekey = smem_u64;
-    load_edge_keys(ekey, edges, nb);
-    __syncthreads();
-    const int top = pow2_floor(nb);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    build_bin_table(smem_raw, edges, nb);
+    const BinView bt = bin_view(smem_raw);
     const size_t stride = (size_t)gridDim.x * kBlock;
     for (size_t j = (size_t)blockIdx.x * kBlock + threadIdx.x; j < n; j += stride) {
-        const double x = __dmul_rn(energy_scale, E_reco[j]);
+        const double x = scaled_energy(energy_scale, E_reco[j]);
         const int ch = channel[j];
         const bool ok = energy_ok(E_true[j]) && (unsigned)ch < (unsigned)kChannels;
-        const int b = find_bin(ekey, nb, top, x);
+        const int b = find_bin(bt, x);
         bin_out[j] = ok ? b : -1;
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// k2: fused reweight + histogram.
-//
-// Shared memory per block:  ekey[nb+1] | chtab[9][4] | hist[kWarps][4*nb]
-// Each warp owns a private histogram, so no atomics are needed: lanes of one warp that hit the same
-// (channel, bin) cell are found with match.any and summed by the lowest such lane in lane order, and
-// that lane alone does the read-modify-write.  Block result = sum over warps in warp order; blocks
-// are merged in two fixed-order levels (groups of kGroup blocks, then groups) by whichever block
-// finishes last, so the histogram is a deterministic function of the inputs and of n.
+// Parameter block of one point in shared memory: kBinArgsDoubles doubles laid out as BinArgs.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void warp_hist_add(double* hist, int key, double w, unsigned lane)
+__device__ __forceinline__ OscTrans load_trans(uint32_t pb, int c)
 {
-    const unsigned FULL = 0xffffffffu;
-    const unsigned peers = __match_any_sync(FULL, key);
-    const bool leader = (peers & ((1u << lane) - 1u)) == 0u;
-    unsigned rem = (leader && key >= 0) ? (peers & ~(1u << lane)) : 0u;
-    double acc = w;
-    while (__any_sync(FULL, rem != 0u)) {
-        const int src = rem ? (__ffs(rem) - 1) : (int)lane;
-        const double v = __shfl_sync(FULL, w, src);
-        if (rem) {
-            acc += v;
-            rem &= rem - 1u;
-        }
-    }
-    if (leader && key >= 0) hist[key] += acc;
-    __syncwarp();
-}
-
-struct ChanConst {
-    double f[kTransFields];
-};
-
-__device__ __forceinline__ OscTrans load_trans(const double* chtab, int c)
-{
+    const uint32_t q = pb + 8u * (6u + (unsigned)c * kTransDoubles);
+    const double2 a = lds_f64x2(q), b = lds_f64x2(q + 16), d = lds_f64x2(q + 32), e = lds_f64x2(q + 48);
     OscTrans t;
-    t.sa = chtab[0 * kChannels + c];
-    t.delta = chtab[1 * kChannels + c];
-    t.ee = chtab[2 * kChannels + c];
-    t.Tr0 = chtab[3 * kChannels + c];
-    t.Ti0 = chtab[4 * kChannels + c];
-    t.T2r0 = chtab[5 * kChannels + c];
-    t.T2i0 = chtab[6 * kChannels + c];
-    t.T2r1 = chtab[7 * kChannels + c];
-    t.T2i1 = chtab[8 * kChannels + c];
+    t.sa = a.x;
+    t.delta = a.y;
+    t.ee = b.x;
+    t.Tr0 = b.y;
+    t.Ti0 = d.x;
+    t.T2r0 = d.y;
+    t.T2i0 = e.x;
+    t.T2r1 = e.y;
+    t.T2i1 = lds_f64(q + 64);
+    t.pad = 0.0;
     return t;
 }
 
-__device__ __forceinline__ void store_chtab(double* chtab, const OscTrans* ch)
+__device__ __forceinline__ OscSet load_set(const double* pb)
 {
-    if (threadIdx.x < kChannels) {
-        const int c = threadIdx.x;
-        const OscTrans t = ch[c];
-        chtab[0 * kChannels + c] = t.sa;
-        chtab[1 * kChannels + c] = t.delta;
-        chtab[2 * kChannels + c] = t.ee;
-        chtab[3 * kChannels + c] = t.Tr0;
-        chtab[4 * kChannels + c] = t.Ti0;
-        chtab[5 * kChannels + c] = t.T2r0;
-        chtab[6 * kChannels + c] = t.T2i0;
-        chtab[7 * kChannels + c] = t.T2r1;
-        chtab[8 * kChannels + c] = t.T2i1;
-    }
+    const double2* q = reinterpret_cast<const double2*>(pb);
+    const double2 a = q[0], b = q[1], d = q[2];
+    OscSet s;
+    s.xq23 = a.x;
+    s.tr = a.y;
+    s.dd = b.x;
+    s.k1 = b.y;
+    s.k0_27 = d.x;
+    return s;
 }
 
-// Scratch owned by one call (stream-ordered allocation): partial[grid][nh] | gpartial[ngroups][nh] |
-// counters[ngroups + 1] (zeroed before the launch).
-struct MergeScratch {
-    double* partial;
-    double* gpartial;
-    unsigned int* counters;
-    int ngroups;
-};
-
-
-// Per-event part of k2: returns the histogram cell (channel * nb + bin, or -1 if the event is
-// dropped, A8/A11) and the weight w0 * P_channel(E_true).
-__device__ __forceinline__ void reweight_one(const OscSet& set, const double* chtab, const unsigned long long* ekey,
-                                             int nb, int top, double energy_scale, bool in, double Et, double Er,
-                                             double wp, int ch, int& key, double& w)
+// Per-event part of k2: the histogram cell (channel * nb + bin, or -1 if the event is dropped, A8/A11)
+// and the weight w0 * P_channel(E_true).
+__device__ __forceinline__ void reweight_one(const OscSet& set, uint32_t pb, const BinView& bt,
+                                             double energy_scale, bool in, double Et, double Er, double wp, int ch,
+                                             int& cell, double& w)
 {
-    const double x = __dmul_rn(energy_scale, Er);           // a3b: one rounded fp64 multiply
-    const int bin = find_bin(ekey, nb, top, x);             // a3c: bit-exact index
+    const double x = scaled_energy(energy_scale, Er);       // a3b: one rounded fp64 multiply
+    const int bin = find_bin(bt, x);                        // a3c: bit-exact index
     const bool ok = in && energy_ok(Et) && (unsigned)ch < (unsigned)kChannels && bin >= 0;
     const int c = ok ? ch : 0;
-    const OscTrans tr = load_trans(chtab, c);
+    const OscTrans tr = load_trans(pb, c);
     const double P = prob_one(set, tr, ok ? Et : 1.0);      // a2a-a2f
     w = __dmul_rn(wp, P);                                   // a3a
-    key = ok ? c * nb + bin : -1;
+    cell = ok ? c * bt.nb + bin : -1;
 }
 
-template <bool VEC>
-__global__ void __launch_bounds__(kBlock)
+// ------------------------------------------------------------------------------------------------
+// k2: fused reweight + histogram, one parameter set.
+// Shared memory per block:  param block | bin table | hist[warps][kSlots][n_sub][4 * nb]
+// ------------------------------------------------------------------------------------------------
+template <bool VEC, int THREADS>
+__global__ void __launch_bounds__(THREADS, 1024 / THREADS)
 reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict__ E_true,
                     const double* __restrict__ E_reco, const double* __restrict__ w0,
                     const int8_t* __restrict__ channel, size_t n, double energy_scale,
-                    const double* __restrict__ edges, int nb, MergeScratch ms, double* __restrict__ hist_out)
+                    const double* __restrict__ edges, int nb, int n_sub, MergeScratch ms,
+                    double* __restrict__ hist_out)
 {
-    extern __shared__ unsigned long long smem_u64[];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int WARPS = THREADS / 32;
     const int nh = kChannels * nb;
-    unsigned long long* ekey = smem_u64;
-    double* chtab = reinterpret_cast<double*>(ekey + (nb + 1));
-    double* hist = chtab + kTransFields * kChannels;
+    double* pbuf = reinterpret_cast<double*>(smem_raw);
+    unsigned char* tab = smem_raw + sizeof(double) * kBinArgsDoubles;
+    double* hist = reinterpret_cast<double*>(tab + bin_table_bytes(nb));
     __shared__ unsigned int s_ticket;
 
     const unsigned lane = threadIdx.x & 31u;
     const unsigned warp = threadIdx.x >> 5;
-    double* myhist = hist + (size_t)warp * nh;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    const int n_hist = WARPS * kSlots * n_sub;
 
-    load_edge_keys(ekey, edges, nb);
-    store_chtab(chtab, a.ch);
-    for (int i = threadIdx.x; i < kWarps * nh; i += kBlock) hist[i] = 0.0;
-    __syncthreads();
+    if (threadIdx.x < kBinArgsDoubles) pbuf[threadIdx.x] = reinterpret_cast<const double*>(&a)[threadIdx.x];
+    for (int i = threadIdx.x; i < n_hist * nh; i += THREADS) hist[i] = 0.0;
+    build_bin_table(tab, edges, nb);
+    const BinView bt = bin_view(tab);
+    const uint32_t pb = smem_u32(pbuf);
+    const LaneHist lh = lane_hist(hist, nh, n_sub, warp, lane);
 
-    const int top = pow2_floor(nb);
-    const size_t ntiles = (n + 2 * kBlock - 1) / (2 * kBlock);
+    const size_t ntiles = (n + 2 * THREADS - 1) / (2 * THREADS);
     for (size_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
-        const size_t base = t * (2 * kBlock);
+        const size_t base = t * (2 * THREADS);
         const size_t j0 = VEC ? base + 2 * threadIdx.x : base + threadIdx.x;
-        const size_t j1 = VEC ? j0 + 1 : j0 + kBlock;
+        const size_t j1 = VEC ? j0 + 1 : j0 + THREADS;
         const bool in0 = j0 < n, in1 = j1 < n;
         double Et0, Et1, Er0, Er1, wp0, wp1;
         int ch0, ch1;
@@ -326,54 +255,143 @@ reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict_
             ch0 = in0 ? (int)channel[j0] : -1;
             ch1 = in1 ? (int)channel[j1] : -1;
         }
-        int key0, key1;
+        int cell0, cell1;
         double w_0, w_1;
-        reweight_one(a.set, chtab, ekey, nb, top, energy_scale, in0, Et0, Er0, wp0, ch0, key0, w_0);
-        reweight_one(a.set, chtab, ekey, nb, top, energy_scale, in1, Et1, Er1, wp1, ch1, key1, w_1);
-        warp_hist_add(myhist, key0, w_0, lane);
-        warp_hist_add(myhist, key1, w_1, lane);
+        reweight_one(a.set, pb, bt, energy_scale, in0, Et0, Er0, wp0, ch0, cell0, w_0);
+        reweight_one(a.set, pb, bt, energy_scale, in1, Et1, Er1, wp1, ch1, cell1, w_1);
+        warp_hist_add2(lh, cell0, w_0, cell1, w_1, lt_mask);
     }
-    __syncthreads();
+    block_merge(hist, n_hist, nh, ms, hist_out, &s_ticket);
+}
 
-    // block result: warps summed in warp order
-    double* my_partial = ms.partial + (size_t)blockIdx.x * nh;
-    for (int i = threadIdx.x; i < nh; i += kBlock) {
-        double s = hist[i];
-#pragma unroll
-        for (int w = 1; w < kWarps; ++w) s += hist[(size_t)w * nh + i];
-        my_partial[i] = s;
+// ------------------------------------------------------------------------------------------------
+// k3: batched parameter sets (row a4).  Block (c, g) owns event chunk c and point group g.  The chunk is
+// staged tile by tile in shared memory -- E_true, w0 and the histogram cell of every event, which does
+// not depend on the parameter set and is therefore decided once per tile -- and every staged tile is
+// reused for all points of the group.  Per point the block fills per-warp sub-histograms, sums them in a
+// fixed order and adds the result to its own slice partial[p][c][:] in global memory; merge_chunks_kernel
+// then sums the chunks of each point in chunk order.
+//
+// Shared memory: param block | bin table | hist[warps][kSlots][n_sub][4 nb] | Et[te] | w0[te] | cellch[te]
+// cellch = cell | channel << 12 (cell < 4 * 768 = 3072), 0xFFFF for a dropped or padding event.
+// ------------------------------------------------------------------------------------------------
+constexpr int kBatchThreads = 512;
+constexpr unsigned short kDropped = 0xFFFFu;
+
+struct BatchGeom {
+    size_t chunk_events;  // events per chunk (multiple of 2)
+    int te;               // tile capacity in events (multiple of 2 * kBatchThreads)
+    int nchunks;
+    int pts_per_group;
+};
+
+__global__ void __launch_bounds__(kBatchThreads, 1)
+reweight_batch_kernel(const double* __restrict__ points, int npts, const double* __restrict__ E_true,
+                      const double* __restrict__ E_reco, const double* __restrict__ w0,
+                      const int8_t* __restrict__ channel, size_t n, BatchGeom geo, double energy_scale,
+                      const double* __restrict__ edges, int nb, int n_sub, double* __restrict__ partial)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int WARPS = kBatchThreads / 32;
+    const int nh = kChannels * nb;
+    const int n_hist = WARPS * kSlots * n_sub;
+    double* pbuf = reinterpret_cast<double*>(smem_raw);
+    unsigned char* tab = smem_raw + sizeof(double) * kBinArgsDoubles;
+    double* hist = reinterpret_cast<double*>(tab + bin_table_bytes(nb));
+    double* sEt = hist + (size_t)n_hist * nh;
+    double* sW = sEt + geo.te;
+    unsigned short* sCell = reinterpret_cast<unsigned short*>(sW + geo.te);
+
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned warp = threadIdx.x >> 5;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    const uint32_t pb = smem_u32(pbuf);
+    const LaneHist lh = lane_hist(hist, nh, n_sub, warp, lane);
+
+    const int chunk = blockIdx.x;
+    const size_t ev_begin = (size_t)chunk * geo.chunk_events;
+    const size_t ev_end = min(n, ev_begin + geo.chunk_events);
+    const int p_begin = blockIdx.y * geo.pts_per_group;
+    const int p_end = min(npts, p_begin + geo.pts_per_group);
+
+    for (int i = threadIdx.x; i < n_hist * nh; i += kBatchThreads) hist[i] = 0.0;
+    build_bin_table(tab, edges, nb);
+    const BinView bt = bin_view(tab);
+
+    bool first_tile = true;
+    for (size_t tile = ev_begin; tile < ev_end || first_tile; tile += geo.te) {
+        // ---- stage one tile: E_true, w0, cell (a3b, a3c taken once per event) -------------------
+        const int m = tile < ev_end ? (int)min((size_t)geo.te, ev_end - tile) : 0;
+        const int m_pad = (m + 2 * kBatchThreads - 1) / (2 * kBatchThreads) * (2 * kBatchThreads);
+        for (int j = threadIdx.x; j < m_pad; j += kBatchThreads) {
+            double Et = 1.0, wv = 0.0;
+            unsigned short cc = kDropped;
+            if (j < m) {
+                const size_t g = tile + j;
+                const double e = ld_stream(E_true + g);
+                const double x = scaled_energy(energy_scale, ld_stream(E_reco + g));
+                const int ch = channel[g];
+                const int bin = find_bin(bt, x);
+                if (energy_ok(e) && (unsigned)ch < (unsigned)kChannels && bin >= 0) {
+                    Et = e;
+                    wv = ld_stream(w0 + g);
+                    cc = (unsigned short)((ch * nb + bin) | (ch << 12));
+                }
+            }
+            sEt[j] = Et;
+            sW[j] = wv;
+            sCell[j] = cc;
+        }
+        __syncthreads();
+
+        // ---- all points of the group over the staged tile ----------------------------------------
+        for (int p = p_begin; p < p_end; ++p) {
+            if (threadIdx.x < kBinArgsDoubles)
+                pbuf[threadIdx.x] = __ldg(points + (size_t)p * kBinArgsDoubles + threadIdx.x);
+            __syncthreads();
+            const OscSet set = load_set(pbuf);
+            for (int j = threadIdx.x; j < m_pad; j += 2 * kBatchThreads) {
+                const int j1 = j + kBatchThreads;
+                const unsigned cc0 = sCell[j], cc1 = sCell[j1];
+                const double Et0 = sEt[j], Et1 = sEt[j1];
+                const double wv0 = sW[j], wv1 = sW[j1];
+                const OscTrans tr0 = load_trans(pb, (cc0 >> 12) & 3u);
+                const OscTrans tr1 = load_trans(pb, (cc1 >> 12) & 3u);
+                const double P0 = prob_one(set, tr0, Et0);
+                const double P1 = prob_one(set, tr1, Et1);
+                const int cell0 = cc0 == kDropped ? -1 : (int)(cc0 & 0xFFFu);
+                const int cell1 = cc1 == kDropped ? -1 : (int)(cc1 & 0xFFFu);
+                warp_hist_add2(lh, cell0, __dmul_rn(wv0, P0), cell1, __dmul_rn(wv1, P1), lt_mask);
+            }
+            __syncthreads();
+            // sub-histograms summed in (warp, slot) order, cleared for the next point
+            double* dst = partial + ((size_t)p * geo.nchunks + chunk) * nh;
+            for (int i = threadIdx.x; i < nh; i += kBatchThreads) {
+                double s = 0.0;
+                for (int w = 0; w < n_hist; ++w) {
+                    s += hist[(size_t)w * nh + i];
+                    hist[(size_t)w * nh + i] = 0.0;
+                }
+                dst[i] = first_tile ? s : dst[i] + s;
+            }
+            // no barrier needed here: the parameter block and the tile arrays were last read before the
+            // barrier above, and the cleared histogram is next touched after the barrier that follows the
+            // next parameter-block load (or the next tile's staging barrier)
+        }
+        first_tile = false;
     }
-    __threadfence();
-    __syncthreads();
+}
 
-    // level 1: the last block of each group of kGroup consecutive blocks sums the group in block order
-    const int group = blockIdx.x / kGroup;
-    const int gfirst = group * kGroup;
-    const int gsize = min(kGroup, (int)gridDim.x - gfirst);
-    if (threadIdx.x == 0) s_ticket = atomicAdd(ms.counters + group, 1u);
-    __syncthreads();
-    if (s_ticket != (unsigned)(gsize - 1)) return;
-    __threadfence();
-    for (int i = threadIdx.x; i < nh; i += kBlock) {
-        const double* src = ms.partial + (size_t)gfirst * nh + i;
-        double s = __ldcg(src);
-#pragma unroll 8
-        for (int b = 1; b < gsize; ++b) s += __ldcg(src + (size_t)b * nh);
-        ms.gpartial[(size_t)group * nh + i] = s;
-    }
-    __threadfence();
-    __syncthreads();
-
-    // level 2: the last group to finish sums the groups in group order
-    if (threadIdx.x == 0) s_ticket = atomicAdd(ms.counters + ms.ngroups, 1u);
-    __syncthreads();
-    if (s_ticket != (unsigned)(ms.ngroups - 1)) return;
-    __threadfence();
-    for (int i = threadIdx.x; i < nh; i += kBlock) {
-        double s = __ldcg(ms.gpartial + i);
-#pragma unroll 8
-        for (int g = 1; g < ms.ngroups; ++g) s += __ldcg(ms.gpartial + (size_t)g * nh + i);
-        hist_out[i] = s;
+// out[p][i] = sum over chunks c (in order) of partial[p][c][i]
+__global__ void __launch_bounds__(256)
+merge_chunks_kernel(const double* __restrict__ partial, int nchunks, int nh, double* __restrict__ out)
+{
+    const size_t p = blockIdx.x;
+    const double* src = partial + p * (size_t)nchunks * nh;
+    for (int i = threadIdx.x; i < nh; i += blockDim.x) {
+        double s = src[i];
+        for (int c = 1; c < nchunks; ++c) s += src[(size_t)c * nh + i];
+        out[p * (size_t)nh + i] = s;
     }
 }
 

@@ -5,16 +5,28 @@
 // needs a handful of primitives on well-conditioned, range-limited arguments, so they are written out
 // here with exactly the work the method needs (op budget table):
 //   rcp_pos / rsqrt_pos : MUFU seed (upper 32 bits) + one third-order correction
-//   sincos_quarter      : argument already in units of pi/2 -> round, exact subtract, two degree-6
-//                         polynomials in f^2 (coefficients: osc_coeffs.h), quadrant fix-up on the
-//                         integer pipe
+//   sincos_quarter_mul  : sin, cos of (pi/2) a b -- the product is rounded to the nearest integer
+//                         and subtracted inside fused multiply-adds (exact residual), then two
+//                         degree-6 polynomials in f^2 (coefficients: osc_coeffs.h) and a quadrant
+//                         fix-up on the integer pipe
 //   cos_third_acos      : largest root t of 8 t^3 - 6 t = U (U = 2 cos(3 phi) in [0, 2]) by an fp32
 //                         polynomial seed and two chord-Newton steps -- replaces acos + cos.
+//
+// The fp64 pipe (16 lanes per SM sub-partition) is the resource that bounds the kernels, so everything
+// that can run elsewhere does: selections, sign flips and guards use integer instructions, the seed of
+// the cubic root runs on the fp32 pipe, and full-width fp64 constants live in __constant__ memory so
+// that DFMA reads them as a constant-bank operand instead of materialising them with two moves each.
 #pragma once
 #include <cuda_runtime.h>
 #include "osc_coeffs.h"
 
 namespace oscb {
+
+// [0..6] sin(pi/2 f)/f in z = f^2, [7..13] cos(pi/2 f) in z, [14] 1.5 * 2^52
+__constant__ double kPoly[15] = {
+    OSC_SINQ_0, OSC_SINQ_1, OSC_SINQ_2, OSC_SINQ_3, OSC_SINQ_4, OSC_SINQ_5, OSC_SINQ_6,
+    OSC_COSQ_0, OSC_COSQ_1, OSC_COSQ_2, OSC_COSQ_3, OSC_COSQ_4, OSC_COSQ_5, OSC_COSQ_6,
+    6755399441055744.0};
 
 __device__ __forceinline__ double mufu_rcp64(double a)
 {
@@ -27,6 +39,13 @@ __device__ __forceinline__ double mufu_rsqrt64(double a)
 {
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+    return y;
+}
+
+__device__ __forceinline__ float mufu_rcp32(float a)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(a));
     return y;
 }
 
@@ -56,65 +75,71 @@ __device__ __forceinline__ double flip_sign_if(double v, int cond_bit31)
     return __hiloint2double(__double2hiint(v) ^ cond_bit31, __double2loint(v));
 }
 
-// sin and cos of (pi/2) * hq for |hq| < 2^31.
-__device__ __forceinline__ void sincos_quarter(double hq, double& s, double& c)
+// max(v, 2^e) for v that is never NaN, decided on the upper word (integer pipe).  hi_floor is the upper
+// word of the power of two; values below it (including zero, denormals and negatives) are replaced.
+__device__ __forceinline__ double floor_at_pow2(double v, int hi_floor)
 {
-    const double MAGIC = 6755399441055744.0; // 1.5 * 2^52: adding it rounds hq to the nearest integer
-    double kd = hq + MAGIC;
-    int k = __double2loint(kd);
+    const int hi = __double2hiint(v);
+    const bool small = hi < hi_floor;
+    return __hiloint2double(small ? hi_floor : hi, small ? 0 : __double2loint(v));
+}
+
+// sin and cos of (pi/2) * a * b for |a b| < 2^31.
+__device__ __forceinline__ void sincos_quarter_mul(double a, double b, double& s, double& c)
+{
+    const double MAGIC = kPoly[14];          // adding 1.5 * 2^52 rounds to the nearest integer
+    double kd = fma(a, b, MAGIC);
+    const int k = __double2loint(kd);
     kd -= MAGIC;
-    double f = hq - kd; // exact, |f| <= 1/2
-    double z = f * f;
-    double ps = fma(OSC_SINQ_6, z, OSC_SINQ_5);
-    double pc = fma(OSC_COSQ_6, z, OSC_COSQ_5);
-    ps = fma(ps, z, OSC_SINQ_4);
-    pc = fma(pc, z, OSC_COSQ_4);
-    ps = fma(ps, z, OSC_SINQ_3);
-    pc = fma(pc, z, OSC_COSQ_3);
-    ps = fma(ps, z, OSC_SINQ_2);
-    pc = fma(pc, z, OSC_COSQ_2);
-    ps = fma(ps, z, OSC_SINQ_1);
-    pc = fma(pc, z, OSC_COSQ_1);
-    ps = fma(ps, z, OSC_SINQ_0);
-    pc = fma(pc, z, OSC_COSQ_0);
+    const double f = fma(a, b, -kd);         // exact product minus integer: |f| <= 1/2 (+ 1 ulp of a b)
+    const double z = f * f;
+    double ps = fma(kPoly[6], z, kPoly[5]);
+    double pc = fma(kPoly[13], z, kPoly[12]);
+    ps = fma(ps, z, kPoly[4]);
+    pc = fma(pc, z, kPoly[11]);
+    ps = fma(ps, z, kPoly[3]);
+    pc = fma(pc, z, kPoly[10]);
+    ps = fma(ps, z, kPoly[2]);
+    pc = fma(pc, z, kPoly[9]);
+    ps = fma(ps, z, kPoly[1]);
+    pc = fma(pc, z, kPoly[8]);
+    ps = fma(ps, z, kPoly[0]);
+    pc = fma(pc, z, 1.0);
     ps = ps * f;
     // quadrant: k odd swaps; sin negative for k & 2; cos negative for (k + 1) & 2
-    bool odd = (k & 1) != 0;
-    double ss = odd ? pc : ps;
-    double cc = odd ? ps : pc;
+    const bool odd = (k & 1) != 0;
+    const double ss = odd ? pc : ps;
+    const double cc = odd ? ps : pc;
     s = flip_sign_if(ss, (k & 2) << 30);
     c = flip_sign_if(cc, ((k + 1) & 2) << 30);
 }
 
 // t = cos(acos(U/2)/3) in [sqrt(3)/2, 1] for U in [0, 2], i.e. the largest root of 8 t^3 - 6 t = U,
 // and rh = 1 / (24 t^2 - 6) = 1 / (2 p'(t)) with p(t) = 4 t^3 - 3 t.
-// The seed and the slope reciprocal come from the fp32 pipe; two chord steps (same slope) take the
-// seed error (~1e-7) to ~1e-13 and ~1e-19; one third-order step makes rh fp64-accurate.
+// The seed (degree-5 polynomial, |error| < 1e-6 including fp32 rounding) and the slope reciprocal come
+// from the fp32 pipe; two chord steps with that fixed slope contract the error by ~3 e0 each
+// (e0 -> ~3e-12 -> ~1e-17); one third-order step makes rh fp64-accurate for the final t.
 __device__ __forceinline__ void cos_third_acos(double U, double& t_out, double& rh_out)
 {
-    float v = __double2float_rn(U) - 1.0f;
-    float tf = OSC_T0_9;
-    tf = fmaf(tf, v, OSC_T0_8);
-    tf = fmaf(tf, v, OSC_T0_7);
-    tf = fmaf(tf, v, OSC_T0_6);
-    tf = fmaf(tf, v, OSC_T0_5);
-    tf = fmaf(tf, v, OSC_T0_4);
-    tf = fmaf(tf, v, OSC_T0_3);
-    tf = fmaf(tf, v, OSC_T0_2);
-    tf = fmaf(tf, v, OSC_T0_1);
-    tf = fmaf(tf, v, OSC_T0_0);
-    float rf = __frcp_rn(fmaf(24.0f * tf, tf, -6.0f));
+    const float v = __double2float_rn(U) - 1.0f;
+    float tf = OSC_T5_5;
+    tf = fmaf(tf, v, OSC_T5_4);
+    tf = fmaf(tf, v, OSC_T5_3);
+    tf = fmaf(tf, v, OSC_T5_2);
+    tf = fmaf(tf, v, OSC_T5_1);
+    tf = fmaf(tf, v, OSC_T5_0);
+    const float rf = mufu_rcp32(fmaf(24.0f * tf, tf, -6.0f));
     double t = (double)tf;
-    double rh = (double)rf;
+    const double rh = (double)rf;
 #pragma unroll
     for (int it = 0; it < 2; ++it) {
-        double tt = t * t;
-        double a = fma(8.0, tt, -6.0);
-        double p2 = fma(a, t, -U);
+        const double tt = t * t;
+        const double a = fma(8.0, tt, -6.0);
+        const double p2 = fma(a, t, -U);
         t = fma(-p2, rh, t);
     }
-    double tt = t * t;
-    double pp = fma(24.0, tt, -6.0);
+    const double tt = t * t;
+    const double pp = fma(24.0, tt, -6.0);
     double d = fma(-pp, rh, 1.0);
     d = fma(d, d, d);
     rh_out = fma(rh, d, rh);

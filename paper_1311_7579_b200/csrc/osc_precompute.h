@@ -18,7 +18,7 @@ struct HostSet {
     osc_params p;
     std::complex<double> M[3][3];  // U diag(m2) U^dagger          (neutrinos; antineutrinos use conj)
     std::complex<double> M2[3][3]; // M M
-    double a;                      // K_MATTER Y_E rho             (A = +-a E)
+    double a = 0.0;                // K_MATTER Y_E rho             (A = +-a E)
     OscSet set;
 };
 
@@ -46,6 +46,7 @@ inline void precompute(const osc_params& p, HostSet& h)
     typedef std::complex<double> cd;
     const double PI = 3.14159265358979323846;
     h.p = p;
+    h.a = 0.0;
     const double s12 = std::sqrt(p.sin2_th12), c12 = std::sqrt(1.0 - p.sin2_th12);
     const double s23 = std::sqrt(p.sin2_th23), c23 = std::sqrt(1.0 - p.sin2_th23);
     const double s13 = std::sqrt(p.sin2_th13), c13 = std::sqrt(1.0 - p.sin2_th13);
@@ -113,6 +114,7 @@ inline OscTrans make_trans(const HostSet& h, int alpha, int beta, int antinu)
     t.T2i0 = sgn * m2.imag();
     t.T2r1 = lin.real();
     t.T2i1 = sgn * lin.imag();
+    t.pad = 0.0;
     return t;
 }
 
@@ -130,6 +132,7 @@ inline void channel_def(int ch, int& fin, int& fout, int& anti)
 inline void make_bin_args(const HostSet& h, BinArgs& b)
 {
     b.set = h.set;
+    b.pad = 0.0;
     for (int c = 0; c < kChannels; ++c) {
         int fin, fout, anti;
         channel_def(c, fin, fout, anti);

@@ -1,0 +1,51 @@
+// osc_smem.cuh -- explicit shared-memory accesses through 32-bit shared-window addresses.
+//
+// The hot loops index shared-memory tables with data-dependent offsets.  Going through generic
+// pointers makes the compiler rebuild the shared-window base (S2UR + ULEA) at many uses; a 32-bit
+// address obtained once with cvta and used with ld.shared / st.shared keeps the address arithmetic to a
+// single integer add.  The loads are declared non-volatile: the tables they read are written once before
+// a barrier; the histogram read-modify-writes use the volatile forms so that their order is preserved.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace oscb {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ unsigned long long lds_u64(uint32_t a)
+{
+    unsigned long long v;
+    asm("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint32_t lds_u16(uint32_t a)
+{
+    unsigned short v;
+    asm("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ double lds_f64(uint32_t a)
+{
+    double v;
+    asm("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ double2 lds_f64x2(uint32_t a)
+{
+    double2 v;
+    asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ double lds_f64_volatile(uint32_t a)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_f64_volatile(uint32_t a, double v)
+{
+    asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory");
+}
+
+} // namespace oscb

@@ -8,7 +8,7 @@
 namespace oscb {
 
 constexpr int kChannels = 4;     // OSC_N_CHANNELS
-constexpr int kTransFields = 9;  // doubles per OscTrans
+constexpr int kTransDoubles = 10; // doubles per OscTrans (9 used + 1 pad: whole 16-byte words in shared memory)
 
 // Energy-independent quantities of one parameter set that the eigenvalue solve needs.  The cubic's
 // coefficients depend on U only through |U_ei|^2, so the block serves neutrinos and antineutrinos.
@@ -28,6 +28,7 @@ struct OscTrans {
     double delta; // 1 if alpha == beta
     double ee;    // 1 if alpha == beta == e
     double Tr0, Ti0, T2r0, T2i0, T2r1, T2i1;
+    double pad;
 };
 
 // osc_prob: one transition.
@@ -43,10 +44,14 @@ struct ProbAllArgs {
     OscTrans tr[4]; // index 2*beta + alpha, alpha, beta in {0, 1}
 };
 
-// osc_reweight_bin: the four channels of include/osc.h.
+// osc_reweight_bin[_batch]: one parameter set with the four channels of include/osc.h.
+// 46 doubles = 23 16-byte words (set padded to 6 doubles).
 struct BinArgs {
     OscSet set;
+    double pad;
     OscTrans ch[kChannels];
 };
+constexpr int kBinArgsDoubles = 6 + kChannels * kTransDoubles;
+static_assert(sizeof(BinArgs) == sizeof(double) * kBinArgsDoubles, "BinArgs layout");
 
 } // namespace oscb

@@ -38,9 +38,12 @@ UNIT = "events/s"
 N_EVENTS = 10_000_000
 SCALES = wl.ENERGY_SCALES
 BYTES_PER_EVENT = 25          # E_true + E_reco + w0 (fp64) + channel (int8): SURVEY.md 8(d), DESIGN.md "k2"
-# fp64 operations the closed form executes per event in k2 (DFMA = 2, DADD/DMUL = 1), counted from the SASS of the
-# shipped kernel's event loop: DESIGN.md "k2: operation budget".
-FLOP_PER_EVENT = 201.0
+# fp64 operations k2 executes per event (DFMA = 2, DMUL/DADD = 1), counted by ncu
+# (smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum / events): DESIGN.md 5.1, profiles/r1_k2_full_a.md.
+FLOP_PER_EVENT = 205.8
+# dram__bytes_read.sum + dram__bytes_write.sum of one k2 launch over 1e7 events (same capture); algorithmic: 250.0e6
+NCU_TRAFFIC_BYTES_1E7 = 253.72e6
+NCU_TRAFFIC_SOURCE = "profiles/r1_k2_full_a.md"
 FP64_LANES_PER_SM_CLK = 64    # B200 (sm_100): 4 sub-partitions x 16 fp64 lanes; DESIGN.md "fp64 roofline"
 
 
@@ -192,6 +195,7 @@ def main():
 
     import paper_1311_7579_b200 as osc   # raises if libosc_b200.so is missing: no fallback
     from paper_1311_7579_b200 import build as _build
+    from paper_1311_7579_b200 import sharding
 
     _build.build_library()
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -222,8 +226,7 @@ def main():
         osc.osc_set_params(**par)                                                           # a1
         for k, s in enumerate(SCALES):
             osc.osc_reweight_bin(d_et, d_er, d_w0, d_ch, s, d_edges, hist_out=hist[k])      # a2a-a3c
-        if world > 1:
-            dist.all_reduce(hist)                                                           # 8(e)
+        sharding.allreduce_hist(hist)                                                       # 8(e): no-op at N = 1
 
     def barrier():
         if world > 1:
@@ -317,12 +320,16 @@ def main():
     sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
     nominal_tflops = sm_count * FP64_LANES_PER_SM_CLK * 2 * sm_max * 1e6 / 1e12
     achieved_tflops = n * FLOP_PER_EVENT / (k_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "achieved": achieved_tflops, "peak": fp64_peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved_tflops / fp64_peak_tflops, "traffic": None,
+    roofline = {"bound": "alu", "achieved": achieved_tflops, "peak": nominal_tflops, "unit": "TFLOP/s",
+                "frac": achieved_tflops / nominal_tflops,
+                "traffic": NCU_TRAFFIC_BYTES_1E7 if n == N_EVENTS else None,
+                "traffic_unit": f"DRAM bytes per launch, ncu ({NCU_TRAFFIC_SOURCE}); algorithmic {n * BYTES_PER_EVENT}",
                 "kernel": "reweight_bin_kernel (k2)", "kernel_ms": k_ms,
                 "flop_per_event": FLOP_PER_EVENT,
-                "peak_source": "DFMA-only probe kernel measured in this run (osc_fp64_peak_probe)",
-                "nominal_peak": nominal_tflops,
+                "peak_source": f"{sm_count} SMs x {FP64_LANES_PER_SM_CLK} fp64 lanes x 2 flop x {sm_max:.0f} MHz "
+                               "(unit counts and clocks.max.sm; DESIGN.md section 6)",
+                "peak_probe": fp64_peak_tflops, "frac_of_probe": achieved_tflops / fp64_peak_tflops,
+                "peak_probe_source": "DFMA-only probe kernel measured in this run (osc_fp64_peak_probe)",
                 "hbm": {"achieved": n * BYTES_PER_EVENT / (k_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
                         "frac": n * BYTES_PER_EVENT / (k_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": peak_src}}
 

@@ -53,9 +53,12 @@ def parse():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--events", type=int, default=N_EVENTS, help="events per GPU (default: configs[2], 1e7)")
+    ap.add_argument("--events", type=int, default=None, help="events per GPU (default: the size the config names)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--workload", default="config2", choices=["config0", "config1", "config2", "config3"],
+                    help="config2 (default) is the bench line; the others time the remaining BASELINE.json configs "
+                         "for BASELINE.md section 4 and give ncu a committed command for k1 / k1b / k3")
     return ap.parse_args()
 
 
@@ -184,10 +187,123 @@ def run_reference(args):
     }))
 
 
+# Per-config description of the secondary workloads: (events, units per event per step, bytes per unit, flop per unit)
+#   flop per unit: ncu-counted fp64 operations of the kernel that runs, bytes: algorithmic.
+OTHER = {
+    "config0": dict(n=100_000, kernel="prob_kernel (k1)", bytes_per_unit=16.0, flop_per_unit=200.0,
+                    what="configs[0]: 1e5 events, Table 1, P(numu->numu) and P(numu->nue) (2 osc_prob calls)"),
+    "config1": dict(n=10_000_000, kernel="prob_all_kernel (k1b)", bytes_per_unit=80.0, flop_per_unit=290.0,
+                    what="configs[1]: 1e7 events, all 9 transitions for nu and nubar (2 osc_prob_all calls = "
+                         "18 output arrays), delta_cp drawn per step, both hierarchies alternate"),
+    "config3": dict(n=1_000_000, kernel="reweight_batch_kernel (k3)", bytes_per_unit=25.0 / 1024, flop_per_unit=205.8,
+                    what="configs[3]: 1e6 events x 1024 oscillation points (32x32 grid of sin2_th23 x dm2_32, "
+                         "delta_cp per point) in ONE osc_reweight_bin_batch call"),
+}
+
+
+def run_other(args):
+    """Secondary workloads (one GPU): same JSON schema, unit = event (x point) evaluations per second."""
+    import torch
+
+    import paper_1311_7579_b200 as osc
+    from paper_1311_7579_b200 import build as _build
+
+    _build.build_library()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(0)
+    osc.osc_set_device(0)
+    dev = torch.device("cuda", 0)
+    cfg = OTHER[args.workload]
+    n = args.events or cfg["n"]
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)       # > L2 (126 MB)
+    if args.workload == "config0":
+        d_et = torch.from_numpy(wl.e_true(n, seed=0)).to(dev)
+        out = torch.empty((2, n), dtype=torch.float64, device=dev)
+        units = 2 * n
+
+        def step(i):
+            flush.fill_(i & 1)                                                  # inputs fit L2: flush between steps
+            osc.osc_set_params(**wl.table1())
+            osc.osc_prob(d_et, 1, 1, 0, P_out=out[0])
+            osc.osc_prob(d_et, 1, 0, 0, P_out=out[1])
+    elif args.workload == "config1":
+        d_et = torch.from_numpy(wl.e_true(n, seed=1)).to(dev)
+        out = torch.empty((2, 9, n), dtype=torch.float64, device=dev)
+        runs = wl.config1_runs()
+        units = 2 * n                                                           # (event, nu/nubar) solves; 9 outputs each
+
+        def step(i):
+            osc.osc_set_params(**runs[i % len(runs)])
+            osc.osc_prob_all(d_et, 0, P_out=out[0])
+            osc.osc_prob_all(d_et, 1, P_out=out[1])
+    else:
+        et, er, w0, ch = wl.events(n, seed=2)
+        d_et, d_er, d_w0, d_ch = (torch.from_numpy(a).to(dev) for a in (et, er, w0, ch))
+        d_edges = torch.from_numpy(wl.bin_edges()).to(dev)
+        pts = wl.scan_points()
+        out = torch.empty((len(pts), osc.N_CHANNELS, wl.N_BINS), dtype=torch.float64, device=dev)
+        units = n * len(pts)
+
+        def step(i):
+            osc.osc_reweight_bin_batch(pts, d_et, d_er, d_w0, d_ch, 1.0, d_edges, hist_out=out)
+
+    warm = max(args.warmup, 3)
+    for i in range(warm):
+        step(i)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    # per-step CUDA events so that the L2 flush of config0 stays outside the timed intervals
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    l0 = osc.osc_launch_count()
+    t0 = time.time()
+    for i, (a, b) in enumerate(evs):
+        if args.workload == "config0":
+            flush.fill_(i & 1)
+            a.record(stream)
+            osc.osc_set_params(**wl.table1())
+            osc.osc_prob(d_et, 1, 1, 0, P_out=out[0])
+            osc.osc_prob(d_et, 1, 0, 0, P_out=out[1])
+        else:
+            a.record(stream)
+            step(i)
+        b.record(stream)
+    torch.cuda.synchronize()
+    t1 = time.time()
+    launches = osc.osc_launch_count() - l0
+    ms = sum(a.elapsed_time(b) for a, b in evs)
+    clocks = sampler.stop(t0, t1)
+    value = units * args.steps / (ms * 1e-3)
+    hbm_peak, peak_src = peaks()
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
+    nominal = sm_count * FP64_LANES_PER_SM_CLK * 2 * sm_max * 1e6 / 1e12
+    tf = value * cfg["flop_per_unit"] / 1e12
+    gbs = value * cfg["bytes_per_unit"] / 1e9
+    hbm_bound = args.workload == "config1"
+    roof = ({"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+             "peak_source": peak_src} if hbm_bound else
+            {"bound": "alu", "achieved": tf, "peak": nominal, "unit": "TFLOP/s", "frac": tf / nominal,
+             "peak_source": "unit counts and clocks.max.sm (DESIGN.md section 6)"})
+    roof.update({"traffic": None, "kernel": cfg["kernel"], "flop_per_unit": cfg["flop_per_unit"],
+                 "bytes_per_unit": cfg["bytes_per_unit"], "alu_tflops": tf, "hbm_gbs": gbs,
+                 "note": "whole-step average (all launches of the step are this kernel)"
+                         + ("; launch-latency bound at this size, fractions are not kernel quality" if n < 1_000_000 else "")})
+    print(json.dumps({
+        "metric": METRIC, "value": value, "unit": "event evaluations/s", "n_gpus": 1, "steps": args.steps, "warmup": warm,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": cfg["what"], "events": n, "units_per_step": units,
+                                        "l2": "flushed between steps" if args.workload == "config0" else "working set > L2"},
+        "clocks": clocks, "e2e": None, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": None}))
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.workload != "config2":
+        run_other(args)
         return
 
     import torch
@@ -211,7 +327,7 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=device)
 
-    n = args.events
+    n = args.events or N_EVENTS
     par = wl.table1()
     et, er, w0, ch = wl.events(n, seed=2 + 1000 * rank)          # each rank its own shard (weak scaling)
     edges = wl.bin_edges()

@@ -209,7 +209,7 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     size_t per_sm = kSmemBudget / (smem + 1024);
     if (const char* e = getenv("OSC_TUNE_BPS")) per_sm = (size_t)atoi(e);
     if (per_sm < 1) per_sm = 1;
-    const size_t max_per_sm = threads == 256 ? kBlocksPerSM : 2 * kBlocksPerSM;
+    const size_t max_per_sm = threads == 256 ? 3 : 6;   // __launch_bounds__(THREADS, 768 / THREADS) of k2
     if (per_sm > max_per_sm && !getenv("OSC_TUNE_BPS")) per_sm = max_per_sm;
     const size_t ntiles = (n + 2 * threads - 1) / (2 * (size_t)threads);
     size_t g = (size_t)sms * per_sm;

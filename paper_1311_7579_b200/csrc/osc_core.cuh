@@ -18,7 +18,7 @@
 // The eigenvalues come from the trigonometric solution of the characteristic cubic
 // lam^3 - c2 lam^2 + c1 lam - c0 (BASELINE.json:north_star item 2): lam_k = c2/3 + (2/3) R tau_k with
 // R^2 = c2^2 - 3 c1 and tau the roots of 4 tau^3 - 3 tau = u, u = (2 c2^3 - 9 c2 c1 + 27 c0)/(2 R^3).
-// Only |u| is solved (largest root t, osc_math.cuh); for u < 0 the roots are negated and reversed.
+// Only |u| is solved (largest root t, osc_math.cuh); for u < 0 the roots are negated, which is R -> -R.
 #pragma once
 #include "osc_math.cuh"
 #include "osc_types.h"
@@ -33,8 +33,6 @@ struct OscEig {
     double sum01, prod01;  // lam0 + lam1, lam0 lam1
 };
 
-__device__ __forceinline__ double select_d(bool c, double a, double b) { return c ? a : b; }
-
 // Rows a2a-a2d: eigenvalues, gap phases and the two sinc-like factors for matter term A at 1/E.
 __device__ __forceinline__ void eig_solve(const OscSet& ps, double A, double invE, OscEig& o)
 {
@@ -47,7 +45,7 @@ __device__ __forceinline__ void eig_solve(const OscSet& ps, double A, double inv
     double c0_27 = A * ps.k0_27;
     double c1_3 = 3.0 * c1;
     double R2 = fma(c2, c2, -c1_3);             // (1/2) sum of squared gaps: > 0 for every valid parameter set
-    R2 = floor_at_pow2(R2, 0x03000000);         // (DESIGN.md "R2 > 0"); the floor 2^-975 only keeps NaN out
+    R2 = floor_hi_word(R2, 0x03000000);         // (DESIGN.md "R2 > 0"); the floor 2^-975 only keeps NaN out
     double tq = fma(2.0, R2, -c1_3);            // 2 c2^2 - 9 c1
     double q = fma(c2, tq, c0_27);              // 2 c2^3 - 9 c2 c1 + 27 c0
 
@@ -55,48 +53,47 @@ __device__ __forceinline__ void eig_solve(const OscSet& ps, double A, double inv
     double rinv = rsqrt_pos(R2);
     double rinv2 = rinv * rinv;
     double U2 = (q * rinv) * rinv2;             // 2 u = 2 cos(3 phi)
-    bool neg = __double2hiint(U2) < 0;
+    const int sgn = __double2hiint(U2) & 0x80000000; // sign of u: for u < 0 the roots of |u| are negated, i.e. R -> -R
     double t, rh;
     cos_third_acos(fabs(U2), t, rh);            // t = cos(phi'), rh = 1 / (24 t^2 - 6)
     double om = 1.0 - t;
     double w = fma(om, t, om);                  // 1 - t^2 = sin^2(phi')
-    w = floor_at_pow2(w, 0x39B00000);           // >= 2^-100: a closed gap stays finite (sinc form below)
+    w = floor_hi_word(w, 0x39B00000);           // >= 2^-100: a closed gap stays finite (sinc form below)
     double y = rsqrt_pos(w);
     double s = w * y;                           // sin(phi')
-    double ga = fma(-HALF_SQ3, s, 1.5 * t);     // gaps in units of (2/3) R:  ga >= gb, ga + gb = largest gap
+    // roots of 4 tau^3 - 3 tau = |u|: t >= t - ga >= -m; gaps (in units of (2/3) R) ga >= gb >= 0
+    double ga = fma(-HALF_SQ3, s, 1.5 * t);
     double gb = SQ3 * s;
     double m = fma(HALF_SQ3, s, 0.5 * t);
-    double tau0 = select_d(neg, m, t);
-    double tau2 = select_d(neg, -t, -m);
 
-    double R = R2 * rinv;
+    // signed radius: eigenvalue "0" is c2/3 + Rs t, eigenvalue "2" is c2/3 - Rs m; for u < 0 that labelling runs
+    // upwards instead of downwards, which the projector form does not care about (all gaps change sign together)
+    double R = flip_sign_if(R2 * rinv, sgn);
     double Rs = R * (2.0 / 3.0);
     double c2_3 = c2 * (1.0 / 3.0);
-    double lam0 = fma(Rs, tau0, c2_3);
-    double lam2 = fma(Rs, tau2, c2_3);
+    double lam0 = fma(Rs, t, c2_3);
+    double lam2 = fma(-Rs, m, c2_3);
     o.sum12 = c2 - lam0;
     o.prod12 = fma(-lam0, o.sum12, c1);
     o.sum01 = c2 - lam2;
     o.prod01 = fma(-lam2, o.sum01, c1);
 
-    // 1/(g_small_pair g02) and 1/(g_big_pair g02): ga (ga + gb) = 3 t^2 - 3/4 = (24 t^2 - 6) / 8
+    // 2/(g01 g02) and 2/(g12 g02) (sign-free products of two gaps): ga (ga + gb) = 3 t^2 - 3/4 = (24 t^2 - 6) / 8
     double rr = rh * rinv2;
     double ka = 36.0 * rr;                                  // 2 / (Rs^2 ga gc)
     double kb = (rr * (36.0 / SQ3)) * (ga * y);             // 2 / (Rs^2 gb gc)
 
-    // a2d gap phases in quarter turns: g R xq23 / E
+    // a2d gap phases in quarter turns: g R xq23 / E (signed with R)
     double RX = R * (ps.xq23 * invE);
-    double ha = select_d(neg, gb, ga);
-    double hb = select_d(neg, ga, gb);
     double s1, c1c, s12, c12;
-    sincos_quarter_mul(ha, RX, s1, c1c);
-    sincos_quarter_mul(hb, RX, s12, c12);
+    sincos_quarter_mul(ga, RX, s1, c1c);
+    sincos_quarter_mul(gb, RX, s12, c12);
     o.s1h = s1;
     o.c1h = c1c;
     o.c02 = fma(c1c, c12, -(s1 * s12));
     o.s02 = fma(s1, c12, c1c * s12);
-    o.kap0 = s1 * select_d(neg, kb, ka);
-    o.kap2 = s12 * select_d(neg, ka, kb);
+    o.kap0 = s1 * ka;
+    o.kap2 = s12 * kb;
 }
 
 // Rows a2e-a2f: |Z_{beta alpha}|^2 for one transition.

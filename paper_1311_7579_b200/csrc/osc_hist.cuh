@@ -39,24 +39,56 @@ __device__ __forceinline__ LaneHist lane_hist(const double* hist, int nh, int n_
     return lh;
 }
 
-// cell0 / cell1: histogram cell of the lane's slot-0 / slot-1 event, or -1 for a dropped event.
+// The accumulation of one warp iteration is split in two so that the latency of MATCH and of the first
+// shared-memory read is hidden behind the probability arithmetic (the cell of an event is known before its
+// weight): warp_hist_plan ranks the lanes and pre-reads the word of every rank-0 lane, warp_hist_commit adds
+// the weights.  Nothing but this warp ever touches its sub-histograms, so the pre-read value is still current
+// at commit time.  cell0 / cell1: histogram cell of the lane's slot-0 / slot-1 event, or -1 for a dropped event.
+struct HistPlan {
+    uint32_t a0, a1;   // shared-window byte address of the target word (all ones: dropped)
+    int r0, r1;        // rank among the lanes of the warp that hit the same word (-1: dropped)
+    int rmax;          // warp-uniform maximum rank
+    double v0, v1;     // current content of the word, valid for rank 0
+};
+
+__device__ __forceinline__ HistPlan warp_hist_plan(const LaneHist& lh, int cell0, int cell1, unsigned lt_mask)
+{
+    const unsigned FULL = 0xffffffffu;
+    HistPlan p;
+    p.a0 = cell0 >= 0 ? lh.h0 + 8u * (unsigned)cell0 : 0xFFFFFFFFu;
+    p.a1 = cell1 >= 0 ? lh.h1 + 8u * (unsigned)cell1 : 0xFFFFFFFFu;
+    const unsigned p0 = __match_any_sync(FULL, p.a0);
+    const unsigned p1 = __match_any_sync(FULL, p.a1);
+    p.r0 = cell0 >= 0 ? __popc(p0 & lt_mask) : -1;
+    p.r1 = cell1 >= 0 ? __popc(p1 & lt_mask) : -1;
+    p.rmax = __reduce_max_sync(FULL, max(p.r0, p.r1));
+    p.v0 = 0.0;
+    p.v1 = 0.0;
+    if (p.r0 == 0) p.v0 = lds_f64_volatile(p.a0);
+    if (p.r1 == 0) p.v1 = lds_f64_volatile(p.a1);
+    return p;
+}
+
+// Phase 0 stores the pre-read words plus the weights; phase r = 1, 2, ... lets exactly the lanes of rank r do a plain
+// read-modify-write: inside a phase all addresses are distinct, and for one address the additions happen in lane order.
+__device__ __forceinline__ void warp_hist_commit(const HistPlan& p, double w0, double w1)
+{
+    if (p.r0 == 0) sts_f64_volatile(p.a0, p.v0 + w0);
+    if (p.r1 == 0) sts_f64_volatile(p.a1, p.v1 + w1);
+    __syncwarp();
+#pragma unroll 1
+    for (int ph = 1; ph <= p.rmax; ++ph) {
+        if (p.r0 == ph) sts_f64_volatile(p.a0, lds_f64_volatile(p.a0) + w0);
+        if (p.r1 == ph) sts_f64_volatile(p.a1, lds_f64_volatile(p.a1) + w1);
+        __syncwarp();
+    }
+}
+
 __device__ __forceinline__ void warp_hist_add2(const LaneHist& lh, int cell0, double w0, int cell1, double w1,
                                                unsigned lt_mask)
 {
-    const unsigned FULL = 0xffffffffu;
-    const uint32_t a0 = cell0 >= 0 ? lh.h0 + 8u * (unsigned)cell0 : 0xFFFFFFFFu;
-    const uint32_t a1 = cell1 >= 0 ? lh.h1 + 8u * (unsigned)cell1 : 0xFFFFFFFFu;
-    const unsigned p0 = __match_any_sync(FULL, a0);
-    const unsigned p1 = __match_any_sync(FULL, a1);
-    const int r0 = cell0 >= 0 ? __popc(p0 & lt_mask) : -1;
-    const int r1 = cell1 >= 0 ? __popc(p1 & lt_mask) : -1;
-    const int rmax = __reduce_max_sync(FULL, max(r0, r1));
-#pragma unroll 1
-    for (int ph = 0; ph <= rmax; ++ph) {
-        if (r0 == ph) sts_f64_volatile(a0, lds_f64_volatile(a0) + w0);
-        if (r1 == ph) sts_f64_volatile(a1, lds_f64_volatile(a1) + w1);
-        __syncwarp();
-    }
+    const HistPlan p = warp_hist_plan(lh, cell0, cell1, lt_mask);
+    warp_hist_commit(p, w0, w1);
 }
 
 // Scratch of one call: counters[ngroups + 1] | partial[grid][nh] | gpartial[ngroups][nh].  It lives in a

@@ -181,28 +181,65 @@ __device__ __forceinline__ OscSet load_set(const double* pb)
     return s;
 }
 
-// Per-event part of k2: the histogram cell (channel * nb + bin, or -1 if the event is dropped, A8/A11)
-// and the weight w0 * P_channel(E_true).
-__device__ __forceinline__ void reweight_one(const OscSet& set, uint32_t pb, const BinView& bt,
-                                             double energy_scale, bool in, double Et, double Er, double wp, int ch,
-                                             int& cell, double& w)
+// Per-event part of k2 that does not need the probability: the histogram cell (channel * nb + bin, or -1 if the
+// event is dropped, A8/A11), the channel whose transition block is to be used and the energy handed to the closed form.
+__device__ __forceinline__ void locate_one(const BinView& bt, double energy_scale, bool in, double Et, double Er,
+                                           int ch, int& cell, int& c, double& Es)
 {
     const double x = scaled_energy(energy_scale, Er);       // a3b: one rounded fp64 multiply
     const int bin = find_bin(bt, x);                        // a3c: bit-exact index
     const bool ok = in && energy_ok(Et) && (unsigned)ch < (unsigned)kChannels && bin >= 0;
-    const int c = ok ? ch : 0;
-    const OscTrans tr = load_trans(pb, c);
-    const double P = prob_one(set, tr, ok ? Et : 1.0);      // a2a-a2f
-    w = __dmul_rn(wp, P);                                   // a3a
+    c = ok ? ch : 0;
+    Es = ok ? Et : 1.0;
     cell = ok ? c * bt.nb + bin : -1;
+}
+
+// Two events of one thread as they come from global memory (VEC: events 2i, 2i+1 by 128-bit loads).
+struct EventPair {
+    double Et0, Et1, Er0, Er1, wp0, wp1;
+    int ch0, ch1;
+};
+
+template <bool VEC, int THREADS>
+__device__ __forceinline__ EventPair load_pair(const double* __restrict__ E_true, const double* __restrict__ E_reco,
+                                               const double* __restrict__ w0, const int8_t* __restrict__ channel,
+                                               size_t n, size_t tile, size_t& j0, size_t& j1)
+{
+    const size_t base = tile * (2 * THREADS);
+    j0 = VEC ? base + 2 * threadIdx.x : base + threadIdx.x;
+    j1 = VEC ? j0 + 1 : j0 + THREADS;
+    const bool in0 = j0 < n, in1 = j1 < n;
+    EventPair e;
+    if (VEC && in1) {
+        const double2 vt = ld_stream2(E_true + j0), vr = ld_stream2(E_reco + j0), vw = ld_stream2(w0 + j0);
+        const unsigned short vc = __ldcs(reinterpret_cast<const unsigned short*>(channel + j0));
+        e.Et0 = vt.x; e.Et1 = vt.y;
+        e.Er0 = vr.x; e.Er1 = vr.y;
+        e.wp0 = vw.x; e.wp1 = vw.y;
+        e.ch0 = (int)(signed char)(vc & 0xffu);
+        e.ch1 = (int)(signed char)(vc >> 8);
+    } else {
+        e.Et0 = in0 ? ld_stream(E_true + j0) : 1.0;
+        e.Et1 = in1 ? ld_stream(E_true + j1) : 1.0;
+        e.Er0 = in0 ? ld_stream(E_reco + j0) : 0.0;
+        e.Er1 = in1 ? ld_stream(E_reco + j1) : 0.0;
+        e.wp0 = in0 ? ld_stream(w0 + j0) : 0.0;
+        e.wp1 = in1 ? ld_stream(w0 + j1) : 0.0;
+        e.ch0 = in0 ? (int)channel[j0] : -1;
+        e.ch1 = in1 ? (int)channel[j1] : -1;
+    }
+    return e;
 }
 
 // ------------------------------------------------------------------------------------------------
 // k2: fused reweight + histogram, one parameter set.
 // Shared memory per block:  param block | bin table | hist[warps][kSlots][n_sub][4 * nb]
+// The loop is software-pipelined by hand: the loads of the block's next tile are issued before the arithmetic
+// of the current one (the kernel is bound by instruction issue around the fp64 pipe, so a warp that sits on a
+// global load is an issue slot lost), and the histogram ranking (MATCH + first read) precedes the closed form.
 // ------------------------------------------------------------------------------------------------
 template <bool VEC, int THREADS>
-__global__ void __launch_bounds__(THREADS, 1024 / THREADS)
+__global__ void __launch_bounds__(THREADS, 768 / THREADS)
 reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict__ E_true,
                     const double* __restrict__ E_reco, const double* __restrict__ w0,
                     const int8_t* __restrict__ channel, size_t n, double energy_scale,
@@ -222,6 +259,10 @@ reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict_
     const unsigned lt_mask = (1u << lane) - 1u;
     const int n_hist = WARPS * kSlots * n_sub;
 
+    const size_t ntiles = (n + 2 * THREADS - 1) / (2 * THREADS);
+    size_t t = blockIdx.x, j0 = 0, j1 = 0;
+    EventPair cur = load_pair<VEC, THREADS>(E_true, E_reco, w0, channel, n, t, j0, j1);   // grid <= ntiles
+
     if (threadIdx.x < kBinArgsDoubles) pbuf[threadIdx.x] = reinterpret_cast<const double*>(&a)[threadIdx.x];
     for (int i = threadIdx.x; i < n_hist * nh; i += THREADS) hist[i] = 0.0;
     build_bin_table(tab, edges, nb);
@@ -229,37 +270,22 @@ reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict_
     const uint32_t pb = smem_u32(pbuf);
     const LaneHist lh = lane_hist(hist, nh, n_sub, warp, lane);
 
-    const size_t ntiles = (n + 2 * THREADS - 1) / (2 * THREADS);
-    for (size_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
-        const size_t base = t * (2 * THREADS);
-        const size_t j0 = VEC ? base + 2 * threadIdx.x : base + threadIdx.x;
-        const size_t j1 = VEC ? j0 + 1 : j0 + THREADS;
+    while (t < ntiles) {
         const bool in0 = j0 < n, in1 = j1 < n;
-        double Et0, Et1, Er0, Er1, wp0, wp1;
-        int ch0, ch1;
-        if (VEC && in1) {
-            const double2 vt = ld_stream2(E_true + j0), vr = ld_stream2(E_reco + j0), vw = ld_stream2(w0 + j0);
-            const unsigned short vc = __ldcs(reinterpret_cast<const unsigned short*>(channel + j0));
-            Et0 = vt.x; Et1 = vt.y;
-            Er0 = vr.x; Er1 = vr.y;
-            wp0 = vw.x; wp1 = vw.y;
-            ch0 = (int)(signed char)(vc & 0xffu);
-            ch1 = (int)(signed char)(vc >> 8);
-        } else {
-            Et0 = in0 ? ld_stream(E_true + j0) : 1.0;
-            Et1 = in1 ? ld_stream(E_true + j1) : 1.0;
-            Er0 = in0 ? ld_stream(E_reco + j0) : 0.0;
-            Er1 = in1 ? ld_stream(E_reco + j1) : 0.0;
-            wp0 = in0 ? ld_stream(w0 + j0) : 0.0;
-            wp1 = in1 ? ld_stream(w0 + j1) : 0.0;
-            ch0 = in0 ? (int)channel[j0] : -1;
-            ch1 = in1 ? (int)channel[j1] : -1;
-        }
-        int cell0, cell1;
-        double w_0, w_1;
-        reweight_one(a.set, pb, bt, energy_scale, in0, Et0, Er0, wp0, ch0, cell0, w_0);
-        reweight_one(a.set, pb, bt, energy_scale, in1, Et1, Er1, wp1, ch1, cell1, w_1);
-        warp_hist_add2(lh, cell0, w_0, cell1, w_1, lt_mask);
+        int cell0, cell1, c0, c1;
+        double Es0, Es1;
+        locate_one(bt, energy_scale, in0, cur.Et0, cur.Er0, cur.ch0, cell0, c0, Es0);
+        locate_one(bt, energy_scale, in1, cur.Et1, cur.Er1, cur.ch1, cell1, c1, Es1);
+        const HistPlan plan = warp_hist_plan(lh, cell0, cell1, lt_mask);
+        const double wp0 = cur.wp0, wp1 = cur.wp1;
+        // prefetch: E_true, E_reco and channel of the current pair are dead from here on
+        t += gridDim.x;
+        if (t < ntiles) cur = load_pair<VEC, THREADS>(E_true, E_reco, w0, channel, n, t, j0, j1);
+        const OscTrans tr0 = load_trans(pb, c0);
+        const OscTrans tr1 = load_trans(pb, c1);
+        const double P0 = prob_one(a.set, tr0, Es0);        // a2a-a2f
+        const double P1 = prob_one(a.set, tr1, Es1);
+        warp_hist_commit(plan, __dmul_rn(wp0, P0), __dmul_rn(wp1, P1));   // a3a, a3c
     }
     block_merge(hist, n_hist, nh, ms, hist_out, &s_ticket);
 }

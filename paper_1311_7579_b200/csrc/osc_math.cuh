@@ -84,6 +84,14 @@ __device__ __forceinline__ double floor_at_pow2(double v, int hi_floor)
     return __hiloint2double(small ? hi_floor : hi, small ? 0 : __double2loint(v));
 }
 
+// v raised to at least 2^e by one integer max on the upper word (hi_floor = upper word of 2^e): zero, denormals,
+// negatives and anything else below 2^e come out in [2^e, 2^(e+1)) -- the low word is kept, the result is only used
+// where "some positive number of that size" is all that matters.  v must not be NaN.
+__device__ __forceinline__ double floor_hi_word(double v, int hi_floor)
+{
+    return __hiloint2double(max(__double2hiint(v), hi_floor), __double2loint(v));
+}
+
 // sin and cos of (pi/2) * a * b for |a b| < 2^31.
 __device__ __forceinline__ void sincos_quarter_mul(double a, double b, double& s, double& c)
 {

@@ -28,10 +28,10 @@ namespace oscb {
 
 constexpr int kLutCells = 2048;
 constexpr int kKeySentinels = 3;
-constexpr unsigned long long kKeyMax = 0xFFFFFFFFFFFFFFFFull;
+constexpr long long kKeyMax = 0x7FFFFFFFFFFFFFFFll;
 
 struct BinHead {
-    unsigned int base;   // upper key word where cell 0 starts
+    int base;            // upper key word where cell 0 starts
     unsigned int shift;  // cell = (upper key word - base) >> shift
     unsigned int nb;
     unsigned int steps;  // forward steps that finish the search from lut[cell], maximum over all cells
@@ -48,14 +48,22 @@ __host__ __device__ inline size_t bin_table_bytes(int nb)
     return bin_lut_offset(nb) + sizeof(unsigned short) * (size_t)kLutCells;
 }
 
-// Unsigned key: a < b as doubles  <=>  key(a) < key(b) for all non-NaN a, b, and key(-0.0) == key(+0.0).
-// Non-negative values keep their bit pattern with the top bit set; negative values map to the two's
-// complement of their bit pattern (2^63 - magnitude).  Positive NaNs sort above +inf, negative NaNs
-// below -inf: either way outside every bin.
-__device__ __forceinline__ unsigned long long order_key(double v)
+// Signed key: a < b as doubles  <=>  key(a) < key(b) for all non-NaN a, b.  Non-negative values keep their bit
+// pattern; negative values have their 63 magnitude bits inverted (key = -1 - magnitude), three integer
+// instructions on the two words.  That puts -0.0 at -1, just below +0.0 at 0, although the two compare equal as
+// doubles; the table therefore stores an edge that is +-0.0 as -1 (edge_key), which makes
+// "edge <= x" and "x < edge" come out as in IEEE for x = -0.0 and x = +0.0 alike.  Positive NaNs sort above
+// +inf, negative NaNs below -inf: either way outside every bin.
+__device__ __forceinline__ long long order_key(double v)
 {
-    const unsigned long long b = (unsigned long long)__double_as_longlong(v);
-    return ((long long)b < 0) ? (0ull - b) : (b | 0x8000000000000000ull);
+    const int hi = __double2hiint(v), lo = __double2loint(v);
+    const int m = hi >> 31;                                  // all ones for a set sign bit
+    return (long long)(((unsigned long long)(unsigned)(hi ^ (m & 0x7FFFFFFF)) << 32) | (unsigned)(lo ^ m));
+}
+__device__ __forceinline__ long long edge_key(double v)
+{
+    const long long k = order_key(v);
+    return k == 0 ? -1ll : k;
 }
 
 // x = fl64(energy_scale * E_reco) (row a3b): one rounded fp64 multiply, never contracted into an fma.
@@ -67,10 +75,11 @@ __device__ __forceinline__ double scaled_energy(double energy_scale, double E_re
 struct BinView {                       // 32-bit shared-window addresses into the shared-memory copy of the table
     uint32_t ekey;
     uint32_t lut;
-    unsigned int base, shift;
+    int base;
+    unsigned int shift;
     int nb;
-    bool two_steps;                    // two forward steps are enough for every cell
-    unsigned long long key0;           // key(edges[0])
+    unsigned int steps;                // forward steps that finish the search from lut[cell] (block-uniform)
+    long long key0;                    // key(edges[0])
 };
 
 __device__ __forceinline__ BinView bin_view(const unsigned char* smem_table)
@@ -80,25 +89,26 @@ __device__ __forceinline__ BinView bin_view(const unsigned char* smem_table)
     v.base = h->base;
     v.shift = h->shift;
     v.nb = (int)h->nb;
-    v.two_steps = h->steps <= 2u;
+    v.steps = h->steps;
     v.ekey = smem_u32(smem_table + bin_keys_offset());
     v.lut = smem_u32(smem_table + bin_lut_offset(v.nb));
-    v.key0 = *reinterpret_cast<const unsigned long long*>(smem_table + bin_keys_offset());
+    v.key0 = *reinterpret_cast<const long long*>(smem_table + bin_keys_offset());
     return v;
 }
 
-// The unique i with edges[i] <= x < edges[i+1], or -1.
+// The unique i with edges[i] <= x < edges[i+1], or -1.  t.steps is the same for all threads of the block, so the
+// branches on it are uniform; a sane binning needs one step.
 __device__ __forceinline__ int find_bin(const BinView& t, double x)
 {
-    const unsigned long long kx = order_key(x);
-    const unsigned int khi = (unsigned int)(kx >> 32);
-    const unsigned int rel = max(khi, t.base) - t.base;
+    const long long kx = order_key(x);
+    const int khi = (int)(kx >> 32);
+    const unsigned int rel = (unsigned int)max(khi, t.base) - (unsigned int)t.base;
     const unsigned int cell = min(rel >> t.shift, (unsigned int)(kLutCells - 1));
     int lo = (int)lds_u16(t.lut + 2u * cell);
-    lo += (lds_u64(t.ekey + 8u * (unsigned)(lo + 1)) <= kx) ? 1 : 0;   // sentinels keep these reads inside the table
-    lo += (lds_u64(t.ekey + 8u * (unsigned)(lo + 1)) <= kx) ? 1 : 0;
-    if (!t.two_steps) {                                               // uniform; not taken for sane binnings
-        while (lo < t.nb && lds_u64(t.ekey + 8u * (unsigned)(lo + 1)) <= kx) ++lo;
+    if (t.steps >= 1u) lo += ((long long)lds_u64(t.ekey + 8u * (unsigned)(lo + 1)) <= kx) ? 1 : 0;   // sentinels keep these
+    if (t.steps >= 2u) lo += ((long long)lds_u64(t.ekey + 8u * (unsigned)(lo + 1)) <= kx) ? 1 : 0;   // reads inside the table
+    if (t.steps > 2u) {
+        while (lo < t.nb && (long long)lds_u64(t.ekey + 8u * (unsigned)(lo + 1)) <= kx) ++lo;
     }
     return (lo < t.nb && t.key0 <= kx) ? lo : -1;
 }
@@ -107,17 +117,17 @@ __device__ __forceinline__ int find_bin(const BinView& t, double x)
 // barriers); about 2 us per block, once per kernel.
 __device__ __forceinline__ void build_bin_table(unsigned char* smem_table, const double* __restrict__ edges, int nb)
 {
-    unsigned long long* key = reinterpret_cast<unsigned long long*>(smem_table + bin_keys_offset());
+    long long* key = reinterpret_cast<long long*>(smem_table + bin_keys_offset());
     unsigned short* lut = reinterpret_cast<unsigned short*>(smem_table + bin_lut_offset(nb));
     BinHead* head = reinterpret_cast<BinHead*>(smem_table);
 
     for (int i = threadIdx.x; i < nb + 1 + kKeySentinels; i += blockDim.x)
-        key[i] = (i <= nb) ? order_key(__ldg(edges + i)) : kKeyMax;
+        key[i] = (i <= nb) ? edge_key(__ldg(edges + i)) : kKeyMax;
     __syncthreads();
     if (threadIdx.x == 0) {
-        const unsigned int lo = (unsigned int)(key[nb > 1 ? 1 : 0] >> 32);
-        const unsigned int hi = (unsigned int)(key[nb] >> 32);
-        const unsigned int span = hi > lo ? hi - lo : 0u;
+        const int lo = (int)(key[nb > 1 ? 1 : 0] >> 32);
+        const int hi = (int)(key[nb] >> 32);
+        const unsigned int span = hi > lo ? (unsigned int)hi - (unsigned int)lo : 0u;
         unsigned int shift = 0;
         while ((span >> shift) >= (unsigned int)kLutCells) ++shift;
         head->base = lo;
@@ -126,11 +136,12 @@ __device__ __forceinline__ void build_bin_table(unsigned char* smem_table, const
         head->steps = 0u;
     }
     __syncthreads();
-    const unsigned int base = head->base, shift = head->shift;
+    const int base = head->base;
+    const unsigned int shift = head->shift;
     for (int c = threadIdx.x; c < kLutCells; c += blockDim.x) {
-        unsigned long long start_hi = (unsigned long long)base + ((unsigned long long)c << shift);
-        if (start_hi > 0xFFFFFFFFull) start_hi = 0xFFFFFFFFull;
-        const unsigned long long start = start_hi << 32;
+        long long start_hi = (long long)base + ((long long)c << shift);                // first upper key word of cell c
+        if (start_hi > 0x7FFFFFFFll) start_hi = 0x7FFFFFFFll;
+        const long long start = start_hi * 4294967296ll;
         int lo = 0, hi = nb;                                   // largest i in [0, nb] with key[i] <= start, else 0
         while (lo < hi) {
             const int mid = (lo + hi + 1) >> 1;

@@ -46,26 +46,40 @@ __device__ __forceinline__ LaneHist lane_hist(const double* hist, int nh, int n_
 // at commit time.  cell0 / cell1: histogram cell of the lane's slot-0 / slot-1 event, or -1 for a dropped event.
 struct HistPlan {
     uint32_t a0, a1;   // shared-window byte address of the target word (all ones: dropped)
-    int r0, r1;        // rank among the lanes of the warp that hit the same word (-1: dropped)
+    unsigned m0, m1;   // lanes of the warp that target the same word (MATCH.ANY)
+    int r0, r1;        // rank among those lanes (-1: dropped)
     int rmax;          // warp-uniform maximum rank
     double v0, v1;     // current content of the word, valid for rank 0
 };
 
-__device__ __forceinline__ HistPlan warp_hist_plan(const LaneHist& lh, int cell0, int cell1, unsigned lt_mask)
+// Step 1 (as early as the cells are known): addresses and MATCH.
+__device__ __forceinline__ void warp_hist_match(HistPlan& p, const LaneHist& lh, int cell0, int cell1)
 {
     const unsigned FULL = 0xffffffffu;
-    HistPlan p;
     p.a0 = cell0 >= 0 ? lh.h0 + 8u * (unsigned)cell0 : 0xFFFFFFFFu;
     p.a1 = cell1 >= 0 ? lh.h1 + 8u * (unsigned)cell1 : 0xFFFFFFFFu;
-    const unsigned p0 = __match_any_sync(FULL, p.a0);
-    const unsigned p1 = __match_any_sync(FULL, p.a1);
-    p.r0 = cell0 >= 0 ? __popc(p0 & lt_mask) : -1;
-    p.r1 = cell1 >= 0 ? __popc(p1 & lt_mask) : -1;
+    p.m0 = __match_any_sync(FULL, p.a0);
+    p.m1 = __match_any_sync(FULL, p.a1);
+}
+
+// Step 2 (once MATCH has had time to come back): ranks and the pre-read of the rank-0 lanes.
+__device__ __forceinline__ void warp_hist_rank(HistPlan& p, unsigned lt_mask)
+{
+    const unsigned FULL = 0xffffffffu;
+    p.r0 = p.a0 != 0xFFFFFFFFu ? __popc(p.m0 & lt_mask) : -1;
+    p.r1 = p.a1 != 0xFFFFFFFFu ? __popc(p.m1 & lt_mask) : -1;
     p.rmax = __reduce_max_sync(FULL, max(p.r0, p.r1));
     p.v0 = 0.0;
     p.v1 = 0.0;
     if (p.r0 == 0) p.v0 = lds_f64_volatile(p.a0);
     if (p.r1 == 0) p.v1 = lds_f64_volatile(p.a1);
+}
+
+__device__ __forceinline__ HistPlan warp_hist_plan(const LaneHist& lh, int cell0, int cell1, unsigned lt_mask)
+{
+    HistPlan p;
+    warp_hist_match(p, lh, cell0, cell1);
+    warp_hist_rank(p, lt_mask);
     return p;
 }
 

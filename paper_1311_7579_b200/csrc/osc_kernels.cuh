@@ -183,41 +183,42 @@ __device__ __forceinline__ OscSet load_set(const double* pb)
 
 // Per-event part of k2 that does not need the probability: the histogram cell (channel * nb + bin, or -1 if the
 // event is dropped, A8/A11), the channel whose transition block is to be used and the energy handed to the closed form.
-__device__ __forceinline__ void locate_one(const BinView& bt, double energy_scale, bool in, double Et, double Er,
-                                           int ch, int& cell, int& c, double& Es)
+// ch is the channel byte zero-extended: 0..3 are valid, every other code (negative int8 values, the 0xFF that
+// load_pair puts in for events past the end) is not.
+__device__ __forceinline__ void locate_one(const BinView& bt, double energy_scale, double Et, double Er, unsigned ch,
+                                           int& cell, unsigned& c, double& Es)
 {
     const double x = scaled_energy(energy_scale, Er);       // a3b: one rounded fp64 multiply
     const int bin = find_bin(bt, x);                        // a3c: bit-exact index
-    const bool ok = in && energy_ok(Et) && (unsigned)ch < (unsigned)kChannels && bin >= 0;
-    c = ok ? ch : 0;
+    const bool ok = energy_ok(Et) && ch < (unsigned)kChannels && bin >= 0;
+    c = ok ? ch : 0u;
     Es = ok ? Et : 1.0;
-    cell = ok ? c * bt.nb + bin : -1;
+    cell = ok ? (int)c * bt.nb + bin : -1;
 }
 
-// Two events of one thread as they come from global memory (VEC: events 2i, 2i+1 by 128-bit loads).
+// Two events of one thread as they come from global memory (VEC: events 2i, 2i+1 by 128-bit loads).  The two channel
+// bytes stay packed (low byte: first event) until they are used, so that nothing waits on the load where it is issued.
 struct EventPair {
     double Et0, Et1, Er0, Er1, wp0, wp1;
-    int ch0, ch1;
+    unsigned chp;
 };
 
 template <bool VEC, int THREADS>
 __device__ __forceinline__ EventPair load_pair(const double* __restrict__ E_true, const double* __restrict__ E_reco,
                                                const double* __restrict__ w0, const int8_t* __restrict__ channel,
-                                               size_t n, size_t tile, size_t& j0, size_t& j1)
+                                               size_t n, size_t tile)
 {
     const size_t base = tile * (2 * THREADS);
-    j0 = VEC ? base + 2 * threadIdx.x : base + threadIdx.x;
-    j1 = VEC ? j0 + 1 : j0 + THREADS;
+    const size_t j0 = VEC ? base + 2 * threadIdx.x : base + threadIdx.x;
+    const size_t j1 = VEC ? j0 + 1 : j0 + THREADS;
     const bool in0 = j0 < n, in1 = j1 < n;
     EventPair e;
     if (VEC && in1) {
         const double2 vt = ld_stream2(E_true + j0), vr = ld_stream2(E_reco + j0), vw = ld_stream2(w0 + j0);
-        const unsigned short vc = __ldcs(reinterpret_cast<const unsigned short*>(channel + j0));
+        e.chp = __ldcs(reinterpret_cast<const unsigned short*>(channel + j0));
         e.Et0 = vt.x; e.Et1 = vt.y;
         e.Er0 = vr.x; e.Er1 = vr.y;
         e.wp0 = vw.x; e.wp1 = vw.y;
-        e.ch0 = (int)(signed char)(vc & 0xffu);
-        e.ch1 = (int)(signed char)(vc >> 8);
     } else {
         e.Et0 = in0 ? ld_stream(E_true + j0) : 1.0;
         e.Et1 = in1 ? ld_stream(E_true + j1) : 1.0;
@@ -225,8 +226,9 @@ __device__ __forceinline__ EventPair load_pair(const double* __restrict__ E_true
         e.Er1 = in1 ? ld_stream(E_reco + j1) : 0.0;
         e.wp0 = in0 ? ld_stream(w0 + j0) : 0.0;
         e.wp1 = in1 ? ld_stream(w0 + j1) : 0.0;
-        e.ch0 = in0 ? (int)channel[j0] : -1;
-        e.ch1 = in1 ? (int)channel[j1] : -1;
+        const unsigned c0 = in0 ? (unsigned)(unsigned char)channel[j0] : 0xFFu;
+        const unsigned c1 = in1 ? (unsigned)(unsigned char)channel[j1] : 0xFFu;
+        e.chp = c0 | (c1 << 8);
     }
     return e;
 }
@@ -238,8 +240,11 @@ __device__ __forceinline__ EventPair load_pair(const double* __restrict__ E_true
 // of the current one (the kernel is bound by instruction issue around the fp64 pipe, so a warp that sits on a
 // global load is an issue slot lost), and the histogram ranking (MATCH + first read) precedes the closed form.
 // ------------------------------------------------------------------------------------------------
+#ifndef OSC_K2_TPS
+#define OSC_K2_TPS 768
+#endif
 template <bool VEC, int THREADS>
-__global__ void __launch_bounds__(THREADS, 768 / THREADS)
+__global__ void __launch_bounds__(THREADS, OSC_K2_TPS / THREADS)
 reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict__ E_true,
                     const double* __restrict__ E_reco, const double* __restrict__ w0,
                     const int8_t* __restrict__ channel, size_t n, double energy_scale,
@@ -260,8 +265,8 @@ reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict_
     const int n_hist = WARPS * kSlots * n_sub;
 
     const size_t ntiles = (n + 2 * THREADS - 1) / (2 * THREADS);
-    size_t t = blockIdx.x, j0 = 0, j1 = 0;
-    EventPair cur = load_pair<VEC, THREADS>(E_true, E_reco, w0, channel, n, t, j0, j1);   // grid <= ntiles
+    size_t t = blockIdx.x;
+    EventPair cur = load_pair<VEC, THREADS>(E_true, E_reco, w0, channel, n, t);   // grid <= ntiles
 
     if (threadIdx.x < kBinArgsDoubles) pbuf[threadIdx.x] = reinterpret_cast<const double*>(&a)[threadIdx.x];
     for (int i = threadIdx.x; i < n_hist * nh; i += THREADS) hist[i] = 0.0;
@@ -271,20 +276,26 @@ reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict_
     const LaneHist lh = lane_hist(hist, nh, n_sub, warp, lane);
 
     while (t < ntiles) {
-        const bool in0 = j0 < n, in1 = j1 < n;
-        int cell0, cell1, c0, c1;
+        int cell0, cell1;
+        unsigned c0, c1;
         double Es0, Es1;
-        locate_one(bt, energy_scale, in0, cur.Et0, cur.Er0, cur.ch0, cell0, c0, Es0);
-        locate_one(bt, energy_scale, in1, cur.Et1, cur.Er1, cur.ch1, cell1, c1, Es1);
-        const HistPlan plan = warp_hist_plan(lh, cell0, cell1, lt_mask);
+        locate_one(bt, energy_scale, cur.Et0, cur.Er0, cur.chp & 0xFFu, cell0, c0, Es0);
+        locate_one(bt, energy_scale, cur.Et1, cur.Er1, cur.chp >> 8, cell1, c1, Es1);
+        HistPlan plan;
+        warp_hist_match(plan, lh, cell0, cell1);
         const double wp0 = cur.wp0, wp1 = cur.wp1;
         // prefetch: E_true, E_reco and channel of the current pair are dead from here on
         t += gridDim.x;
-        if (t < ntiles) cur = load_pair<VEC, THREADS>(E_true, E_reco, w0, channel, n, t, j0, j1);
-        const OscTrans tr0 = load_trans(pb, c0);
-        const OscTrans tr1 = load_trans(pb, c1);
-        const double P0 = prob_one(a.set, tr0, Es0);        // a2a-a2f
-        const double P1 = prob_one(a.set, tr1, Es1);
+        if (t < ntiles) cur = load_pair<VEC, THREADS>(E_true, E_reco, w0, channel, n, t);
+        const OscTrans tr0 = load_trans(pb, (int)c0);
+        const OscTrans tr1 = load_trans(pb, (int)c1);
+        const double A0 = tr0.sa * Es0, A1 = tr1.sa * Es1;  // a2a
+        OscEig e0, e1;
+        eig_solve(a.set, A0, rcp_pos(Es0), e0);             // a2b-a2d
+        eig_solve(a.set, A1, rcp_pos(Es1), e1);
+        warp_hist_rank(plan, lt_mask);
+        const double P0 = assemble(e0, A0, tr0);            // a2e-a2f
+        const double P1 = assemble(e1, A1, tr1);
         warp_hist_commit(plan, __dmul_rn(wp0, P0), __dmul_rn(wp1, P1));   // a3a, a3c
     }
     block_merge(hist, n_hist, nh, ms, hist_out, &s_ticket);

@@ -212,6 +212,7 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     const size_t max_per_sm = threads == 256 ? 3 : 6;   // __launch_bounds__(THREADS, 768 / THREADS) of k2
     if (per_sm > max_per_sm && !getenv("OSC_TUNE_BPS")) per_sm = max_per_sm;
     const size_t ntiles = (n + 2 * threads - 1) / (2 * (size_t)threads);
+    if (ntiles > 0xFFFFFFFFull) return fail(OSC_ERR_INVALID_ARG, "n = %zu events is more than one call takes (2^32 tiles)", n);
     size_t g = (size_t)sms * per_sm;
     if (ntiles < g) g = ntiles;
     const int grid = (int)g;

@@ -96,8 +96,10 @@ __device__ __forceinline__ BinView bin_view(const unsigned char* smem_table)
     return v;
 }
 
-// The unique i with edges[i] <= x < edges[i+1], or -1.  t.steps is the same for all threads of the block, so the
-// branches on it are uniform; a sane binning needs one step.
+// The unique i with edges[i] <= x < edges[i+1], or -1.  STEPS = 1: the caller has checked that t.steps <= 1 (one
+// forward step finishes the search in every cell -- any sane binning); STEPS = 0: two branch-free steps and, if the
+// table says that this is not enough, a loop.
+template <int STEPS>
 __device__ __forceinline__ int find_bin(const BinView& t, double x)
 {
     const long long kx = order_key(x);
@@ -105,10 +107,12 @@ __device__ __forceinline__ int find_bin(const BinView& t, double x)
     const unsigned int rel = (unsigned int)max(khi, t.base) - (unsigned int)t.base;
     const unsigned int cell = min(rel >> t.shift, (unsigned int)(kLutCells - 1));
     int lo = (int)lds_u16(t.lut + 2u * cell);
-    if (t.steps >= 1u) lo += ((long long)lds_u64(t.ekey + 8u * (unsigned)(lo + 1)) <= kx) ? 1 : 0;   // sentinels keep these
-    if (t.steps >= 2u) lo += ((long long)lds_u64(t.ekey + 8u * (unsigned)(lo + 1)) <= kx) ? 1 : 0;   // reads inside the table
-    if (t.steps > 2u) {
-        while (lo < t.nb && (long long)lds_u64(t.ekey + 8u * (unsigned)(lo + 1)) <= kx) ++lo;
+    lo += ((long long)lds_u64(t.ekey + 8u * (unsigned)(lo + 1)) <= kx) ? 1 : 0;       // sentinels keep these reads
+    if (STEPS != 1) {                                                                 // inside the table
+        lo += ((long long)lds_u64(t.ekey + 8u * (unsigned)(lo + 1)) <= kx) ? 1 : 0;
+        if (t.steps > 2u) {
+            while (lo < t.nb && (long long)lds_u64(t.ekey + 8u * (unsigned)(lo + 1)) <= kx) ++lo;
+        }
     }
     return (lo < t.nb && t.key0 <= kx) ? lo : -1;
 }

@@ -142,7 +142,7 @@ bin_index_kernel(const double* __restrict__ E_true, const double* __restrict__ E
         const double x = scaled_energy(energy_scale, E_reco[j]);
         const int ch = channel[j];
         const bool ok = energy_ok(E_true[j]) && (unsigned)ch < (unsigned)kChannels;
-        const int b = find_bin(bt, x);
+        const int b = find_bin<0>(bt, x);
         bin_out[j] = ok ? b : -1;
     }
 }
@@ -185,11 +185,12 @@ __device__ __forceinline__ OscSet load_set(const double* pb)
 // event is dropped, A8/A11), the channel whose transition block is to be used and the energy handed to the closed form.
 // ch is the channel byte zero-extended: 0..3 are valid, every other code (negative int8 values, the 0xFF that
 // load_pair puts in for events past the end) is not.
+template <int STEPS>
 __device__ __forceinline__ void locate_one(const BinView& bt, double energy_scale, double Et, double Er, unsigned ch,
                                            int& cell, unsigned& c, double& Es)
 {
     const double x = scaled_energy(energy_scale, Er);       // a3b: one rounded fp64 multiply
-    const int bin = find_bin(bt, x);                        // a3c: bit-exact index
+    const int bin = find_bin<STEPS>(bt, x);                 // a3c: bit-exact index
     const bool ok = energy_ok(Et) && ch < (unsigned)kChannels && bin >= 0;
     c = ok ? ch : 0u;
     Es = ok ? Et : 1.0;
@@ -206,9 +207,9 @@ struct EventPair {
 template <bool VEC, int THREADS>
 __device__ __forceinline__ EventPair load_pair(const double* __restrict__ E_true, const double* __restrict__ E_reco,
                                                const double* __restrict__ w0, const int8_t* __restrict__ channel,
-                                               size_t n, size_t tile)
+                                               size_t n, unsigned tile)
 {
-    const size_t base = tile * (2 * THREADS);
+    const size_t base = (size_t)tile * (2 * THREADS);
     const size_t j0 = VEC ? base + 2 * threadIdx.x : base + threadIdx.x;
     const size_t j1 = VEC ? j0 + 1 : j0 + THREADS;
     const bool in0 = j0 < n, in1 = j1 < n;
@@ -231,6 +232,39 @@ __device__ __forceinline__ EventPair load_pair(const double* __restrict__ E_true
         e.chp = c0 | (c1 << 8);
     }
     return e;
+}
+
+// Event loop of k2 (STEPS as in find_bin): software-pipelined by hand, see the kernel's comment.
+template <bool VEC, int THREADS, int STEPS>
+__device__ __forceinline__ void k2_loop(const BinArgs& a, const double* __restrict__ E_true,
+                                        const double* __restrict__ E_reco, const double* __restrict__ w0,
+                                        const int8_t* __restrict__ channel, size_t n, double energy_scale,
+                                        const BinView& bt, uint32_t pb, const LaneHist& lh, unsigned lt_mask,
+                                        unsigned ntiles, unsigned t, EventPair cur)
+{
+    while (t < ntiles) {
+        int cell0, cell1;
+        unsigned c0, c1;
+        double Es0, Es1;
+        locate_one<STEPS>(bt, energy_scale, cur.Et0, cur.Er0, cur.chp & 0xFFu, cell0, c0, Es0);
+        locate_one<STEPS>(bt, energy_scale, cur.Et1, cur.Er1, cur.chp >> 8, cell1, c1, Es1);
+        HistPlan plan;
+        warp_hist_match(plan, lh, cell0, cell1);
+        const double wp0 = cur.wp0, wp1 = cur.wp1;
+        // prefetch: E_true, E_reco and channel of the current pair are dead from here on
+        t += gridDim.x;
+        if (t < ntiles) cur = load_pair<VEC, THREADS>(E_true, E_reco, w0, channel, n, t);
+        const OscTrans tr0 = load_trans(pb, (int)c0);
+        const OscTrans tr1 = load_trans(pb, (int)c1);
+        const double A0 = tr0.sa * Es0, A1 = tr1.sa * Es1;  // a2a
+        OscEig e0, e1;
+        eig_solve(a.set, A0, rcp_pos(Es0), e0);             // a2b-a2d
+        eig_solve(a.set, A1, rcp_pos(Es1), e1);
+        warp_hist_rank(plan, lt_mask);
+        const double P0 = assemble(e0, A0, tr0);            // a2e-a2f
+        const double P1 = assemble(e1, A1, tr1);
+        warp_hist_commit(plan, __dmul_rn(wp0, P0), __dmul_rn(wp1, P1));   // a3a, a3c
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -261,43 +295,29 @@ reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict_
 
     const unsigned lane = threadIdx.x & 31u;
     const unsigned warp = threadIdx.x >> 5;
-    const unsigned lt_mask = (1u << lane) - 1u;
     const int n_hist = WARPS * kSlots * n_sub;
 
-    const size_t ntiles = (n + 2 * THREADS - 1) / (2 * THREADS);
-    size_t t = blockIdx.x;
+    // tiles are counted in 32 bits (the host rejects n >= 2^32 tiles); pinned so that the loop does not recompute it
+    const unsigned ntiles = pin_u32((unsigned)((n + 2 * THREADS - 1) / (2 * THREADS)));
+    const unsigned t = blockIdx.x;
     EventPair cur = load_pair<VEC, THREADS>(E_true, E_reco, w0, channel, n, t);   // grid <= ntiles
 
     if (threadIdx.x < kBinArgsDoubles) pbuf[threadIdx.x] = reinterpret_cast<const double*>(&a)[threadIdx.x];
     for (int i = threadIdx.x; i < n_hist * nh; i += THREADS) hist[i] = 0.0;
     build_bin_table(tab, edges, nb);
-    const BinView bt = bin_view(tab);
-    const uint32_t pb = smem_u32(pbuf);
-    const LaneHist lh = lane_hist(hist, nh, n_sub, warp, lane);
+    BinView bt = bin_view(tab);
+    bt.ekey = pin_u32(bt.ekey);
+    bt.lut = pin_u32(bt.lut);
+    const uint32_t pb = pin_u32(smem_u32(pbuf));
+    LaneHist lh = lane_hist(hist, nh, n_sub, warp, lane);
+    lh.h0 = pin_u32(lh.h0);
+    lh.h1 = pin_u32(lh.h1);
+    const unsigned lt_mask = pin_u32((1u << lane) - 1u);
 
-    while (t < ntiles) {
-        int cell0, cell1;
-        unsigned c0, c1;
-        double Es0, Es1;
-        locate_one(bt, energy_scale, cur.Et0, cur.Er0, cur.chp & 0xFFu, cell0, c0, Es0);
-        locate_one(bt, energy_scale, cur.Et1, cur.Er1, cur.chp >> 8, cell1, c1, Es1);
-        HistPlan plan;
-        warp_hist_match(plan, lh, cell0, cell1);
-        const double wp0 = cur.wp0, wp1 = cur.wp1;
-        // prefetch: E_true, E_reco and channel of the current pair are dead from here on
-        t += gridDim.x;
-        if (t < ntiles) cur = load_pair<VEC, THREADS>(E_true, E_reco, w0, channel, n, t);
-        const OscTrans tr0 = load_trans(pb, (int)c0);
-        const OscTrans tr1 = load_trans(pb, (int)c1);
-        const double A0 = tr0.sa * Es0, A1 = tr1.sa * Es1;  // a2a
-        OscEig e0, e1;
-        eig_solve(a.set, A0, rcp_pos(Es0), e0);             // a2b-a2d
-        eig_solve(a.set, A1, rcp_pos(Es1), e1);
-        warp_hist_rank(plan, lt_mask);
-        const double P0 = assemble(e0, A0, tr0);            // a2e-a2f
-        const double P1 = assemble(e1, A1, tr1);
-        warp_hist_commit(plan, __dmul_rn(wp0, P0), __dmul_rn(wp1, P1));   // a3a, a3c
-    }
+    if (bt.steps <= 1u)
+        k2_loop<VEC, THREADS, 1>(a, E_true, E_reco, w0, channel, n, energy_scale, bt, pb, lh, lt_mask, ntiles, t, cur);
+    else
+        k2_loop<VEC, THREADS, 0>(a, E_true, E_reco, w0, channel, n, energy_scale, bt, pb, lh, lt_mask, ntiles, t, cur);
     block_merge(hist, n_hist, nh, ms, hist_out, &s_ticket);
 }
 
@@ -368,7 +388,7 @@ reweight_batch_kernel(const double* __restrict__ points, int npts, const double*
                 const double e = ld_stream(E_true + g);
                 const double x = scaled_energy(energy_scale, ld_stream(E_reco + g));
                 const int ch = channel[g];
-                const int bin = find_bin(bt, x);
+                const int bin = find_bin<0>(bt, x);
                 if (energy_ok(e) && (unsigned)ch < (unsigned)kChannels && bin >= 0) {
                     Et = e;
                     wv = ld_stream(w0 + g);

@@ -11,6 +11,16 @@
 
 namespace oscb {
 
+// A loop-invariant 32-bit value the compiler must keep in a register: without this it prefers to recompute shared-window
+// addresses, lane masks and table offsets inside the event loop (a dozen integer instructions per iteration that all
+// compete with the fp64 instructions for issue slots and register-file reads).
+__device__ __forceinline__ uint32_t pin_u32(uint32_t v)
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %1;" : "=r"(r) : "r"(v));
+    return r;
+}
+
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ unsigned long long lds_u64(uint32_t a)

@@ -377,18 +377,22 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
     int sms = 0;
     if ((rc = sm_count(&sms))) return rc;
 
-    // geometry: 1 block per SM (shared-memory bound); blocks = nchunks x ngroups ~ 4 waves
-    const size_t hist1 = sizeof(double) * (kBatchThreads / 32) * kSlots * nh;
+    // geometry: 1 block of 512 threads per SM (shared-memory bound; two blocks of 256 measured 2 % slower on
+    // configs[3]); blocks = nchunks x ngroups ~ 4 waves
+    const int threads = 512;
+    const size_t budget = kSmemBudget;
+    const size_t hist1 = sizeof(double) * (threads / 32) * kSlots * nh;
     const int n_sub = (2 * hist1 <= 64 * 1024) ? 2 : 1;
     const size_t fixed = sizeof(double) * kBinArgsDoubles + bin_table_bytes(n_bins) + n_sub * hist1;
-    if (fixed + 18 * 2 * kBatchThreads > kSmemBudget)
+    if (fixed + (size_t)kBatchBytesPerEvent * 2 * threads > budget)
         return fail(OSC_ERR_INVALID_ARG, "osc_reweight_bin_batch: n_bins = %d needs more shared memory than one SM has "
                                          "(limit for the batched call: about 380 bins)", n_bins);
-    const int tile_quant = 2 * kBatchThreads;
-    int te = (int)((kSmemBudget - fixed) / 18 / tile_quant * tile_quant);
+    const int blocks_per_sm = 512 / threads;
+    const int tile_quant = 2 * threads;
+    int te = (int)((budget - fixed) / kBatchBytesPerEvent / tile_quant * tile_quant);
     if (te > 8192) te = 8192;
     BatchGeom geo;
-    const int target_blocks = 4 * sms;
+    const int target_blocks = 4 * sms * blocks_per_sm;
     int ngroups = n_points < 16 ? n_points : 16;
     size_t max_chunks = (n + tile_quant - 1) / tile_quant;          // at least one thread-pair row per chunk
     size_t nchunks = (size_t)(target_blocks + ngroups - 1) / ngroups;
@@ -405,7 +409,7 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
     ngroups = (n_points + geo.pts_per_group - 1) / geo.pts_per_group;
     if ((size_t)te > round_up(geo.chunk_events, tile_quant)) te = (int)round_up(geo.chunk_events, tile_quant);
     geo.te = te;
-    const size_t smem = fixed + (size_t)18 * te;
+    const size_t smem = fixed + (size_t)kBatchBytesPerEvent * te;
 
     const size_t bytes_points = round_up((size_t)n_points * sizeof(BinArgs), 256);
     const size_t bytes_partial = (size_t)n_points * nchunks * nh * sizeof(double);
@@ -415,9 +419,10 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
     double* partial = reinterpret_cast<double*>(sc.p + bytes_points);
     // pageable source: the copy is staged before the call returns, so `blocks` may go out of scope
     CUDA_TRY(cudaMemcpyAsync(d_points, blocks.data(), (size_t)n_points * sizeof(BinArgs), cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaFuncSetAttribute(reweight_batch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    reweight_batch_kernel<<<dim3((unsigned)nchunks, (unsigned)ngroups), kBatchThreads, smem, st>>>(
-        d_points, n_points, E_true, E_reco, w0, channel, n, geo, energy_scale, bin_edges, n_bins, n_sub, partial);
+    const dim3 grid((unsigned)nchunks, (unsigned)ngroups);
+    CUDA_TRY(cudaFuncSetAttribute(reweight_batch_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    reweight_batch_kernel<512><<<grid, 512, smem, st>>>(d_points, n_points, E_true, E_reco, w0, channel, n, geo,
+                                                        energy_scale, bin_edges, n_bins, n_sub, partial);
     if ((rc = post_launch("osc_reweight_bin_batch"))) return rc;
     merge_chunks_kernel<<<n_points, 256, 0, st>>>(partial, (int)nchunks, (int)nh, hist_out);
     return post_launch("osc_reweight_bin_batch merge");

@@ -329,20 +329,24 @@ reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict_
 // fixed order and adds the result to its own slice partial[p][c][:] in global memory; merge_chunks_kernel
 // then sums the chunks of each point in chunk order.
 //
-// Shared memory: param block | bin table | hist[warps][kSlots][n_sub][4 nb] | Et[te] | w0[te] | cellch[te]
-// cellch = cell | channel << 12 (cell < 4 * 768 = 3072), 0xFFFF for a dropped or padding event.
+// Shared memory: param block | bin table | hist[warps][kSlots][n_sub][4 nb] | Et[te] | w0[te] | plan[te]
+// plan (32 bit) = cell | channel << 12 | rank << 16 (cell < 4 * 768 = 3072), 0xFFFFFFFF for a dropped or padding event.
+// The rank of an event among the lanes of its warp that hit the same histogram word (osc_hist.cuh) depends on the
+// cells only, not on the parameter set: MATCH runs once per staged tile, not once per point.
 // ------------------------------------------------------------------------------------------------
-constexpr int kBatchThreads = 512;
-constexpr unsigned short kDropped = 0xFFFFu;
+constexpr unsigned kDropped = 0xFFFFFFFFu;
+constexpr int kBatchBytesPerEvent = 20;   // E_true + w0 (fp64) + plan (u32)
 
 struct BatchGeom {
     size_t chunk_events;  // events per chunk (multiple of 2)
-    int te;               // tile capacity in events (multiple of 2 * kBatchThreads)
+    int te;               // tile capacity in events (multiple of 2 * THREADS)
     int nchunks;
     int pts_per_group;
 };
 
-__global__ void __launch_bounds__(kBatchThreads, 1)
+// Launched with 512 threads, one block per SM.
+template <int kBatchThreads>
+__global__ void __launch_bounds__(kBatchThreads, 512 / kBatchThreads)
 reweight_batch_kernel(const double* __restrict__ points, int npts, const double* __restrict__ E_true,
                       const double* __restrict__ E_reco, const double* __restrict__ w0,
                       const int8_t* __restrict__ channel, size_t n, BatchGeom geo, double energy_scale,
@@ -357,7 +361,7 @@ reweight_batch_kernel(const double* __restrict__ points, int npts, const double*
     double* hist = reinterpret_cast<double*>(tab + bin_table_bytes(nb));
     double* sEt = hist + (size_t)n_hist * nh;
     double* sW = sEt + geo.te;
-    unsigned short* sCell = reinterpret_cast<unsigned short*>(sW + geo.te);
+    unsigned* sPlan = reinterpret_cast<unsigned*>(sW + geo.te);
 
     const unsigned lane = threadIdx.x & 31u;
     const unsigned warp = threadIdx.x >> 5;
@@ -382,7 +386,7 @@ reweight_batch_kernel(const double* __restrict__ points, int npts, const double*
         const int m_pad = (m + 2 * kBatchThreads - 1) / (2 * kBatchThreads) * (2 * kBatchThreads);
         for (int j = threadIdx.x; j < m_pad; j += kBatchThreads) {
             double Et = 1.0, wv = 0.0;
-            unsigned short cc = kDropped;
+            unsigned cc = kDropped;
             if (j < m) {
                 const size_t g = tile + j;
                 const double e = ld_stream(E_true + g);
@@ -392,14 +396,24 @@ reweight_batch_kernel(const double* __restrict__ points, int npts, const double*
                 if (energy_ok(e) && (unsigned)ch < (unsigned)kChannels && bin >= 0) {
                     Et = e;
                     wv = ld_stream(w0 + g);
-                    cc = (unsigned short)((ch * nb + bin) | (ch << 12));
+                    cc = (unsigned)((ch * nb + bin) | (ch << 12));
                 }
             }
             sEt[j] = Et;
             sW[j] = wv;
-            sCell[j] = cc;
+            sPlan[j] = cc;
         }
         __syncthreads();
+        // ---- rank the events of every warp iteration once (same thread -> event map as the point loop) ----
+        for (int j = threadIdx.x; j < m_pad; j += 2 * kBatchThreads) {
+            const int j1 = j + kBatchThreads;
+            const unsigned cc0 = sPlan[j], cc1 = sPlan[j1];
+            HistPlan pl;
+            warp_hist_match(pl, lh, cc0 == kDropped ? -1 : (int)(cc0 & 0xFFFu), cc1 == kDropped ? -1 : (int)(cc1 & 0xFFFu));
+            if (cc0 != kDropped) sPlan[j] = cc0 | ((unsigned)__popc(pl.m0 & lt_mask) << 16);
+            if (cc1 != kDropped) sPlan[j1] = cc1 | ((unsigned)__popc(pl.m1 & lt_mask) << 16);
+        }
+        // (every thread re-reads only the words it wrote itself: no barrier needed before the point loop)
 
         // ---- all points of the group over the staged tile ----------------------------------------
         for (int p = p_begin; p < p_end; ++p) {
@@ -409,16 +423,23 @@ reweight_batch_kernel(const double* __restrict__ points, int npts, const double*
             const OscSet set = load_set(pbuf);
             for (int j = threadIdx.x; j < m_pad; j += 2 * kBatchThreads) {
                 const int j1 = j + kBatchThreads;
-                const unsigned cc0 = sCell[j], cc1 = sCell[j1];
+                const unsigned cc0 = sPlan[j], cc1 = sPlan[j1];
                 const double Et0 = sEt[j], Et1 = sEt[j1];
-                const double wv0 = sW[j], wv1 = sW[j1];
+                HistPlan pl;
+                pl.r0 = (int)cc0 >> 16;                                  // -1 for a dropped event
+                pl.r1 = (int)cc1 >> 16;
+                pl.a0 = lh.h0 + 8u * (cc0 & 0xFFFu);
+                pl.a1 = lh.h1 + 8u * (cc1 & 0xFFFu);
+                pl.rmax = __reduce_max_sync(0xffffffffu, max(pl.r0, pl.r1));
+                pl.v0 = 0.0;
+                pl.v1 = 0.0;
+                if (pl.r0 == 0) pl.v0 = lds_f64_volatile(pl.a0);
+                if (pl.r1 == 0) pl.v1 = lds_f64_volatile(pl.a1);
                 const OscTrans tr0 = load_trans(pb, (cc0 >> 12) & 3u);
                 const OscTrans tr1 = load_trans(pb, (cc1 >> 12) & 3u);
                 const double P0 = prob_one(set, tr0, Et0);
                 const double P1 = prob_one(set, tr1, Et1);
-                const int cell0 = cc0 == kDropped ? -1 : (int)(cc0 & 0xFFFu);
-                const int cell1 = cc1 == kDropped ? -1 : (int)(cc1 & 0xFFFu);
-                warp_hist_add2(lh, cell0, __dmul_rn(wv0, P0), cell1, __dmul_rn(wv1, P1), lt_mask);
+                warp_hist_commit(pl, __dmul_rn(sW[j], P0), __dmul_rn(sW[j1], P1));
             }
             __syncthreads();
             // sub-histograms summed in (warp, slot) order, cleared for the next point

@@ -7,7 +7,7 @@
 //   rcp_pos / rsqrt_pos : MUFU seed (upper 32 bits) + one third-order correction
 //   sincos_quarter_mul  : sin, cos of (pi/2) a b -- the product is rounded to the nearest integer
 //                         and subtracted inside fused multiply-adds (exact residual), then two
-//                         degree-6 polynomials in f^2 (coefficients: osc_coeffs.h) and a quadrant
+//                         polynomials in f^2 (degree 5 for the sine, 6 for the cosine) (coefficients: osc_coeffs.h) and a quadrant
 //                         fix-up on the integer pipe
 //   cos_third_acos      : largest root t of 8 t^3 - 6 t = U (U = 2 cos(3 phi) in [0, 2]) by an fp32
 //                         polynomial seed and two chord-Newton steps -- replaces acos + cos.
@@ -22,9 +22,9 @@
 
 namespace oscb {
 
-// [0..6] sin(pi/2 f)/f in z = f^2, [7..13] cos(pi/2 f) in z, [14] 1.5 * 2^52
-__constant__ double kPoly[15] = {
-    OSC_SINQ_0, OSC_SINQ_1, OSC_SINQ_2, OSC_SINQ_3, OSC_SINQ_4, OSC_SINQ_5, OSC_SINQ_6,
+// [0..5] sin(pi/2 f)/f in z = f^2, [6..12] cos(pi/2 f) in z, [13] 1.5 * 2^52
+__constant__ double kPoly[14] = {
+    OSC_SINQ_0, OSC_SINQ_1, OSC_SINQ_2, OSC_SINQ_3, OSC_SINQ_4, OSC_SINQ_5,
     OSC_COSQ_0, OSC_COSQ_1, OSC_COSQ_2, OSC_COSQ_3, OSC_COSQ_4, OSC_COSQ_5, OSC_COSQ_6,
     6755399441055744.0};
 
@@ -95,24 +95,23 @@ __device__ __forceinline__ double floor_hi_word(double v, int hi_floor)
 // sin and cos of (pi/2) * a * b for |a b| < 2^31.
 __device__ __forceinline__ void sincos_quarter_mul(double a, double b, double& s, double& c)
 {
-    const double MAGIC = kPoly[14];          // adding 1.5 * 2^52 rounds to the nearest integer
+    const double MAGIC = kPoly[13];          // adding 1.5 * 2^52 rounds to the nearest integer
     double kd = fma(a, b, MAGIC);
     const int k = __double2loint(kd);
     kd -= MAGIC;
     const double f = fma(a, b, -kd);         // exact product minus integer: |f| <= 1/2 (+ 1 ulp of a b)
     const double z = f * f;
-    double ps = fma(kPoly[6], z, kPoly[5]);
-    double pc = fma(kPoly[13], z, kPoly[12]);
-    ps = fma(ps, z, kPoly[4]);
-    pc = fma(pc, z, kPoly[11]);
-    ps = fma(ps, z, kPoly[3]);
+    double pc = fma(kPoly[12], z, kPoly[11]);
+    double ps = fma(kPoly[5], z, kPoly[4]);
     pc = fma(pc, z, kPoly[10]);
-    ps = fma(ps, z, kPoly[2]);
+    ps = fma(ps, z, kPoly[3]);
     pc = fma(pc, z, kPoly[9]);
-    ps = fma(ps, z, kPoly[1]);
+    ps = fma(ps, z, kPoly[2]);
     pc = fma(pc, z, kPoly[8]);
+    ps = fma(ps, z, kPoly[1]);
+    pc = fma(pc, z, kPoly[7]);
     ps = fma(ps, z, kPoly[0]);
-    pc = fma(pc, z, 1.0);
+    pc = fma(pc, z, kPoly[6]);
     ps = ps * f;
     // quadrant: k odd swaps; sin negative for k & 2; cos negative for (k + 1) & 2
     const bool odd = (k & 1) != 0;

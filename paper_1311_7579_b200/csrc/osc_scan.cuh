@@ -1,0 +1,378 @@
+// osc_scan.cuh -- k4: the batched call for parameter scans.
+//
+// The paper's scan floats theta23 and dm2_32; BASELINE.json configs[3] is a 32 x 32 grid of the
+// two with a delta_cp per point.  With U = R23 D R13 D^dagger R12, D = diag(1, 1, e^{i delta}) (PDG form,
+// DESIGN.md A6), D^dagger commutes with R12 and with diag(m^2), and A e e^dagger commutes with W = R23 D, so
+//
+//     T = W T' W^dagger,   T' = R13 R12 diag(m^2) R12^T R13^T + A e e^T   (real symmetric, no theta23, no delta)
+//     S = exp(-i T x) = W S' W^dagger,   S' = exp(-i T' x)                 (complex symmetric)
+//     S_{beta alpha} = sum_{ij} W_{beta i} conj(W_{alpha j}) S'_{ij}        (antineutrinos: W -> conj(W), A -> -A)
+//
+// All points that share (theta12, theta13, dm2_21, dm2_32, rho, L, hierarchy) -- a "group" -- share S', which is
+// where the eigen-solve and every transcendental sits; a point of the group costs a three-term complex
+// combination of S' entries.  The rows of W are (1,0,0), (0,c23,s23 e^{i delta}), (0,-s23,c23 e^{i delta}), so a
+// transition needs at most three distinct entries of S'.
+//
+// Work layout.  The histogram cell (channel, bin) of an event does not depend on the point either, so the events
+// are first sorted by cell (stable counting sort: scan_count / scan_offsets / scan_scatter).  A sorted cell is
+// cut into pieces of at most `piece` events; one warp takes a piece and, for every group, alternates
+//     phase A  lane = event : S' entries of 32 events into the warp's shared-memory slice
+//     phase B  lane = point : every lane walks the slice (broadcast reads) and adds w0 |sum_k c_k z_k|^2 to ONE
+//              REGISTER, because every event of the piece falls into the same histogram cell.
+// There is no histogram in shared memory, no atomic and no collision; partial[piece][point] is summed over the
+// pieces of a cell in order by scan_merge, so the result is a deterministic function of the inputs.
+#pragma once
+#include <cstdint>
+
+#include "osc_bins.cuh"
+#include "osc_core.cuh"
+#include "osc_types.h"
+
+namespace oscb {
+
+constexpr int kScanLanes = 32;        // points per sub-group (one per lane)
+constexpr int kScanElems = 3;         // entries of S' per channel, at most
+constexpr int kScanWarps = 4;         // warps per block of the event-ordered kernels
+constexpr unsigned short kNoCell = 0xFFFFu;
+
+// Entry (i, j) of T' and T'^2 as functions of the matter term A:  T'_ij = Tr0 + A ee,
+// (T'^2)_ij = T2r0 + A T2r1 + A^2 ee;  delta = [i == j], ee = [i == j == e].
+struct ScanElem {
+    double delta, ee, Tr0, T2r0, T2r1;
+};
+
+struct ScanChan {
+    double sa;                 // +-K_MATTER Y_E rho (sign: antineutrino channel)
+    int nk;                    // entries used (1..3)
+    int real_coef;             // 1 if every coefficient of every lane is real (imaginary parts exactly 0)
+    ScanElem el[kScanElems];
+};
+
+struct ScanGroup {
+    OscSet set;
+    double pad;
+    ScanChan ch[kChannels];
+};
+
+// Coefficients of one sub-group (at most 32 points of one group): coef[channel][k][re, im][lane].
+struct ScanSub {
+    int group;
+    int pt[kScanLanes];        // index of the lane's point in the caller's list, -1 for an unused lane
+    int pad[3];
+    double coef[kChannels][kScanElems][2][kScanLanes];
+};
+
+struct ScanGeom {
+    size_t range;              // events per warp range of the sort passes (multiple of 32)
+    unsigned nranges;
+    unsigned piece;            // events per piece (multiple of 32)
+    unsigned max_units;        // upper bound on the number of pieces (grid size of the main kernel)
+    int ncells;                // kChannels * nb
+    int nsubs;
+    int subs_per_slot;         // sub-groups one warp walks (blockIdx.y selects the slot)
+};
+
+} // namespace oscb
+
+namespace oscb {
+
+// ------------------------------------------------------------------------------------------------
+// Sort pass 1: histogram cell of every event (kNoCell: dropped, A8/A11) and, per warp range, the number of
+// events in every cell.  count is [ncells][nranges]; an exclusive scan over the flattened array is exactly
+// the destination of the first event of (cell, range) in a stable sort by cell.
+// Shared memory: bin table | wcnt[kScanWarps][ncells] (u32)
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(32 * kScanWarps)
+scan_count_kernel(const double* __restrict__ E_true, const double* __restrict__ E_reco,
+                  const int8_t* __restrict__ channel, size_t n, double energy_scale,
+                  const double* __restrict__ edges, int nb, ScanGeom geo, unsigned short* __restrict__ cellid,
+                  unsigned int* __restrict__ count)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    build_bin_table(smem_raw, edges, nb);
+    const BinView bt = bin_view(smem_raw);
+    const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    unsigned int* wcnt = reinterpret_cast<unsigned int*>(smem_raw + bin_table_bytes(nb)) + (size_t)warp * geo.ncells;
+    const unsigned r = blockIdx.x * kScanWarps + warp;
+    if (r >= geo.nranges) return;
+    for (int c = lane; c < geo.ncells; c += 32) wcnt[c] = 0u;
+    __syncwarp();
+    const size_t begin = (size_t)r * geo.range, end = min(n, begin + geo.range);
+    for (size_t j0 = begin; j0 < end; j0 += 32) {
+        const size_t j = j0 + lane;
+        unsigned cell = kNoCell;
+        if (j < end) {
+            const double x = scaled_energy(energy_scale, E_reco[j]);
+            const int bin = find_bin<0>(bt, x);
+            const unsigned ch = (unsigned)(unsigned char)channel[j];
+            if (energy_ok(E_true[j]) && ch < (unsigned)kChannels && bin >= 0) cell = ch * (unsigned)nb + (unsigned)bin;
+            cellid[j] = (unsigned short)cell;
+        }
+        const unsigned m = __match_any_sync(0xffffffffu, cell);
+        if (cell != kNoCell && lane == 31u - (unsigned)__clz((int)m)) wcnt[cell] += (unsigned)__popc(m);
+        __syncwarp();
+    }
+    for (int c = lane; c < geo.ncells; c += 32) count[(size_t)c * geo.nranges + r] = wcnt[c];
+}
+
+// Block-wide exclusive scan of one value per thread (1024 threads); returns the prefix, *total gets the sum.
+__device__ __forceinline__ unsigned block_exclusive_scan_1024(unsigned v, unsigned* s_warp, unsigned* total)
+{
+    const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    unsigned inc = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const unsigned o = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= (unsigned)d) inc += o;
+    }
+    __syncthreads();                       // s_warp may still be read from a previous call
+    if (lane == 31) s_warp[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        unsigned w = s_warp[lane], winc = w;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned o = __shfl_up_sync(0xffffffffu, winc, d);
+            if (lane >= (unsigned)d) winc += o;
+        }
+        s_warp[lane] = winc - w;           // exclusive prefix of the warp sums
+        if (lane == 31) s_warp[32] = winc;
+    }
+    __syncthreads();
+    *total = s_warp[32];
+    return s_warp[warp] + inc - v;
+}
+
+// Sort pass 2 (one block of 1024 threads): count -> exclusive offsets in place; cell_begin[c] = first sorted
+// position of cell c (cell_begin[ncells] = number of kept events); unit_begin[c] = index of the first piece of
+// cell c (unit_begin[ncells] = number of pieces).
+__global__ void __launch_bounds__(1024)
+scan_offsets_kernel(unsigned int* __restrict__ count, ScanGeom geo, unsigned int* __restrict__ cell_begin,
+                    unsigned int* __restrict__ unit_begin)
+{
+    __shared__ unsigned s_warp[33];
+    const size_t total_n = (size_t)geo.ncells * geo.nranges;
+    const size_t per = (total_n + 1023) / 1024;
+    const size_t b = (size_t)threadIdx.x * per, e = min(total_n, b + per);
+    unsigned sum = 0;
+    for (size_t i = b; i < e; ++i) sum += count[i];
+    unsigned total;
+    unsigned run = block_exclusive_scan_1024(sum, s_warp, &total);
+    for (size_t i = b; i < e; ++i) {
+        const unsigned v = count[i];
+        count[i] = run;
+        run += v;
+    }
+    __syncthreads();
+    for (int c = threadIdx.x; c <= geo.ncells; c += 1024)
+        cell_begin[c] = c < geo.ncells ? count[(size_t)c * geo.nranges] : total;
+    __syncthreads();
+    // pieces per cell: at most 3 cells per thread (ncells <= 4 * 768)
+    const int cper = (geo.ncells + 1023) / 1024;
+    const int c0 = threadIdx.x * cper, c1 = min(geo.ncells, c0 + cper);
+    unsigned np = 0;
+    for (int c = c0; c < c1; ++c) np += (cell_begin[c + 1] - cell_begin[c] + geo.piece - 1) / geo.piece;
+    unsigned utotal;
+    unsigned urun = block_exclusive_scan_1024(np, s_warp, &utotal);
+    for (int c = c0; c < c1; ++c) {
+        unit_begin[c] = urun;
+        urun += (cell_begin[c + 1] - cell_begin[c] + geo.piece - 1) / geo.piece;
+    }
+    if (threadIdx.x == 0) unit_begin[geo.ncells] = utotal;
+}
+
+// Sort pass 3: stable scatter of (E_true, w0) into cell order.  Same warp ranges as pass 1.
+// Shared memory: wcnt[kScanWarps][ncells] (u32)
+__global__ void __launch_bounds__(32 * kScanWarps)
+scan_scatter_kernel(const double* __restrict__ E_true, const double* __restrict__ w0,
+                    const unsigned short* __restrict__ cellid, size_t n, ScanGeom geo,
+                    const unsigned int* __restrict__ offsets, double* __restrict__ sEt, double* __restrict__ sW)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    unsigned int* wcnt = reinterpret_cast<unsigned int*>(smem_raw) + (size_t)warp * geo.ncells;
+    const unsigned r = blockIdx.x * kScanWarps + warp;
+    if (r >= geo.nranges) return;
+    for (int c = lane; c < geo.ncells; c += 32) wcnt[c] = 0u;
+    __syncwarp();
+    const size_t begin = (size_t)r * geo.range, end = min(n, begin + geo.range);
+    for (size_t j0 = begin; j0 < end; j0 += 32) {
+        const size_t j = j0 + lane;
+        const unsigned cell = j < end ? (unsigned)cellid[j] : (unsigned)kNoCell;
+        const unsigned m = __match_any_sync(0xffffffffu, cell);
+        unsigned before = 0;
+        if (cell != kNoCell) before = wcnt[cell];
+        __syncwarp();
+        if (cell != kNoCell) {
+            const size_t dst = (size_t)offsets[(size_t)cell * geo.nranges + r] + before + (unsigned)__popc(m & lt_mask);
+            sEt[dst] = E_true[j];
+            sW[dst] = w0[j];
+            if (lane == 31u - (unsigned)__clz((int)m)) wcnt[cell] = before + (unsigned)__popc(m);
+        }
+        __syncwarp();
+    }
+}
+
+} // namespace oscb
+
+namespace oscb {
+
+// Entry (i, j) of S' (common phase dropped, as in osc_core.cuh) for a real symmetric T': the imaginary parts of
+// T'_ij and (T'^2)_ij vanish, which removes a third of assemble()'s arithmetic.
+__device__ __forceinline__ void scan_amp(const OscEig& e, double A, const ScanElem& el, double& zr, double& zi)
+{
+    const double Tr = fma(A, el.ee, el.Tr0);
+    const double T2r = fma(A, fma(A, el.ee, el.T2r1), el.T2r0);
+    const double N0r = fma(e.prod12, el.delta, fma(-e.sum12, Tr, T2r));
+    const double N2r = fma(e.prod01, el.delta, fma(-e.sum01, Tr, T2r));
+    const double kn = e.kap2 * N2r;
+    zr = fma(el.delta, e.c1h, -(kn * e.s02));
+    zi = fma(el.delta, e.s1h, fma(kn, e.c02, -(e.kap0 * N0r)));
+}
+
+constexpr int kSliceEvents = 64;      // events per phase-A slice of a warp (two per lane)
+constexpr int kSliceDoubles = 8;      // z0r z0i z1r z1i z2r z2i w0 pad
+
+__device__ __forceinline__ ScanElem ldg_elem(const ScanElem* p)
+{
+    ScanElem e;
+    e.delta = __ldg(&p->delta);
+    e.ee = __ldg(&p->ee);
+    e.Tr0 = __ldg(&p->Tr0);
+    e.T2r0 = __ldg(&p->T2r0);
+    e.T2r1 = __ldg(&p->T2r1);
+    return e;
+}
+
+// Phase B: lane = point.  Every lane walks the `cnt` events of the slice (all lanes read the same words: one
+// shared-memory wavefront per 128-bit load) and accumulates w0 |sum_k c_k z_k|^2.
+template <int NK, bool REALC>
+__device__ __forceinline__ double scan_phase_b(uint32_t slice, int cnt, const double (&cr)[kScanElems],
+                                               const double (&ci)[kScanElems], double acc)
+{
+#pragma unroll 4
+    for (int j = 0; j < cnt; ++j) {
+        const uint32_t a = slice + (uint32_t)j * (8u * kSliceDoubles);
+        const double2 z0 = lds_f64x2(a), z1 = NK > 1 ? lds_f64x2(a + 16) : make_double2(0.0, 0.0);
+        const double2 z2 = NK > 2 ? lds_f64x2(a + 32) : make_double2(0.0, 0.0);
+        const double w = lds_f64(a + 48);
+        double ar = cr[0] * z0.x, ai = cr[0] * z0.y;
+        if (NK > 1) { ar = fma(cr[1], z1.x, ar); ai = fma(cr[1], z1.y, ai); }
+        if (NK > 2) { ar = fma(cr[2], z2.x, ar); ai = fma(cr[2], z2.y, ai); }
+        if (!REALC) {
+            ar = fma(-ci[0], z0.y, ar); ai = fma(ci[0], z0.x, ai);
+            if (NK > 1) { ar = fma(-ci[1], z1.y, ar); ai = fma(ci[1], z1.x, ai); }
+            if (NK > 2) { ar = fma(-ci[2], z2.y, ar); ai = fma(ci[2], z2.x, ai); }
+        }
+        const double P = fma(ar, ar, ai * ai);
+        acc = fma(w, P, acc);
+    }
+    return acc;
+}
+
+// ------------------------------------------------------------------------------------------------
+// k4 main kernel.  Warp (blockIdx.x * kScanWarps + warp) owns one piece of one sorted cell; blockIdx.y selects the
+// slot of sub-groups it walks.  partial[piece][point] is written once by exactly one lane.
+// Shared memory: slice[kScanWarps][kSliceEvents][kSliceDoubles]
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(32 * kScanWarps)
+scan_main_kernel(const ScanGroup* __restrict__ groups, const ScanSub* __restrict__ subs,
+                 const double* __restrict__ sEt, const double* __restrict__ sW,
+                 const unsigned int* __restrict__ cell_begin, const unsigned int* __restrict__ unit_begin, ScanGeom geo,
+                 int nb, int npoints, double* __restrict__ partial)
+{
+    __shared__ __align__(16) double s_slice[kScanWarps][kSliceEvents][kSliceDoubles];
+    const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const unsigned u = blockIdx.x * kScanWarps + warp;
+    if (u >= __ldg(unit_begin + geo.ncells)) return;
+    // cell of piece u: the largest c with unit_begin[c] <= u (uniform binary search; empty cells share a value
+    // with their successor and are skipped by taking the largest)
+    int lo = 0, hi = geo.ncells - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (__ldg(unit_begin + mid) <= u) lo = mid; else hi = mid - 1;
+    }
+    const int cell = lo;
+    const unsigned cb = __ldg(cell_begin + cell), ce = __ldg(cell_begin + cell + 1);
+    const unsigned begin = cb + (u - __ldg(unit_begin + cell)) * geo.piece;
+    const unsigned end = min(ce, begin + geo.piece);
+    const int ch = cell / nb;
+
+    double* my = &s_slice[warp][0][0];
+    const uint32_t slice = smem_u32(my);
+    const int s_begin = blockIdx.y * geo.subs_per_slot, s_end = min(geo.nsubs, s_begin + geo.subs_per_slot);
+    for (int s = s_begin; s < s_end; ++s) {
+        const ScanSub* sub = subs + s;
+        const ScanGroup* g = groups + __ldg(&sub->group);
+        OscSet set;
+        set.xq23 = __ldg(&g->set.xq23);
+        set.tr = __ldg(&g->set.tr);
+        set.dd = __ldg(&g->set.dd);
+        set.k1 = __ldg(&g->set.k1);
+        set.k0_27 = __ldg(&g->set.k0_27);
+        const ScanChan* gc = &g->ch[ch];
+        const double sa = __ldg(&gc->sa);
+        const int nk = __ldg(&gc->nk);
+        const bool realc = __ldg(&gc->real_coef) != 0;
+        const ScanElem el0 = ldg_elem(&gc->el[0]), el1 = ldg_elem(&gc->el[1]), el2 = ldg_elem(&gc->el[2]);
+        double cr[kScanElems], ci[kScanElems];
+#pragma unroll
+        for (int k = 0; k < kScanElems; ++k) {
+            cr[k] = __ldg(&sub->coef[ch][k][0][lane]);
+            ci[k] = __ldg(&sub->coef[ch][k][1][lane]);
+        }
+        const int pt = __ldg(&sub->pt[lane]);
+        double acc = 0.0;
+        for (unsigned s0 = begin; s0 < end; s0 += kSliceEvents) {
+            // ---- phase A: lane = event (two per lane), S' entries into the slice -------------------------
+            const unsigned e0 = s0 + lane, e1 = e0 + 32;
+            const double E0 = e0 < end ? __ldg(sEt + e0) : 1.0, E1 = e1 < end ? __ldg(sEt + e1) : 1.0;
+            const double w0v = e0 < end ? __ldg(sW + e0) : 0.0, w1v = e1 < end ? __ldg(sW + e1) : 0.0;
+            const double A0 = sa * E0, A1 = sa * E1;
+            OscEig g0, g1;
+            eig_solve(set, A0, rcp_pos(E0), g0);
+            eig_solve(set, A1, rcp_pos(E1), g1);
+            double* r0 = my + (size_t)lane * kSliceDoubles;
+            double* r1 = r0 + 32 * kSliceDoubles;
+            double zr, zi;
+            scan_amp(g0, A0, el0, zr, zi); r0[0] = zr; r0[1] = zi;
+            scan_amp(g1, A1, el0, zr, zi); r1[0] = zr; r1[1] = zi;
+            if (nk > 1) {
+                scan_amp(g0, A0, el1, zr, zi); r0[2] = zr; r0[3] = zi;
+                scan_amp(g1, A1, el1, zr, zi); r1[2] = zr; r1[3] = zi;
+            }
+            if (nk > 2) {
+                scan_amp(g0, A0, el2, zr, zi); r0[4] = zr; r0[5] = zi;
+                scan_amp(g1, A1, el2, zr, zi); r1[4] = zr; r1[5] = zi;
+            }
+            r0[6] = w0v;
+            r1[6] = w1v;
+            __syncwarp();
+            // ---- phase B: lane = point ------------------------------------------------------------------
+            const int cnt = (int)min((unsigned)kSliceEvents, end - s0);
+            if (nk == 3 && realc) acc = scan_phase_b<3, true>(slice, cnt, cr, ci, acc);
+            else if (nk == 3) acc = scan_phase_b<3, false>(slice, cnt, cr, ci, acc);
+            else if (nk == 2) acc = scan_phase_b<2, false>(slice, cnt, cr, ci, acc);
+            else acc = scan_phase_b<1, false>(slice, cnt, cr, ci, acc);
+            __syncwarp();
+        }
+        if (pt >= 0) partial[(size_t)u * npoints + pt] = acc;
+    }
+}
+
+// out[p][cell] = sum over the pieces of the cell, in order, of partial[piece][p]; 0 for an empty cell.
+__global__ void __launch_bounds__(256)
+scan_merge_kernel(const double* __restrict__ partial, const unsigned int* __restrict__ unit_begin, int ncells,
+                  int npoints, double* __restrict__ out)
+{
+    const int cell = blockIdx.x;
+    const unsigned u0 = unit_begin[cell], u1 = unit_begin[cell + 1];
+    for (int p = threadIdx.x; p < npoints; p += blockDim.x) {
+        double s = 0.0;
+        for (unsigned u = u0; u < u1; ++u) s += partial[(size_t)u * npoints + p];
+        out[(size_t)p * ncells + cell] = s;
+    }
+}
+
+} // namespace oscb

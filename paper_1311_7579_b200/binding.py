@@ -186,6 +186,12 @@ def osc_reweight_bin(E_true, E_reco, w0, channel, energy_scale: float, bin_edges
     return hist_out
 
 
+def pack_params(points: Sequence):
+    """The osc_params array of a list of parameter sets (marshalling only).  osc_reweight_bin_batch takes either
+    the list or this array; a caller that scans the same points repeatedly packs them once."""
+    return (osc_params * max(len(points), 1))(*[make_params(q) for q in points])
+
+
 def osc_reweight_bin_batch(points: Sequence, E_true, E_reco, w0, channel, energy_scale: float, bin_edges,
                            hist_out=None, stream=None):
     """[n_points, N_CHANNELS, n_bins] histograms, one slice per parameter set, in one call."""
@@ -194,7 +200,7 @@ def osc_reweight_bin_batch(points: Sequence, E_true, E_reco, w0, channel, energy
     n, pt, pr, pw, pc = _event_ptrs(E_true, E_reco, w0, channel)
     nb = bin_edges.numel() - 1
     npts = len(points)
-    arr = (osc_params * max(npts, 1))(*[make_params(q) for q in points])
+    arr = points if isinstance(points, ctypes.Array) else pack_params(points)
     if hist_out is None:
         hist_out = torch.empty((npts, N_CHANNELS, nb), dtype=torch.float64, device=E_true.device)
     if hist_out.numel() != npts * N_CHANNELS * nb:

@@ -350,6 +350,55 @@ int osc_reweight_bin(const double* E_true, const double* E_reco, const double* w
                            static_cast<cudaStream_t>(stream));
 }
 
+namespace {
+
+// Pinned staging for host-built tables that a batched call uploads: a small ring of page-locked buffers, each
+// fenced by an event recorded after the copy that reads it, so that the upload is a true asynchronous copy (a
+// pageable source makes cudaMemcpyAsync wait for the stream) and the call returns while earlier work still runs.
+struct PinnedRing {
+    static constexpr int kSlots = 4;
+    struct Slot {
+        void* host = nullptr;
+        size_t cap = 0;
+        cudaEvent_t ev = nullptr;
+        bool in_flight = false;
+    };
+    Slot slot[kSlots];
+    int next = 0;
+    std::mutex mu;
+
+    int acquire(size_t bytes, Slot** out)
+    {
+        std::lock_guard<std::mutex> lk(mu);
+        Slot& s = slot[next];
+        next = (next + 1) % kSlots;
+        if (s.in_flight) {
+            CUDA_TRY(cudaEventSynchronize(s.ev));
+            s.in_flight = false;
+        }
+        if (!s.ev) CUDA_TRY(cudaEventCreateWithFlags(&s.ev, cudaEventDisableTiming));
+        if (s.cap < bytes) {
+            if (s.host) CUDA_TRY(cudaFreeHost(s.host));
+            s.host = nullptr;
+            s.cap = 0;
+            const size_t cap = round_up(bytes + bytes / 2, 1 << 16);
+            CUDA_TRY(cudaMallocHost(&s.host, cap));
+            s.cap = cap;
+        }
+        *out = &s;
+        return OSC_OK;
+    }
+    int fence(Slot* s, cudaStream_t st)
+    {
+        CUDA_TRY(cudaEventRecord(s->ev, st));
+        s->in_flight = true;
+        return OSC_OK;
+    }
+};
+PinnedRing g_ring;
+
+} // namespace
+
 // ------------------------------------------------------------------------------------------------
 // k4 (osc_scan.cuh): host side of the factorised batched call.
 // ------------------------------------------------------------------------------------------------
@@ -516,9 +565,13 @@ int launch_batch_scan(const ScanPlan& plan, int n_points, const double* E_true, 
     ScanGroup* d_groups = reinterpret_cast<ScanGroup*>(q); q += b_groups;
     ScanSub* d_subs = reinterpret_cast<ScanSub*>(q); q += b_subs;
     double* partial = reinterpret_cast<double*>(q);
-    // pageable sources: both copies are staged before the calls return
-    CUDA_TRY(cudaMemcpyAsync(d_groups, plan.groups.data(), plan.groups.size() * sizeof(ScanGroup), cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaMemcpyAsync(d_subs, plan.subs.data(), plan.subs.size() * sizeof(ScanSub), cudaMemcpyHostToDevice, st));
+    // groups and sub-groups are contiguous on the device: one asynchronous copy from a pinned staging slot
+    PinnedRing::Slot* slot = nullptr;
+    if ((rc = g_ring.acquire(b_groups + b_subs, &slot))) return rc;
+    std::memcpy(slot->host, plan.groups.data(), plan.groups.size() * sizeof(ScanGroup));
+    std::memcpy(static_cast<char*>(slot->host) + b_groups, plan.subs.data(), plan.subs.size() * sizeof(ScanSub));
+    CUDA_TRY(cudaMemcpyAsync(d_groups, slot->host, b_groups + b_subs, cudaMemcpyHostToDevice, st));
+    if ((rc = g_ring.fence(slot, st))) return rc;
 
     const unsigned sort_blocks = (geo.nranges + kScanWarps - 1) / kScanWarps;
     const size_t smem_cnt = sizeof(unsigned int) * kScanWarps * (size_t)geo.ncells;
@@ -530,9 +583,12 @@ int launch_batch_scan(const ScanPlan& plan, int n_points, const double* E_true, 
     scan_count_kernel<<<sort_blocks, 32 * kScanWarps, smem_count, st>>>(E_true, E_reco, channel, n, energy_scale, bin_edges,
                                                                         n_bins, geo, cellid, count);
     if ((rc = post_launch("osc_reweight_bin_batch (sort: count)"))) return rc;
-    scan_offsets_kernel<<<1, 1024, 0, st>>>(count, geo, cell_begin, unit_begin);
+    scan_offsets_cell_kernel<<<geo.ncells, 1024, 0, st>>>(count, geo, cell_begin);
+    if ((rc = post_launch("osc_reweight_bin_batch (sort: offsets per cell)"))) return rc;
+    scan_offsets_kernel<<<1, 1024, 0, st>>>(geo, cell_begin, unit_begin);
     if ((rc = post_launch("osc_reweight_bin_batch (sort: offsets)"))) return rc;
-    scan_scatter_kernel<<<sort_blocks, 32 * kScanWarps, smem_cnt, st>>>(E_true, w0, cellid, n, geo, count, sEt, sW);
+    scan_scatter_kernel<<<sort_blocks, 32 * kScanWarps, smem_cnt, st>>>(E_true, w0, cellid, n, geo, count, cell_begin,
+                                                                        sEt, sW);
     if ((rc = post_launch("osc_reweight_bin_batch (sort: scatter)"))) return rc;
     const dim3 grid((geo.max_units + kScanWarps - 1) / kScanWarps, (unsigned)slots);
     scan_main_kernel<<<grid, 32 * kScanWarps, 0, st>>>(d_groups, d_subs, sEt, sW, cell_begin, unit_begin, geo, n_bins,
@@ -626,8 +682,12 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
     if ((rc = sc.alloc(bytes_points + bytes_partial, st))) return rc;
     double* d_points = reinterpret_cast<double*>(sc.p);
     double* partial = reinterpret_cast<double*>(sc.p + bytes_points);
-    // pageable source: the copy is staged before the call returns, so `blocks` may go out of scope
-    CUDA_TRY(cudaMemcpyAsync(d_points, blocks.data(), (size_t)n_points * sizeof(BinArgs), cudaMemcpyHostToDevice, st));
+    // asynchronous upload from a pinned staging slot (PinnedRing)
+    PinnedRing::Slot* slot = nullptr;
+    if ((rc = g_ring.acquire((size_t)n_points * sizeof(BinArgs), &slot))) return rc;
+    std::memcpy(slot->host, blocks.data(), (size_t)n_points * sizeof(BinArgs));
+    CUDA_TRY(cudaMemcpyAsync(d_points, slot->host, (size_t)n_points * sizeof(BinArgs), cudaMemcpyHostToDevice, st));
+    if ((rc = g_ring.fence(slot, st))) return rc;
     const dim3 grid((unsigned)nchunks, (unsigned)ngroups);
     CUDA_TRY(cudaFuncSetAttribute(reweight_batch_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     reweight_batch_kernel<512><<<grid, 512, smem, st>>>(d_points, n_points, E_true, E_reco, w0, channel, n, geo,

@@ -78,8 +78,8 @@ namespace oscb {
 
 // ------------------------------------------------------------------------------------------------
 // Sort pass 1: histogram cell of every event (kNoCell: dropped, A8/A11) and, per warp range, the number of
-// events in every cell.  count is [ncells][nranges]; an exclusive scan over the flattened array is exactly
-// the destination of the first event of (cell, range) in a stable sort by cell.
+// events in every cell.  count is [ncells][nranges]: first sorted position of cell c plus the exclusive prefix over
+// the ranges inside row c is the destination of the first event of (cell, range) in a stable sort by cell.
 // Shared memory: bin table | wcnt[kScanWarps][ncells] (u32)
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(32 * kScanWarps)
@@ -143,42 +143,54 @@ __device__ __forceinline__ unsigned block_exclusive_scan_1024(unsigned v, unsign
     return s_warp[warp] + inc - v;
 }
 
-// Sort pass 2 (one block of 1024 threads): count -> exclusive offsets in place; cell_begin[c] = first sorted
-// position of cell c (cell_begin[ncells] = number of kept events); unit_begin[c] = index of the first piece of
-// cell c (unit_begin[ncells] = number of pieces).
+// Sort pass 2a (one block of 1024 threads per cell): count[cell][:] -> exclusive prefix within the cell, in place;
+// cell_total[cell] = number of kept events of the cell.
 __global__ void __launch_bounds__(1024)
-scan_offsets_kernel(unsigned int* __restrict__ count, ScanGeom geo, unsigned int* __restrict__ cell_begin,
-                    unsigned int* __restrict__ unit_begin)
+scan_offsets_cell_kernel(unsigned int* __restrict__ count, ScanGeom geo, unsigned int* __restrict__ cell_total)
 {
     __shared__ unsigned s_warp[33];
-    const size_t total_n = (size_t)geo.ncells * geo.nranges;
-    const size_t per = (total_n + 1023) / 1024;
-    const size_t b = (size_t)threadIdx.x * per, e = min(total_n, b + per);
-    unsigned sum = 0;
-    for (size_t i = b; i < e; ++i) sum += count[i];
-    unsigned total;
-    unsigned run = block_exclusive_scan_1024(sum, s_warp, &total);
-    for (size_t i = b; i < e; ++i) {
-        const unsigned v = count[i];
-        count[i] = run;
-        run += v;
+    unsigned int* row = count + (size_t)blockIdx.x * geo.nranges;
+    unsigned carry = 0;
+    for (unsigned base = 0; base < geo.nranges; base += 1024) {
+        const unsigned i = base + threadIdx.x;
+        const unsigned v = i < geo.nranges ? row[i] : 0u;
+        unsigned total;
+        const unsigned ex = block_exclusive_scan_1024(v, s_warp, &total);
+        if (i < geo.nranges) row[i] = carry + ex;
+        carry += total;
     }
-    __syncthreads();
-    for (int c = threadIdx.x; c <= geo.ncells; c += 1024)
-        cell_begin[c] = c < geo.ncells ? count[(size_t)c * geo.nranges] : total;
-    __syncthreads();
-    // pieces per cell: at most 3 cells per thread (ncells <= 4 * 768)
+    if (threadIdx.x == 0) cell_total[blockIdx.x] = carry;
+}
+
+// Sort pass 2b (one block of 1024 threads): cell_begin[c] = first sorted position of cell c (cell_begin[ncells] =
+// number of kept events; on entry cell_begin[c] holds the cell's total); unit_begin[c] = index of the first piece of
+// cell c (unit_begin[ncells] = number of pieces).  At most 3 cells per thread (ncells <= 4 * 768).
+__global__ void __launch_bounds__(1024)
+scan_offsets_kernel(ScanGeom geo, unsigned int* __restrict__ cell_begin, unsigned int* __restrict__ unit_begin)
+{
+    __shared__ unsigned s_warp[33];
     const int cper = (geo.ncells + 1023) / 1024;
-    const int c0 = threadIdx.x * cper, c1 = min(geo.ncells, c0 + cper);
-    unsigned np = 0;
-    for (int c = c0; c < c1; ++c) np += (cell_begin[c + 1] - cell_begin[c] + geo.piece - 1) / geo.piece;
-    unsigned utotal;
+    const int c0 = min(geo.ncells, (int)threadIdx.x * cper), c1 = min(geo.ncells, c0 + cper);
+    unsigned len[3] = {0u, 0u, 0u};
+    unsigned sum = 0, np = 0;
+    for (int c = c0; c < c1; ++c) {
+        len[c - c0] = cell_begin[c];
+        sum += len[c - c0];
+        np += (len[c - c0] + geo.piece - 1) / geo.piece;
+    }
+    unsigned total, utotal;
+    unsigned run = block_exclusive_scan_1024(sum, s_warp, &total);
     unsigned urun = block_exclusive_scan_1024(np, s_warp, &utotal);
     for (int c = c0; c < c1; ++c) {
+        cell_begin[c] = run;
         unit_begin[c] = urun;
-        urun += (cell_begin[c + 1] - cell_begin[c] + geo.piece - 1) / geo.piece;
+        run += len[c - c0];
+        urun += (len[c - c0] + geo.piece - 1) / geo.piece;
     }
-    if (threadIdx.x == 0) unit_begin[geo.ncells] = utotal;
+    if (threadIdx.x == 0) {
+        cell_begin[geo.ncells] = total;
+        unit_begin[geo.ncells] = utotal;
+    }
 }
 
 // Sort pass 3: stable scatter of (E_true, w0) into cell order.  Same warp ranges as pass 1.
@@ -186,7 +198,8 @@ scan_offsets_kernel(unsigned int* __restrict__ count, ScanGeom geo, unsigned int
 __global__ void __launch_bounds__(32 * kScanWarps)
 scan_scatter_kernel(const double* __restrict__ E_true, const double* __restrict__ w0,
                     const unsigned short* __restrict__ cellid, size_t n, ScanGeom geo,
-                    const unsigned int* __restrict__ offsets, double* __restrict__ sEt, double* __restrict__ sW)
+                    const unsigned int* __restrict__ offsets, const unsigned int* __restrict__ cell_begin,
+                    double* __restrict__ sEt, double* __restrict__ sW)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -205,7 +218,8 @@ scan_scatter_kernel(const double* __restrict__ E_true, const double* __restrict_
         if (cell != kNoCell) before = wcnt[cell];
         __syncwarp();
         if (cell != kNoCell) {
-            const size_t dst = (size_t)offsets[(size_t)cell * geo.nranges + r] + before + (unsigned)__popc(m & lt_mask);
+            const size_t dst = (size_t)cell_begin[cell] + offsets[(size_t)cell * geo.nranges + r] + before +
+                               (unsigned)__popc(m & lt_mask);
             sEt[dst] = E_true[j];
             sW[dst] = w0[j];
             if (lane == 31u - (unsigned)__clz((int)m)) wcnt[cell] = before + (unsigned)__popc(m);

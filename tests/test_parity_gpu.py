@@ -383,6 +383,112 @@ def test_batch_point_count_edge_cases(osc):
 
 
 # ------------------------------------------------------------------------------------------------
+# k4, the factorised path of the batched call (points that differ only in theta23 / delta_cp share the
+# eigen-problem).  OSC_BATCH_PATH forces one path or the other (include/osc.h), so both are checked against the
+# oracle on the same inputs, and against each other.
+# ------------------------------------------------------------------------------------------------
+class batch_path:
+    def __init__(self, which):
+        self.which = which
+
+    def __enter__(self):
+        import os
+        self.old = os.environ.get("OSC_BATCH_PATH")
+        os.environ["OSC_BATCH_PATH"] = self.which
+
+    def __exit__(self, *a):
+        import os
+        if self.old is None:
+            del os.environ["OSC_BATCH_PATH"]
+        else:
+            os.environ["OSC_BATCH_PATH"] = self.old
+
+
+def ragged_group_points(seed=21):
+    """Three eigen-problems with 1, 33 and 36 points (the second and third spill into a second sub-group of lanes),
+    interleaved in the list; theta23 covers 0 and 1, delta_cp the whole circle."""
+    rng = np.random.default_rng(seed)
+    bases = [wl.table1(rho_g_cm3=0.0, L_km=1300.0, hierarchy=-1),
+             wl.table1(dm2_32=2.1e-3, rho_g_cm3=5.0),
+             wl.table1(sin2_th13=0.03, sin2_th12=0.28, L_km=810.0)]
+    sizes = [1, 33, 36]
+    pts = []
+    for g, (b, m) in enumerate(zip(bases, sizes)):
+        th = rng.uniform(0.0, 1.0, m)
+        th[0] = 0.0 if g == 1 else th[0]
+        th[-1] = 1.0 if g == 2 else th[-1]
+        for k in range(m):
+            pts.append(dict(b, sin2_th23=float(th[k]), delta_cp=float(rng.uniform(-math.pi, math.pi))))
+    order = rng.permutation(len(pts))
+    return [pts[i] for i in order]
+
+
+def test_k4_ragged_groups_vs_oracle(osc):
+    pts = ragged_group_points()
+    n = 3_000 + 7
+    et, er, w0, ch = wl.events(n, seed=22)
+    et[5] = -1.0; et[6] = float("nan"); ch[7] = 9; ch[8] = -3; er[9] = 77.0     # dropped events (A8, A11)
+    edges = wl.bin_edges()
+    d = [dev(a) for a in (et, er, w0, ch)]
+    ref = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 1.03, edges)
+    with batch_path("k4"):
+        got4 = host(osc.osc_reweight_bin_batch(pts, *d, 1.03, dev(edges)))
+    with batch_path("k3"):
+        got3 = host(osc.osc_reweight_bin_batch(pts, *d, 1.03, dev(edges)))
+    assert_hist_close(got4, ref, "k4 ragged groups")
+    assert_hist_close(got3, ref, "k3 ragged groups")
+    assert np.array_equal(got4 == 0.0, got3 == 0.0)
+
+
+def test_k4_equals_k3_on_the_grid_with_more_events(osc):
+    pts = wl.scan_points()[:96]          # three dm2_32 groups of 32 points
+    n = 200_000 + 33
+    et, er, w0, ch = wl.events(n, seed=23)
+    edges = wl.bin_edges()
+    d = [dev(a) for a in (et, er, w0, ch)]
+    de = dev(edges)
+    with batch_path("k4"):
+        a = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, de))
+        b = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, de))
+    with batch_path("k3"):
+        c = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, de))
+    assert np.array_equal(a, b), "k4 is not bit-reproducible"
+    assert_hist_close(a, c, "k4 vs k3")
+    # the oracle on a sample of points (full 200k events each)
+    pick = [0, 37, 95]
+    ref = oracle.reweight_bin_batch([oracle.Params(**pts[i]) for i in pick], et, er, w0, ch, 1.0, edges)
+    assert_hist_close(a[pick], ref, "k4 vs oracle")
+
+
+@pytest.mark.parametrize("n", [0, 1, 31, 64, 65, 129, 1000])
+@pytest.mark.parametrize("nb,kind", [(1, "uniform"), (7, "random"), (50, "uniform")])
+def test_k4_small_and_ragged_sizes(osc, n, nb, kind):
+    rng = np.random.default_rng(100 + n + nb)
+    if kind == "uniform":
+        edges = wl.bin_edges(nb, 5.0)
+    else:
+        edges = np.sort(rng.uniform(0.05, 6.0, nb + 1))
+    pts = [wl.table1(sin2_th23=0.3 + 0.05 * k, delta_cp=-3.0 + 0.7 * k) for k in range(9)]
+    et, er, w0, ch = wl.events(max(n, 1), seed=24)
+    et, er, w0, ch = et[:n], er[:n], w0[:n], ch[:n]
+    with batch_path("k4"):
+        got = host(osc.osc_reweight_bin_batch(pts, dev(et), dev(er), dev(w0), dev(ch), 0.97, dev(edges)))
+    ref = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 0.97, edges)
+    assert got.shape == (9, 4, nb)
+    assert_hist_close(got, ref, f"k4 n={n} nb={nb}")
+
+
+def test_k4_all_events_dropped(osc):
+    n = 500
+    et, er, w0, ch = wl.events(n, seed=25)
+    er[:] = 99.0
+    pts = [wl.table1(sin2_th23=0.4), wl.table1(sin2_th23=0.6)]
+    with batch_path("k4"):
+        got = host(osc.osc_reweight_bin_batch(pts, dev(et), dev(er), dev(w0), dev(ch), 1.0, dev(wl.bin_edges())))
+    assert got.shape == (2, 4, 50) and float(np.abs(got).sum()) == 0.0
+
+
+# ------------------------------------------------------------------------------------------------
 # asynchrony: parameters are captured at enqueue time; work runs on the caller's stream
 # ------------------------------------------------------------------------------------------------
 def test_params_captured_at_enqueue_on_side_stream(osc):

@@ -483,7 +483,7 @@ void build_scan_plan(const osc_params* points, int n_points, ScanPlan& plan)
                 }
             ScanChan& sc = sg.ch[c];
             sc.nk = nk;
-            sc.real_coef = 1;
+            sc.tmask = 0;
             for (int k = 0; k < nk; ++k) {
                 const OscTrans t = make_trans(h, el_j[c][k], el_i[c][k], anti);   // entry (i, j): alpha = j, beta = i
                 sc.sa = t.sa;
@@ -494,8 +494,38 @@ void build_scan_plan(const osc_params* points, int n_points, ScanPlan& plan)
                 sc.el[k].T2r1 = t.T2r1;
             }
         }
-        // sub-groups of at most 32 points: coefficients C_ij = W_{beta i} conj(W_{alpha j}) (+ C_ji for i != j)
+        // coefficients c_k = C_ij = W_{beta i} conj(W_{alpha j}) (+ C_ji for i != j) of every point, and from them the
+        // monomials of |sum_k c_k z_k|^2 in the canonical term order of osc_scan.cuh
         const std::vector<int>& mem = members[g];
+        std::vector<std::array<double, kChannels * kScanTerms>> mono(mem.size());
+        for (size_t q = 0; q < mem.size(); ++q) {
+            const osc_params& pp = points[mem[q]];
+            const double s23 = std::sqrt(pp.sin2_th23), c23 = std::sqrt(1.0 - pp.sin2_th23);
+            for (int c = 0; c < kChannels; ++c) {
+                int fin, fout, anti;
+                channel_def(c, fin, fout, anti);
+                const double d = anti ? -pp.delta_cp : pp.delta_cp;          // antineutrinos: W -> conj(W)
+                const cd ep(std::cos(d), std::sin(d));
+                const cd W[3][3] = {{cd(1.0), cd(0.0), cd(0.0)}, {cd(0.0), cd(c23), s23 * ep}, {cd(0.0), cd(-s23), c23 * ep}};
+                cd ck[kScanElems] = {cd(0.0), cd(0.0), cd(0.0)};
+                for (int k = 0; k < sg.ch[c].nk; ++k) {
+                    const int i = el_i[c][k], j = el_j[c][k];
+                    ck[k] = W[fout][i] * std::conj(W[fin][j]);
+                    if (i != j) ck[k] += W[fout][j] * std::conj(W[fin][i]);
+                }
+                double* mo = &mono[q][(size_t)c * kScanTerms];
+                static const int PK[3] = {0, 0, 1}, PL[3] = {1, 2, 2};
+                for (int k = 0; k < 3; ++k) mo[k] = std::norm(ck[k]);
+                for (int r = 0; r < 3; ++r) {
+                    const cd x = ck[PK[r]] * std::conj(ck[PL[r]]);
+                    mo[3 + r] = 2.0 * x.real();
+                    mo[6 + r] = -2.0 * x.imag();
+                }
+                for (int t = 0; t < kScanTerms; ++t)
+                    if (mo[t] != 0.0) sg.ch[c].tmask |= 1 << t;
+            }
+        }
+        // sub-groups of at most 32 points; the used terms of a channel are stored compacted, in canonical order
         for (size_t first = 0; first < mem.size(); first += kScanLanes) {
             plan.subs.emplace_back();
             ScanSub& sub = plan.subs.back();
@@ -503,23 +533,11 @@ void build_scan_plan(const osc_params* points, int n_points, ScanPlan& plan)
             sub.group = (int)g;
             for (int l = 0; l < kScanLanes; ++l) sub.pt[l] = -1;
             for (int l = 0; l < kScanLanes && first + l < mem.size(); ++l) {
-                const osc_params& pp = points[mem[first + l]];
                 sub.pt[l] = mem[first + l];
-                const double s23 = std::sqrt(pp.sin2_th23), c23 = std::sqrt(1.0 - pp.sin2_th23);
                 for (int c = 0; c < kChannels; ++c) {
-                    int fin, fout, anti;
-                    channel_def(c, fin, fout, anti);
-                    const double d = anti ? -pp.delta_cp : pp.delta_cp;          // antineutrinos: W -> conj(W)
-                    const cd ep(std::cos(d), std::sin(d));
-                    const cd W[3][3] = {{cd(1.0), cd(0.0), cd(0.0)}, {cd(0.0), cd(c23), s23 * ep}, {cd(0.0), cd(-s23), c23 * ep}};
-                    for (int k = 0; k < sg.ch[c].nk; ++k) {
-                        const int i = el_i[c][k], j = el_j[c][k];
-                        cd coef = W[fout][i] * std::conj(W[fin][j]);
-                        if (i != j) coef += W[fout][j] * std::conj(W[fin][i]);
-                        sub.coef[c][k][0][l] = coef.real();
-                        sub.coef[c][k][1][l] = coef.imag();
-                        if (coef.imag() != 0.0) sg.ch[c].real_coef = 0;
-                    }
+                    int tt = 0;
+                    for (int t = 0; t < kScanTerms; ++t)
+                        if (sg.ch[c].tmask & (1 << t)) sub.mono[c][tt++][l] = mono[first + l][(size_t)c * kScanTerms + t];
                 }
             }
         }

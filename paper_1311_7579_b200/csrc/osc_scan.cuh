@@ -16,9 +16,13 @@
 // Work layout.  The histogram cell (channel, bin) of an event does not depend on the point either, so the events
 // are first sorted by cell (stable counting sort: scan_count / scan_offsets / scan_scatter).  A sorted cell is
 // cut into pieces of at most `piece` events; one warp takes a piece and, for every group, alternates
-//     phase A  lane = event : S' entries of 32 events into the warp's shared-memory slice
-//     phase B  lane = point : every lane walks the slice (broadcast reads) and adds w0 |sum_k c_k z_k|^2 to ONE
-//              REGISTER, because every event of the piece falls into the same histogram cell.
+//     phase A  lane = event : S' entries z_k of 64 events; what goes into the warp's shared-memory slice are the
+//              real numbers q_t = w0 |z_k|^2, w0 Re(z_k conj z_l), w0 Im(z_k conj z_l) that the points combine
+//     phase B  lane = point : w0 |sum_k c_k z_k|^2 = sum_t q_t m_t with the lane's monomials m_t = |c_k|^2,
+//              2 Re(c_k conj c_l), -2 Im(c_k conj c_l): every lane walks the slice (broadcast reads) and adds the
+//              terms to ONE REGISTER, because every event of the piece falls into the same histogram cell.
+//              Six fused multiply-adds per event and point for numu -> numu (real coefficients: the Im terms
+//              drop out), four for numu -> nue.
 // There is no histogram in shared memory, no atomic and no collision; partial[piece][point] is summed over the
 // pieces of a cell in order by scan_merge, so the result is a deterministic function of the inputs.
 #pragma once
@@ -41,10 +45,12 @@ struct ScanElem {
     double delta, ee, Tr0, T2r0, T2r1;
 };
 
+constexpr int kScanTerms = 9;         // |z0|^2 |z1|^2 |z2|^2  Re01 Re02 Re12  Im01 Im02 Im12 (canonical order)
+
 struct ScanChan {
     double sa;                 // +-K_MATTER Y_E rho (sign: antineutrino channel)
-    int nk;                    // entries used (1..3)
-    int real_coef;             // 1 if every coefficient of every lane is real (imaginary parts exactly 0)
+    int nk;                    // entries of S' used (1..3)
+    int tmask;                 // bit t set: term t of the canonical list is used (its monomial is non-zero for some point)
     ScanElem el[kScanElems];
 };
 
@@ -54,12 +60,13 @@ struct ScanGroup {
     ScanChan ch[kChannels];
 };
 
-// Coefficients of one sub-group (at most 32 points of one group): coef[channel][k][re, im][lane].
+// Monomials of one sub-group (at most 32 points of one group): mono[channel][t'][lane], t' counting the used
+// terms of the channel in canonical order.
 struct ScanSub {
     int group;
     int pt[kScanLanes];        // index of the lane's point in the caller's list, -1 for an unused lane
     int pad[3];
-    double coef[kChannels][kScanElems][2][kScanLanes];
+    double mono[kChannels][kScanTerms][kScanLanes];
 };
 
 struct ScanGeom {
@@ -246,7 +253,7 @@ __device__ __forceinline__ void scan_amp(const OscEig& e, double A, const ScanEl
 }
 
 constexpr int kSliceEvents = 64;      // events per phase-A slice of a warp (two per lane)
-constexpr int kSliceDoubles = 8;      // z0r z0i z1r z1i z2r z2i w0 pad
+constexpr int kSliceDoubles = 10;     // up to nine terms, padded to whole 16-byte words
 
 __device__ __forceinline__ ScanElem ldg_elem(const ScanElem* p)
 {
@@ -259,30 +266,58 @@ __device__ __forceinline__ ScanElem ldg_elem(const ScanElem* p)
     return e;
 }
 
-// Phase B: lane = point.  Every lane walks the `cnt` events of the slice (all lanes read the same words: one
-// shared-memory wavefront per 128-bit load) and accumulates w0 |sum_k c_k z_k|^2.
-template <int NK, bool REALC>
-__device__ __forceinline__ double scan_phase_b(uint32_t slice, int cnt, const double (&cr)[kScanElems],
-                                               const double (&ci)[kScanElems], double acc)
+// Phase A tail: the used terms of one event, times w0, compacted in canonical order into its slice row.
+__device__ __forceinline__ void scan_store_terms(double* row, int tmask, double w, const double (&zr)[kScanElems],
+                                                 const double (&zi)[kScanElems])
 {
-#pragma unroll 4
-    for (int j = 0; j < cnt; ++j) {
-        const uint32_t a = slice + (uint32_t)j * (8u * kSliceDoubles);
-        const double2 z0 = lds_f64x2(a), z1 = NK > 1 ? lds_f64x2(a + 16) : make_double2(0.0, 0.0);
-        const double2 z2 = NK > 2 ? lds_f64x2(a + 32) : make_double2(0.0, 0.0);
-        const double w = lds_f64(a + 48);
-        double ar = cr[0] * z0.x, ai = cr[0] * z0.y;
-        if (NK > 1) { ar = fma(cr[1], z1.x, ar); ai = fma(cr[1], z1.y, ai); }
-        if (NK > 2) { ar = fma(cr[2], z2.x, ar); ai = fma(cr[2], z2.y, ai); }
-        if (!REALC) {
-            ar = fma(-ci[0], z0.y, ar); ai = fma(ci[0], z0.x, ai);
-            if (NK > 1) { ar = fma(-ci[1], z1.y, ar); ai = fma(ci[1], z1.x, ai); }
-            if (NK > 2) { ar = fma(-ci[2], z2.y, ar); ai = fma(ci[2], z2.x, ai); }
+    int t = 0;
+    if (tmask & 1) row[t++] = w * fma(zr[0], zr[0], zi[0] * zi[0]);
+    if (tmask & 2) row[t++] = w * fma(zr[1], zr[1], zi[1] * zi[1]);
+    if (tmask & 4) row[t++] = w * fma(zr[2], zr[2], zi[2] * zi[2]);
+    if (tmask & 8) row[t++] = w * fma(zr[0], zr[1], zi[0] * zi[1]);
+    if (tmask & 16) row[t++] = w * fma(zr[0], zr[2], zi[0] * zi[2]);
+    if (tmask & 32) row[t++] = w * fma(zr[1], zr[2], zi[1] * zi[2]);
+    if (tmask & 64) row[t++] = w * fma(zi[0], zr[1], -(zr[0] * zi[1]));
+    if (tmask & 128) row[t++] = w * fma(zi[0], zr[2], -(zr[0] * zi[2]));
+    if (tmask & 256) row[t++] = w * fma(zi[1], zr[2], -(zr[1] * zi[2]));
+}
+
+// Phase B: lane = point.  Every lane walks the `cnt` events of the slice (all lanes read the same words: one
+// shared-memory wavefront per load) and accumulates sum_t q_t m_t.  Four events per step feed four independent
+// accumulators, so that one warp alone covers the latency of the fp64 pipe; consecutive fused multiply-adds share
+// the monomial operand.
+template <int NT>
+__device__ __forceinline__ void scan_phase_b(uint32_t slice, int cnt, const double (&m)[kScanTerms], double (&acc)[4])
+{
+    constexpr uint32_t ROW = 8u * kSliceDoubles;
+    int j = 0;
+    for (; j + 3 < cnt; j += 4) {
+        const uint32_t a = slice + (uint32_t)j * ROW;
+#pragma unroll
+        for (int t = 0; t + 1 < NT; t += 2) {
+            const double2 q0 = lds_f64x2(a + 8u * t), q1 = lds_f64x2(a + ROW + 8u * t);
+            const double2 q2 = lds_f64x2(a + 2 * ROW + 8u * t), q3 = lds_f64x2(a + 3 * ROW + 8u * t);
+            acc[0] = fma(q0.x, m[t], acc[0]);
+            acc[1] = fma(q1.x, m[t], acc[1]);
+            acc[2] = fma(q2.x, m[t], acc[2]);
+            acc[3] = fma(q3.x, m[t], acc[3]);
+            acc[0] = fma(q0.y, m[t + 1], acc[0]);
+            acc[1] = fma(q1.y, m[t + 1], acc[1]);
+            acc[2] = fma(q2.y, m[t + 1], acc[2]);
+            acc[3] = fma(q3.y, m[t + 1], acc[3]);
         }
-        const double P = fma(ar, ar, ai * ai);
-        acc = fma(w, P, acc);
+        if (NT & 1) {
+            acc[0] = fma(lds_f64(a + 8u * (NT - 1)), m[NT - 1], acc[0]);
+            acc[1] = fma(lds_f64(a + ROW + 8u * (NT - 1)), m[NT - 1], acc[1]);
+            acc[2] = fma(lds_f64(a + 2 * ROW + 8u * (NT - 1)), m[NT - 1], acc[2]);
+            acc[3] = fma(lds_f64(a + 3 * ROW + 8u * (NT - 1)), m[NT - 1], acc[3]);
+        }
     }
-    return acc;
+    for (; j < cnt; ++j) {
+        const uint32_t a = slice + (uint32_t)j * ROW;
+#pragma unroll
+        for (int t = 0; t < NT; ++t) acc[0] = fma(lds_f64(a + 8u * t), m[t], acc[0]);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -328,18 +363,16 @@ scan_main_kernel(const ScanGroup* __restrict__ groups, const ScanSub* __restrict
         const ScanChan* gc = &g->ch[ch];
         const double sa = __ldg(&gc->sa);
         const int nk = __ldg(&gc->nk);
-        const bool realc = __ldg(&gc->real_coef) != 0;
+        const int tmask = __ldg(&gc->tmask);
+        const int nt = __popc(tmask);
         const ScanElem el0 = ldg_elem(&gc->el[0]), el1 = ldg_elem(&gc->el[1]), el2 = ldg_elem(&gc->el[2]);
-        double cr[kScanElems], ci[kScanElems];
+        double m[kScanTerms];
 #pragma unroll
-        for (int k = 0; k < kScanElems; ++k) {
-            cr[k] = __ldg(&sub->coef[ch][k][0][lane]);
-            ci[k] = __ldg(&sub->coef[ch][k][1][lane]);
-        }
+        for (int t = 0; t < kScanTerms; ++t) m[t] = t < nt ? __ldg(&sub->mono[ch][t][lane]) : 0.0;
         const int pt = __ldg(&sub->pt[lane]);
-        double acc = 0.0;
+        double acc[4] = {0.0, 0.0, 0.0, 0.0};
         for (unsigned s0 = begin; s0 < end; s0 += kSliceEvents) {
-            // ---- phase A: lane = event (two per lane), S' entries into the slice -------------------------
+            // ---- phase A: lane = event (two per lane): S' entries, then the terms into the slice ------------
             const unsigned e0 = s0 + lane, e1 = e0 + 32;
             const double E0 = e0 < end ? __ldg(sEt + e0) : 1.0, E1 = e1 < end ? __ldg(sEt + e1) : 1.0;
             const double w0v = e0 < end ? __ldg(sW + e0) : 0.0, w1v = e1 < end ? __ldg(sW + e1) : 0.0;
@@ -347,31 +380,38 @@ scan_main_kernel(const ScanGroup* __restrict__ groups, const ScanSub* __restrict
             OscEig g0, g1;
             eig_solve(set, A0, rcp_pos(E0), g0);
             eig_solve(set, A1, rcp_pos(E1), g1);
-            double* r0 = my + (size_t)lane * kSliceDoubles;
-            double* r1 = r0 + 32 * kSliceDoubles;
-            double zr, zi;
-            scan_amp(g0, A0, el0, zr, zi); r0[0] = zr; r0[1] = zi;
-            scan_amp(g1, A1, el0, zr, zi); r1[0] = zr; r1[1] = zi;
+            double zr0[kScanElems] = {0.0, 0.0, 0.0}, zi0[kScanElems] = {0.0, 0.0, 0.0};
+            double zr1[kScanElems] = {0.0, 0.0, 0.0}, zi1[kScanElems] = {0.0, 0.0, 0.0};
+            scan_amp(g0, A0, el0, zr0[0], zi0[0]);
+            scan_amp(g1, A1, el0, zr1[0], zi1[0]);
             if (nk > 1) {
-                scan_amp(g0, A0, el1, zr, zi); r0[2] = zr; r0[3] = zi;
-                scan_amp(g1, A1, el1, zr, zi); r1[2] = zr; r1[3] = zi;
+                scan_amp(g0, A0, el1, zr0[1], zi0[1]);
+                scan_amp(g1, A1, el1, zr1[1], zi1[1]);
             }
             if (nk > 2) {
-                scan_amp(g0, A0, el2, zr, zi); r0[4] = zr; r0[5] = zi;
-                scan_amp(g1, A1, el2, zr, zi); r1[4] = zr; r1[5] = zi;
+                scan_amp(g0, A0, el2, zr0[2], zi0[2]);
+                scan_amp(g1, A1, el2, zr1[2], zi1[2]);
             }
-            r0[6] = w0v;
-            r1[6] = w1v;
+            scan_store_terms(my + (size_t)lane * kSliceDoubles, tmask, w0v, zr0, zi0);
+            scan_store_terms(my + (size_t)(lane + 32) * kSliceDoubles, tmask, w1v, zr1, zi1);
             __syncwarp();
             // ---- phase B: lane = point ------------------------------------------------------------------
             const int cnt = (int)min((unsigned)kSliceEvents, end - s0);
-            if (nk == 3 && realc) acc = scan_phase_b<3, true>(slice, cnt, cr, ci, acc);
-            else if (nk == 3) acc = scan_phase_b<3, false>(slice, cnt, cr, ci, acc);
-            else if (nk == 2) acc = scan_phase_b<2, false>(slice, cnt, cr, ci, acc);
-            else acc = scan_phase_b<1, false>(slice, cnt, cr, ci, acc);
+            switch (nt) {
+            case 1: scan_phase_b<1>(slice, cnt, m, acc); break;
+            case 2: scan_phase_b<2>(slice, cnt, m, acc); break;
+            case 3: scan_phase_b<3>(slice, cnt, m, acc); break;
+            case 4: scan_phase_b<4>(slice, cnt, m, acc); break;
+            case 5: scan_phase_b<5>(slice, cnt, m, acc); break;
+            case 6: scan_phase_b<6>(slice, cnt, m, acc); break;
+            case 7: scan_phase_b<7>(slice, cnt, m, acc); break;
+            case 8: scan_phase_b<8>(slice, cnt, m, acc); break;
+            case 9: scan_phase_b<9>(slice, cnt, m, acc); break;
+            default: break;                                     // no term: every monomial of the group is zero
+            }
             __syncwarp();
         }
-        if (pt >= 0) partial[(size_t)u * npoints + pt] = acc;
+        if (pt >= 0) partial[(size_t)u * npoints + pt] = (acc[0] + acc[1]) + (acc[2] + acc[3]);
     }
 }
 

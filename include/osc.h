@@ -109,13 +109,35 @@ int osc_reweight_bin(const double *E_true, const double *E_reco, const double *w
                      void *stream);
 
 /* Batched parameter sets (row a4; BASELINE.json configs[3]): slice p of hist_out equals
- * osc_reweight_bin run with points[p].  Independent of the state set by osc_set_params.
+ * osc_reweight_bin run with points[p] (to rounding: the order of the additions differs).  Independent of
+ * the state set by osc_set_params.
  *   points    HOST [n_points]; validated and copied before the call returns
- *   hist_out  DEVICE [n_points][OSC_N_CHANNELS][n_bins] fp64, OVERWRITTEN */
+ *   hist_out  DEVICE [n_points][OSC_N_CHANNELS][n_bins] fp64, OVERWRITTEN
+ * Two code paths, chosen per call from the point list (results agree to rounding, both are
+ * bit-reproducible from run to run):
+ *   - points that differ only in sin2_th23 and delta_cp share the matter eigen-problem.  When the list has
+ *     at least 8 points per such group on average (a scan grid: "only theta23 and dm2_32
+ *     float"), the events are sorted by histogram cell once and the eigen-solve is done once per (event,
+ *     group); a point then costs 4 to 6 fused multiply-adds per event (kernel k4, csrc/osc_scan.cuh);
+ *   - otherwise every (event, point) pair gets the full closed form from event tiles staged in shared
+ *     memory (kernel k3).
+ * The environment variable OSC_BATCH_PATH = k3 | k4, read at every call, forces one path (tests use it
+ * to check both paths on the same inputs); any other value, or none, leaves the choice to the library. */
 int osc_reweight_bin_batch(const osc_params *points, int n_points, const double *E_true,
                            const double *E_reco, const double *w0, const int8_t *channel, size_t n,
                            double energy_scale, const double *bin_edges, int n_bins, double *hist_out,
                            void *stream);
+
+/* Binned Poisson likelihood of rebuilt PDFs against a data histogram (PAPER.md:125-128,
+ * eq. 2.1, read as a product of Poisson probabilities of the bin contents -- DESIGN.md R5):
+ *     out[p] = -2 ln lambda_p = 2 sum_i [ mu - D_i + D_i ln(D_i / mu) ],   mu = norm * hist[p][i],
+ * the likelihood ratio against the saturated model (D_i ln(...) := 0 for D_i = 0; mu = 0 with D_i > 0 gives
+ * +inf; a negative or non-finite mu or D_i gives NaN).  Run after osc_reweight_bin_batch on the same stream,
+ * it leaves n_points doubles to copy back per scan instead of n_points histograms.
+ *   hist  DEVICE [n_points][n_cells] fp64 (n_cells = OSC_N_CHANNELS * n_bins for a full batched output)
+ *   data  DEVICE [n_cells] fp64, >= 0;   norm  finite, > 0;   out  DEVICE [n_points] fp64, overwritten */
+int osc_neg2lnl(const double *hist, int n_points, int n_cells, const double *data, double norm, double *out,
+                void *stream);
 
 /* Debug/verification export of the integer binning decision of osc_reweight_bin (row a3c):
  *   bin_out  DEVICE [n] int32: the bin index b of event j, or -1 if the event is dropped. */

@@ -77,6 +77,8 @@ def lib() -> ctypes.CDLL:
                                              _dp, ctypes.c_int, _dp]
         _lib.oracle_reweight_bin_batch.argtypes = [P, ctypes.c_int, _dp, _dp, _dp, _i8p, ctypes.c_size_t,
                                                    ctypes.c_double, _dp, ctypes.c_int, _dp]
+        _lib.oracle_neg2lnl.argtypes = [_dp, ctypes.c_int, ctypes.c_int, _dp, ctypes.c_double, _dp]
+        _lib.oracle_neg2lnl.restype = ctypes.c_int
         _lib.oracle_set_threads.argtypes = [ctypes.c_int]
         for f in ("oracle_prob", "oracle_prob_all", "oracle_evolution", "oracle_eigenvalues",
                   "oracle_bin_index", "oracle_reweight_bin", "oracle_reweight_bin_batch",
@@ -178,4 +180,14 @@ def reweight_bin_batch(points, E_true, E_reco, w0, channel, energy_scale: float,
     _check(lib().oracle_reweight_bin_batch(arr, len(points), _ptr(E_true), _ptr(E_reco), _ptr(w0),
                                            _ptr(channel, _i8p), E_true.size, float(energy_scale),
                                            _ptr(edges), nb, _ptr(out)), "oracle_reweight_bin_batch")
+    return out
+
+
+def neg2lnl(hist, data, norm: float = 1.0) -> np.ndarray:
+    """[n_points] values of the Poisson likelihood ratio -2 ln lambda of norm * hist[p] against data."""
+    data = _f64(data).ravel()
+    hist = _f64(hist).reshape(-1, data.size)
+    out = np.empty(hist.shape[0], dtype=np.float64)
+    _check(lib().oracle_neg2lnl(_ptr(hist), hist.shape[0], data.size, _ptr(data), float(norm), _ptr(out)),
+           "oracle_neg2lnl")
     return out

@@ -389,6 +389,31 @@ int oracle_reweight_bin_batch(const oracle_params *points, int n_points, const d
     return 0;
 }
 
+/* Binned Poisson likelihood ratio (eq. 2.1; reading R5 in DESIGN.md): for every point p
+ *   out[p] = 2 sum_i [ mu - D_i + D_i ln(D_i / mu) ],  mu = norm * hist[p][i],
+ * the term D_i ln(.) taken as 0 for D_i = 0; mu = 0 with D_i > 0 gives +inf, mu = 0 with D_i = 0 gives 0;
+ * a negative or non-finite mu or D_i gives NaN.  Long double, bins in index order.
+ * Pinned in tests/test_oracle_pins.py against scipy.stats.poisson.logpmf and closed forms. */
+int oracle_neg2lnl(const double *hist, int n_points, int n_cells, const double *data, double norm, double *out)
+{
+    if (!hist || !data || !out || n_points < 0 || n_cells < 1 || !(norm > 0.0)) return -1;
+    for (int p = 0; p < n_points; ++p) {
+        real s = 0.0L;
+        for (int i = 0; i < n_cells; ++i) {
+            const real mu = (real)norm * (real)hist[(size_t)p * n_cells + i];
+            const real D = (real)data[i];
+            real term;
+            if (!(mu >= 0.0L) || !(D >= 0.0L) || isinf(mu) || isinf(D)) term = NAN;
+            else if (mu == 0.0L) term = (D == 0.0L) ? 0.0L : INFINITY;
+            else if (D == 0.0L) term = mu;
+            else term = mu - D + D * logl(D / mu);
+            s += term;
+        }
+        out[p] = (double)(2.0L * s);
+    }
+    return 0;
+}
+
 int oracle_n_channels(void) { return ORACLE_N_CHANNELS; }
 
 #ifdef _OPENMP

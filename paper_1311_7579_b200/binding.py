@@ -24,7 +24,7 @@ PARAM_FIELDS = ("sin2_th12", "sin2_th23", "sin2_th13", "dm2_32", "dm2_21", "delt
 
 # every symbol include/osc.h declares (tests/test_abi.py checks the header against this list)
 EXPORTS = ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_batch",
-           "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_last_error", "osc_launch_count",
+           "osc_neg2lnl", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_last_error", "osc_launch_count",
            "osc_version", "osc_set_device", "osc_get_device", "osc_fp64_peak_probe")
 
 
@@ -58,13 +58,14 @@ def lib() -> ctypes.CDLL:
     L.osc_reweight_bin.argtypes = [_dp, _dp, _dp, _dp, sz, d, _dp, i, _dp, vp]
     L.osc_reweight_bin_batch.argtypes = [ctypes.POINTER(osc_params), i, _dp, _dp, _dp, _dp, sz, d, _dp, i, _dp, vp]
     L.osc_bin_index.argtypes = [_dp, _dp, _dp, sz, d, _dp, i, _dp, vp]
+    L.osc_neg2lnl.argtypes = [_dp, i, i, _dp, d, _dp, vp]
     L.osc_prob_host.argtypes = [_dp, sz, i, i, i, _dp]
     L.osc_reweight_bin_host.argtypes = [_dp, _dp, _dp, _dp, sz, d, _dp, i, _dp]
     L.osc_set_device.argtypes = [i]
     L.osc_get_device.argtypes = [ctypes.POINTER(i)]
     L.osc_fp64_peak_probe.argtypes = [i, i, ctypes.POINTER(d), vp]
     for name in ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_batch",
-                 "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_set_device", "osc_get_device",
+                 "osc_neg2lnl", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_set_device", "osc_get_device",
                  "osc_fp64_peak_probe"):
         getattr(L, name).restype = i
     L.osc_last_error.restype = ctypes.c_char_p
@@ -209,6 +210,23 @@ def osc_reweight_bin_batch(points: Sequence, E_true, E_reco, w0, channel, energy
                                         _dev(bin_edges, torch.float64, "bin_edges"), nb,
                                         _dev(hist_out, torch.float64, "hist_out"), _stream(stream)))
     return hist_out
+
+
+def osc_neg2lnl(hist, data, norm: float = 1.0, out=None, stream=None):
+    """[n_points] tensor of -2 ln lambda (Poisson likelihood ratio) of hist[p] * norm against data."""
+    import torch
+
+    n_cells = data.numel()
+    if n_cells == 0 or hist.numel() % n_cells != 0:
+        raise ValueError("hist must hold n_points * data.numel() values")
+    npts = hist.numel() // n_cells
+    if out is None:
+        out = torch.empty(npts, dtype=torch.float64, device=hist.device)
+    if out.numel() != npts:
+        raise ValueError("out must hold n_points values")
+    _check(lib().osc_neg2lnl(_dev(hist, torch.float64, "hist"), npts, n_cells, _dev(data, torch.float64, "data"),
+                             float(norm), _dev(out, torch.float64, "out"), _stream(stream)))
+    return out
 
 
 def osc_bin_index(E_true, E_reco, channel, energy_scale: float, bin_edges, bin_out=None, stream=None):

@@ -16,6 +16,7 @@
 
 #include "../../include/osc.h"
 #include "osc_kernels.cuh"
+#include "osc_like.cuh"
 #include "osc_scan.cuh"
 #include "osc_precompute.h"
 
@@ -713,6 +714,21 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
     if ((rc = post_launch("osc_reweight_bin_batch"))) return rc;
     merge_chunks_kernel<<<n_points, 256, 0, st>>>(partial, (int)nchunks, (int)nh, hist_out);
     return post_launch("osc_reweight_bin_batch merge");
+}
+
+int osc_neg2lnl(const double* hist, int n_points, int n_cells, const double* data, double norm, double* out,
+                void* stream)
+{
+    if (n_points < 0 || n_cells < 1) return fail(OSC_ERR_INVALID_ARG, "osc_neg2lnl: n_points < 0 or n_cells < 1");
+    if (n_points == 0) return OSC_OK;
+    if (!hist || !data || !out) return fail(OSC_ERR_INVALID_ARG, "osc_neg2lnl: null pointer");
+    if (!(norm > 0.0) || !std::isfinite(norm)) return fail(OSC_ERR_INVALID_ARG, "osc_neg2lnl: norm must be finite and > 0");
+    if (!aligned(hist, 8) || !aligned(data, 8) || !aligned(out, 8))
+        return fail(OSC_ERR_ALIGNMENT, "osc_neg2lnl: fp64 array not 8-byte aligned");
+    const int warps = 8;
+    neg2lnl_kernel<<<(n_points + warps - 1) / warps, 32 * warps, 0, static_cast<cudaStream_t>(stream)>>>(
+        hist, n_points, n_cells, data, norm, out);
+    return post_launch("osc_neg2lnl");
 }
 
 int osc_bin_index(const double* E_true, const double* E_reco, const int8_t* channel, size_t n, double energy_scale,

@@ -355,3 +355,47 @@ def test_p12_batch_slices_and_energy_scales():
     one_bin = np.array([-1e30, 1e30])
     totals = [oracle.reweight_bin(pts[4], et, er, w0, ch, s, one_bin) for s in workloads.ENERGY_SCALES]
     assert np.array_equal(totals[0], totals[1]) and np.array_equal(totals[1], totals[2])
+
+
+# ------------------------------------------------------------------------------------------------
+# P13: binned Poisson likelihood ratio (eq. 2.1; reading R5)
+# ------------------------------------------------------------------------------------------------
+def test_p13_neg2lnl_against_scipy_poisson_pmf():
+    """For integer data -2 ln lambda = -2 [ln Pois(D | mu) - ln Pois(D | D)], bin by bin (scipy's pmf, not a
+    retyped formula)."""
+    from scipy.stats import poisson
+
+    rng = np.random.default_rng(5)
+    mu = rng.uniform(0.05, 400.0, (7, 60))
+    D = rng.poisson(mu[3]).astype(np.float64)
+    D[::11] = 0.0
+    got = oracle.neg2lnl(mu, D, 1.0)
+    for p in range(mu.shape[0]):
+        sat = np.where(D > 0, poisson.logpmf(D, np.maximum(D, 1e-300)), 0.0)
+        ref = -2.0 * np.sum(poisson.logpmf(D, mu[p]) - sat)
+        assert abs(got[p] - ref) <= 1e-9 * max(abs(ref), 1.0)
+
+
+def test_p13_neg2lnl_closed_forms():
+    rng = np.random.default_rng(6)
+    mu = rng.uniform(0.1, 50.0, (3, 40))
+    # data equal to the expectation: exactly the saturated model
+    assert np.all(np.abs(oracle.neg2lnl(mu[1:2], mu[1], 1.0)) < 1e-12)
+    # empty data: 2 * sum(mu); the normalisation multiplies the expectation
+    z = np.zeros(40)
+    np.testing.assert_allclose(oracle.neg2lnl(mu, z, 1.0), 2.0 * mu.sum(axis=1), rtol=1e-14)
+    np.testing.assert_allclose(oracle.neg2lnl(mu, z, 2.5), 5.0 * mu.sum(axis=1), rtol=1e-14)
+    # one bin, D = e * mu: 2 [mu - e mu + e mu] = 2 mu
+    got = oracle.neg2lnl(np.array([[3.0]]), np.array([3.0 * math.e]), 1.0)
+    assert abs(got[0] - 6.0) < 1e-13
+    # scaling norm and 1/hist together changes nothing; the result is >= 0 and additive over bins
+    D = rng.poisson(mu[0]).astype(np.float64)
+    a = oracle.neg2lnl(mu, D, 1.0)
+    np.testing.assert_allclose(oracle.neg2lnl(mu / 4.0, D, 4.0), a, rtol=1e-13)
+    assert np.all(a >= 0.0)
+    np.testing.assert_allclose(oracle.neg2lnl(mu[:, :17], D[:17], 1.0) + oracle.neg2lnl(mu[:, 17:], D[17:], 1.0), a,
+                               rtol=1e-13)
+    # degenerate bins: mu = 0 with and without data; invalid entries
+    assert oracle.neg2lnl(np.array([[0.0, 1.0]]), np.array([0.0, 1.0]), 1.0)[0] == 0.0
+    assert np.isinf(oracle.neg2lnl(np.array([[0.0, 1.0]]), np.array([2.0, 1.0]), 1.0)[0])
+    assert np.isnan(oracle.neg2lnl(np.array([[-1.0, 1.0]]), np.array([2.0, 1.0]), 1.0)[0])

@@ -489,6 +489,43 @@ def test_k4_all_events_dropped(osc):
 
 
 # ------------------------------------------------------------------------------------------------
+# NEXT-2: Poisson likelihood ratio of the batched histograms on the device (osc_neg2lnl)
+# ------------------------------------------------------------------------------------------------
+def test_neg2lnl_after_batch(osc):
+    pts = wl.scan_points()[::16][:64]
+    n = 50_000 + 3
+    et, er, w0, ch = wl.events(n, seed=31)
+    edges = wl.bin_edges()
+    d = [dev(a) for a in (et, er, w0, ch)]
+    hist = osc.osc_reweight_bin_batch(pts, *d, 1.0, dev(edges))
+    # "data": Poisson draws around the Table-1 expectation (seeded, made on the host from the oracle's histogram)
+    ref_hist = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 1.0, edges)
+    base = oracle.reweight_bin(oracle.Params(**wl.table1()), et, er, w0, ch, 1.0, edges)
+    norm = 0.02
+    data = np.random.default_rng(32).poisson(norm * base).astype(np.float64).ravel()
+    got = host(osc.osc_neg2lnl(hist, dev(data), norm))
+    ref = oracle.neg2lnl(ref_hist, data, norm)
+    assert got.shape == (64,)
+    scale = float(norm * ref_hist.sum(axis=(1, 2)).max() + data.sum())
+    assert np.max(np.abs(got - ref)) <= 1e-12 * scale + 1e-9 * np.max(np.abs(ref))
+
+
+def test_neg2lnl_edge_cases(osc):
+    hist = np.array([[0.0, 2.0, 5.0], [0.0, 2.0, 5.0], [1.0, 0.0, 3.0], [1.0, -1.0, 3.0], [4.0, 4.0, 4.0]])
+    data = np.array([0.0, 2.0, 5.0])
+    got = host(osc.osc_neg2lnl(dev(hist), dev(data), 1.0))
+    ref = oracle.neg2lnl(hist, data, 1.0)
+    assert got[0] == 0.0 and got[1] == 0.0
+    assert np.isinf(got[2]) and np.isinf(ref[2]) and np.isnan(got[3]) and np.isnan(ref[3])
+    assert abs(got[4] - ref[4]) <= 1e-13 * abs(ref[4])
+    many = np.random.default_rng(33).uniform(0.0, 30.0, (1000, 37))
+    d37 = np.random.default_rng(34).poisson(15.0, 37).astype(np.float64)
+    g, r = host(osc.osc_neg2lnl(dev(many), dev(d37), 0.7)), oracle.neg2lnl(many, d37, 0.7)
+    np.testing.assert_allclose(g, r, rtol=1e-12)
+    assert osc.osc_neg2lnl(dev(many[:0]), dev(d37), 1.0).numel() == 0
+
+
+# ------------------------------------------------------------------------------------------------
 # asynchrony: parameters are captured at enqueue time; work runs on the caller's stream
 # ------------------------------------------------------------------------------------------------
 def test_params_captured_at_enqueue_on_side_stream(osc):

@@ -108,6 +108,18 @@ int osc_reweight_bin(const double *E_true, const double *E_reco, const double *w
                      size_t n, double energy_scale, const double *bin_edges, int n_bins, double *hist_out,
                      void *stream);
 
+/* osc_reweight_bin for several energy-scale values in one pass over the events: slice k
+ * of hist_out equals osc_reweight_bin run with energy_scales[k] (to rounding: the order of the additions
+ * differs; the result is bit-reproducible from run to run).  The oscillation weight does not depend on the
+ * energy scale (it uses the unscaled E_true), so the closed form runs once per event instead of
+ * once per event and scale.
+ *   energy_scales  HOST [n_scales], 1 <= n_scales <= 4, each finite and > 0
+ *   hist_out       DEVICE [n_scales][OSC_N_CHANNELS][n_bins] fp64, OVERWRITTEN
+ * Binnings whose sub-histograms do not fit shared memory n_scales times fall back to one pass per scale. */
+int osc_reweight_bin_scales(const double *E_true, const double *E_reco, const double *w0, const int8_t *channel,
+                            size_t n, const double *energy_scales, int n_scales, const double *bin_edges,
+                            int n_bins, double *hist_out, void *stream);
+
 /* Batched parameter sets (row a4; BASELINE.json configs[3]): slice p of hist_out equals
  * osc_reweight_bin run with points[p] (to rounding: the order of the additions differs).  Independent of
  * the state set by osc_set_params.

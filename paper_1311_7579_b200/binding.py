@@ -23,7 +23,7 @@ PARAM_FIELDS = ("sin2_th12", "sin2_th23", "sin2_th13", "dm2_32", "dm2_21", "delt
                 "L_km", "hierarchy")
 
 # every symbol include/osc.h declares (tests/test_abi.py checks the header against this list)
-EXPORTS = ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_batch",
+EXPORTS = ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_scales", "osc_reweight_bin_batch",
            "osc_neg2lnl", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_last_error", "osc_launch_count",
            "osc_version", "osc_set_device", "osc_get_device", "osc_fp64_peak_probe")
 
@@ -56,6 +56,7 @@ def lib() -> ctypes.CDLL:
     L.osc_prob.argtypes = [_dp, sz, i, i, i, _dp, vp]
     L.osc_prob_all.argtypes = [_dp, sz, i, _dp, vp]
     L.osc_reweight_bin.argtypes = [_dp, _dp, _dp, _dp, sz, d, _dp, i, _dp, vp]
+    L.osc_reweight_bin_scales.argtypes = [_dp, _dp, _dp, _dp, sz, ctypes.POINTER(d), i, _dp, i, _dp, vp]
     L.osc_reweight_bin_batch.argtypes = [ctypes.POINTER(osc_params), i, _dp, _dp, _dp, _dp, sz, d, _dp, i, _dp, vp]
     L.osc_bin_index.argtypes = [_dp, _dp, _dp, sz, d, _dp, i, _dp, vp]
     L.osc_neg2lnl.argtypes = [_dp, i, i, _dp, d, _dp, vp]
@@ -64,7 +65,8 @@ def lib() -> ctypes.CDLL:
     L.osc_set_device.argtypes = [i]
     L.osc_get_device.argtypes = [ctypes.POINTER(i)]
     L.osc_fp64_peak_probe.argtypes = [i, i, ctypes.POINTER(d), vp]
-    for name in ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_batch",
+    for name in ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_scales",
+                 "osc_reweight_bin_batch",
                  "osc_neg2lnl", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_set_device", "osc_get_device",
                  "osc_fp64_peak_probe"):
         getattr(L, name).restype = i
@@ -184,6 +186,24 @@ def osc_reweight_bin(E_true, E_reco, w0, channel, energy_scale: float, bin_edges
         raise ValueError("hist_out must hold N_CHANNELS * n_bins values")
     _check(lib().osc_reweight_bin(pt, pr, pw, pc, n, float(energy_scale), _dev(bin_edges, torch.float64, "bin_edges"),
                                   nb, _dev(hist_out, torch.float64, "hist_out"), _stream(stream)))
+    return hist_out
+
+
+def osc_reweight_bin_scales(E_true, E_reco, w0, channel, energy_scales: Sequence[float], bin_edges, hist_out=None,
+                            stream=None):
+    """[n_scales, N_CHANNELS, n_bins] histograms, one slice per energy-scale value, in one pass over the events."""
+    import torch
+
+    n, pt, pr, pw, pc = _event_ptrs(E_true, E_reco, w0, channel)
+    nb = bin_edges.numel() - 1
+    ns = len(energy_scales)
+    arr = (ctypes.c_double * max(ns, 1))(*[float(v) for v in energy_scales])
+    if hist_out is None:
+        hist_out = torch.empty((ns, N_CHANNELS, nb), dtype=torch.float64, device=E_true.device)
+    if hist_out.numel() != ns * N_CHANNELS * nb:
+        raise ValueError("hist_out must hold n_scales * N_CHANNELS * n_bins values")
+    _check(lib().osc_reweight_bin_scales(pt, pr, pw, pc, n, arr, ns, _dev(bin_edges, torch.float64, "bin_edges"), nb,
+                                         _dev(hist_out, torch.float64, "hist_out"), _stream(stream)))
     return hist_out
 
 

@@ -246,6 +246,64 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
                                        n_bins, n_sub, ms, hist_out);
 }
 
+template <bool VEC, int NS>
+int launch_k2s(int grid, size_t smem, cudaStream_t st, const BinArgs& args, const ScaleArgs& sc, const double* E_true,
+               const double* E_reco, const double* w0, const int8_t* channel, size_t n, const double* bin_edges,
+               int n_bins, int n_sub, const MergeScratch& ms, double* hist_out)
+{
+    CUDA_TRY(cudaFuncSetAttribute(reweight_bin_scales_kernel<VEC, 256, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)smem));
+    reweight_bin_scales_kernel<VEC, 256, NS><<<grid, 256, smem, st>>>(args, sc, E_true, E_reco, w0, channel, n, bin_edges,
+                                                                      n_bins, n_sub, ms, hist_out);
+    return post_launch("osc_reweight_bin_scales");
+}
+
+// k2s for n_scales in [2, kMaxScales]; returns 1 (not an error code) when the sub-histograms of all scales do not
+// fit the shared memory of one SM twice, in which case the caller runs one k2 pass per scale.
+int launch_reweight_scales(const BinArgs& args, const double* E_true, const double* E_reco, const double* w0,
+                           const int8_t* channel, size_t n, const double* scales, int n_scales,
+                           const double* bin_edges, int n_bins, double* hist_out, cudaStream_t st)
+{
+    const size_t nht = (size_t)n_scales * kChannels * n_bins;
+    const size_t fixed = sizeof(double) * kBinArgsDoubles + bin_table_bytes(n_bins);
+    const size_t sub1 = sizeof(double) * 8 * kSlots * nht;              // 8 warps
+    if (2 * (fixed + sub1 + 1024) > kSmemBudget) return 1;
+    const int n_sub = 2 * (fixed + 2 * sub1 + 1024) <= kSmemBudget ? 2 : 1;
+    const size_t smem = fixed + n_sub * sub1;
+    int sms = 0;
+    int rc = sm_count(&sms);
+    if (rc) return rc;
+    const size_t ntiles = (n + 511) / 512;
+    if (ntiles > 0xFFFFFFFFull) return fail(OSC_ERR_INVALID_ARG, "n = %zu events is more than one call takes (2^32 tiles)", n);
+    size_t g = (size_t)sms * 2;
+    if (ntiles < g) g = ntiles;
+    const int grid = (int)g;
+    const int ngroups = (grid + kGroup - 1) / kGroup;
+    const size_t bytes_partial = (size_t)grid * nht * sizeof(double);
+    const size_t bytes_gpartial = (size_t)ngroups * nht * sizeof(double);
+    char* scratch = nullptr;
+    if ((rc = stream_scratch(kCounterBytes + bytes_partial + bytes_gpartial, st, &scratch))) return rc;
+    MergeScratch ms;
+    ms.counters = reinterpret_cast<unsigned int*>(scratch);
+    ms.partial = reinterpret_cast<double*>(scratch + kCounterBytes);
+    ms.gpartial = reinterpret_cast<double*>(scratch + kCounterBytes + bytes_partial);
+    ms.ngroups = ngroups;
+    ScaleArgs sc;
+    for (int k = 0; k < kMaxScales; ++k) sc.s[k] = k < n_scales ? scales[k] : 1.0;
+    const bool vec = aligned(E_true, 16) && aligned(E_reco, 16) && aligned(w0, 16) && aligned(channel, 2);
+#define OSC_K2S(NS)                                                                                                  \
+    return vec ? launch_k2s<true, NS>(grid, smem, st, args, sc, E_true, E_reco, w0, channel, n, bin_edges, n_bins,    \
+                                      n_sub, ms, hist_out)                                                           \
+               : launch_k2s<false, NS>(grid, smem, st, args, sc, E_true, E_reco, w0, channel, n, bin_edges, n_bins,   \
+                                       n_sub, ms, hist_out)
+    switch (n_scales) {
+    case 2: OSC_K2S(2);
+    case 3: OSC_K2S(3);
+    default: OSC_K2S(4);
+    }
+#undef OSC_K2S
+}
+
 // Device staging buffers of the *_host entry points (grown on demand, reused between calls).
 struct HostPath {
     std::mutex mu;
@@ -618,6 +676,36 @@ int launch_batch_scan(const ScanPlan& plan, int n_points, const double* E_true, 
 }
 
 } // namespace
+
+int osc_reweight_bin_scales(const double* E_true, const double* E_reco, const double* w0, const int8_t* channel,
+                            size_t n, const double* energy_scales, int n_scales, const double* bin_edges, int n_bins,
+                            double* hist_out, void* stream)
+{
+    if (n_scales < 1 || n_scales > kMaxScales)
+        return fail(OSC_ERR_INVALID_ARG, "n_scales = %d outside [1, %d]", n_scales, kMaxScales);
+    if (!energy_scales) return fail(OSC_ERR_INVALID_ARG, "null energy_scales");
+    int rc = OSC_OK;
+    for (int k = 0; k < n_scales; ++k)
+        if ((rc = check_bin_args(E_true, E_reco, w0, channel, n, energy_scales[k], bin_edges, n_bins, hist_out))) return rc;
+    if (n > 0 && !w0) return fail(OSC_ERR_INVALID_ARG, "null w0 with n > 0");
+    if (!aligned(hist_out, 8)) return fail(OSC_ERR_ALIGNMENT, "hist_out not 8-byte aligned");
+    HostSet h;
+    if ((rc = snapshot(h))) return rc;
+    BinArgs args;
+    make_bin_args(h, args);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t nh = (size_t)kChannels * n_bins;
+    if (n_scales > 1 && n > 0) {
+        rc = launch_reweight_scales(args, E_true, E_reco, w0, channel, n, energy_scales, n_scales, bin_edges, n_bins,
+                                    hist_out, st);
+        if (rc != 1) return rc;
+    }
+    for (int k = 0; k < n_scales; ++k)          // one scale, no events, or histograms too large to fuse
+        if ((rc = launch_reweight(args, E_true, E_reco, w0, channel, n, energy_scales[k], bin_edges, n_bins,
+                                  hist_out + (size_t)k * nh, st)))
+            return rc;
+    return OSC_OK;
+}
 
 int osc_reweight_bin_batch(const osc_params* points, int n_points, const double* E_true, const double* E_reco,
                            const double* w0, const int8_t* channel, size_t n, double energy_scale,

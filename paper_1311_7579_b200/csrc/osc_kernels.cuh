@@ -322,6 +322,103 @@ reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict_
 }
 
 // ------------------------------------------------------------------------------------------------
+// k2s: k2 for several energy-scale values in one pass ("all-systematics call").  The
+// oscillation weight does not depend on the energy scale (A9: it acts on E_reco only), so the closed form runs once
+// per event and only the binning and the histogram update run once per scale.  The NS histograms are laid out as one
+// histogram of NS * 4 * nb cells (scale-major), which is also the layout of hist_out, so the sub-histogram and merge
+// machinery of k2 is used unchanged.
+// ------------------------------------------------------------------------------------------------
+constexpr int kMaxScales = 4;
+
+struct ScaleArgs {
+    double s[kMaxScales];
+};
+
+template <bool VEC, int THREADS, int NS, int STEPS>
+__device__ __forceinline__ void k2s_loop(const BinArgs& a, const double* __restrict__ E_true,
+                                         const double* __restrict__ E_reco, const double* __restrict__ w0,
+                                         const int8_t* __restrict__ channel, size_t n, const ScaleArgs& sc,
+                                         const BinView& bt, uint32_t pb, const LaneHist& lh, unsigned lt_mask,
+                                         unsigned ntiles, unsigned t, EventPair cur)
+{
+    const int nh = kChannels * bt.nb;
+    while (t < ntiles) {
+        const unsigned ch0 = cur.chp & 0xFFu, ch1 = cur.chp >> 8;
+        const bool ok0 = energy_ok(cur.Et0) && ch0 < (unsigned)kChannels;
+        const bool ok1 = energy_ok(cur.Et1) && ch1 < (unsigned)kChannels;
+        const unsigned c0 = ok0 ? ch0 : 0u, c1 = ok1 ? ch1 : 0u;
+        const double Es0 = ok0 ? cur.Et0 : 1.0, Es1 = ok1 ? cur.Et1 : 1.0;
+        HistPlan plan[NS];
+#pragma unroll
+        for (int k = 0; k < NS; ++k) {
+            const int b0 = find_bin<STEPS>(bt, scaled_energy(sc.s[k], cur.Er0));     // a3b, a3c per scale
+            const int b1 = find_bin<STEPS>(bt, scaled_energy(sc.s[k], cur.Er1));
+            const int cell0 = (ok0 && b0 >= 0) ? k * nh + (int)c0 * bt.nb + b0 : -1;
+            const int cell1 = (ok1 && b1 >= 0) ? k * nh + (int)c1 * bt.nb + b1 : -1;
+            warp_hist_match(plan[k], lh, cell0, cell1);
+        }
+        const double wp0 = cur.wp0, wp1 = cur.wp1;
+        t += gridDim.x;
+        if (t < ntiles) cur = load_pair<VEC, THREADS>(E_true, E_reco, w0, channel, n, t);
+        const OscTrans tr0 = load_trans(pb, (int)c0);
+        const OscTrans tr1 = load_trans(pb, (int)c1);
+        const double A0 = tr0.sa * Es0, A1 = tr1.sa * Es1;  // a2a
+        OscEig e0, e1;
+        eig_solve(a.set, A0, rcp_pos(Es0), e0);             // a2b-a2d
+        eig_solve(a.set, A1, rcp_pos(Es1), e1);
+#pragma unroll
+        for (int k = 0; k < NS; ++k) warp_hist_rank(plan[k], lt_mask);
+        const double w_0 = __dmul_rn(wp0, assemble(e0, A0, tr0));   // a2e-a2f, a3a
+        const double w_1 = __dmul_rn(wp1, assemble(e1, A1, tr1));
+#pragma unroll
+        for (int k = 0; k < NS; ++k) warp_hist_commit(plan[k], w_0, w_1);
+    }
+}
+
+// Shared memory per block:  param block | bin table | hist[warps][kSlots][n_sub][NS * 4 * nb]
+template <bool VEC, int THREADS, int NS>
+__global__ void __launch_bounds__(THREADS, 512 / THREADS)
+reweight_bin_scales_kernel(const __grid_constant__ BinArgs a, const __grid_constant__ ScaleArgs sc,
+                           const double* __restrict__ E_true, const double* __restrict__ E_reco,
+                           const double* __restrict__ w0, const int8_t* __restrict__ channel, size_t n,
+                           const double* __restrict__ edges, int nb, int n_sub, MergeScratch ms,
+                           double* __restrict__ hist_out)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int WARPS = THREADS / 32;
+    const int nht = NS * kChannels * nb;
+    double* pbuf = reinterpret_cast<double*>(smem_raw);
+    unsigned char* tab = smem_raw + sizeof(double) * kBinArgsDoubles;
+    double* hist = reinterpret_cast<double*>(tab + bin_table_bytes(nb));
+    __shared__ unsigned int s_ticket;
+
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned warp = threadIdx.x >> 5;
+    const int n_hist = WARPS * kSlots * n_sub;
+    const unsigned ntiles = pin_u32((unsigned)((n + 2 * THREADS - 1) / (2 * THREADS)));
+    const unsigned t = blockIdx.x;
+    EventPair cur = load_pair<VEC, THREADS>(E_true, E_reco, w0, channel, n, t);   // grid <= ntiles
+
+    if (threadIdx.x < kBinArgsDoubles) pbuf[threadIdx.x] = reinterpret_cast<const double*>(&a)[threadIdx.x];
+    for (int i = threadIdx.x; i < n_hist * nht; i += THREADS) hist[i] = 0.0;
+    build_bin_table(tab, edges, nb);
+    BinView bt = bin_view(tab);
+    bt.ekey = pin_u32(bt.ekey);
+    bt.lut = pin_u32(bt.lut);
+    const uint32_t pb = pin_u32(smem_u32(pbuf));
+    LaneHist lh = lane_hist(hist, nht, n_sub, warp, lane);
+    lh.h0 = pin_u32(lh.h0);
+    lh.h1 = pin_u32(lh.h1);
+    const unsigned lt_mask = pin_u32((1u << lane) - 1u);
+
+    if (bt.steps <= 1u)
+        k2s_loop<VEC, THREADS, NS, 1>(a, E_true, E_reco, w0, channel, n, sc, bt, pb, lh, lt_mask, ntiles, t, cur);
+    else
+        k2s_loop<VEC, THREADS, NS, 0>(a, E_true, E_reco, w0, channel, n, sc, bt, pb, lh, lt_mask, ntiles, t, cur);
+    block_merge(hist, n_hist, nht, ms, hist_out, &s_ticket);
+}
+
+// ------------------------------------------------------------------------------------------------
 // k3: batched parameter sets (row a4).  Block (c, g) owns event chunk c and point group g.  The chunk is
 // staged tile by tile in shared memory -- E_true, w0 and the histogram cell of every event, which does
 // not depend on the parameter set and is therefore decided once per tile -- and every staged tile is

@@ -489,6 +489,50 @@ def test_k4_all_events_dropped(osc):
 
 
 # ------------------------------------------------------------------------------------------------
+# NEXT-3: several energy scales in one pass (osc_reweight_bin_scales)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("scales", [(1.0,), (0.97, 1.03), wl.ENERGY_SCALES, (0.9, 0.97, 1.0, 1.1)])
+def test_scales_one_pass_vs_oracle_and_single_calls(osc, scales):
+    n = 300_000 + 11
+    et, er, w0, ch = wl.events(n, seed=41)
+    et[3] = 0.0; ch[4] = 7; er[5] = -2.0
+    edges = wl.bin_edges()
+    d = [dev(a) for a in (et, er, w0, ch)]
+    de = dev(edges)
+    op = set_params(osc, wl.table1(delta_cp=-1.1))
+    got = host(osc.osc_reweight_bin_scales(*d, scales, de))
+    again = host(osc.osc_reweight_bin_scales(*d, scales, de))
+    assert got.shape == (len(scales), 4, 50) and np.array_equal(got, again)
+    for k, s in enumerate(scales):
+        assert_hist_close(got[k], oracle.reweight_bin(op, et, er, w0, ch, s, edges), f"scales[{k}]={s}")
+        single = host(osc.osc_reweight_bin(*d, s, de))
+        np.testing.assert_allclose(got[k], single, rtol=1e-12, atol=0.0)
+
+
+@pytest.mark.parametrize("n", [0, 1, 33, 513, 1025])
+def test_scales_ragged_and_unaligned(osc, n):
+    et, er, w0, ch = wl.events(n + 3, seed=42)
+    edges = wl.bin_edges(13, 4.0)
+    op = set_params(osc, wl.table1(hierarchy=-1))
+    big = [dev(a) for a in (et, er, w0, ch)]
+    d = [t[1:1 + n] for t in big]                      # 8-byte aligned only: the scalar load path
+    got = host(osc.osc_reweight_bin_scales(*d, wl.ENERGY_SCALES, dev(edges)))
+    for k, s in enumerate(wl.ENERGY_SCALES):
+        ref = oracle.reweight_bin(op, et[1:1 + n], er[1:1 + n], w0[1:1 + n], ch[1:1 + n], s, edges)
+        assert_hist_close(got[k], ref, f"scales ragged n={n} s={s}")
+
+
+def test_scales_fall_back_for_large_binnings(osc):
+    n = 20_000
+    et, er, w0, ch = wl.events(n, seed=43)
+    edges = wl.bin_edges(700, 5.0)                     # three scales of 4 x 700 bins do not fit shared memory
+    op = set_params(osc, wl.table1())
+    got = host(osc.osc_reweight_bin_scales(dev(et), dev(er), dev(w0), dev(ch), wl.ENERGY_SCALES, dev(edges)))
+    for k, s in enumerate(wl.ENERGY_SCALES):
+        assert_hist_close(got[k], oracle.reweight_bin(op, et, er, w0, ch, s, edges), f"fallback s={s}")
+
+
+# ------------------------------------------------------------------------------------------------
 # NEXT-2: Poisson likelihood ratio of the batched histograms on the device (osc_neg2lnl)
 # ------------------------------------------------------------------------------------------------
 def test_neg2lnl_after_batch(osc):

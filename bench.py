@@ -40,10 +40,10 @@ SCALES = wl.ENERGY_SCALES
 BYTES_PER_EVENT = 25          # E_true + E_reco + w0 (fp64) + channel (int8): SURVEY.md 8(d), DESIGN.md "k2"
 # fp64 operations k2 executes per event (DFMA = 2, DMUL/DADD = 1), counted by ncu
 # (smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum / events): DESIGN.md 5.1, profiles/r1_k2_full_a.md.
-FLOP_PER_EVENT = 205.8
+FLOP_PER_EVENT = 199.3        # 75.0 DFMA + 42.0 DMUL + 7.3 DADD per event (profiles/r1_k2_full_b.md)
 # dram__bytes_read.sum + dram__bytes_write.sum of one k2 launch over 1e7 events (same capture); algorithmic: 250.0e6
-NCU_TRAFFIC_BYTES_1E7 = 253.72e6
-NCU_TRAFFIC_SOURCE = "profiles/r1_k2_full_a.md"
+NCU_TRAFFIC_BYTES_1E7 = 253.66e6
+NCU_TRAFFIC_SOURCE = "profiles/r1_k2_full_b.md"
 FP64_LANES_PER_SM_CLK = 64    # B200 (sm_100): 4 sub-partitions x 16 fp64 lanes; DESIGN.md "fp64 roofline"
 
 
@@ -56,9 +56,11 @@ def parse():
     ap.add_argument("--events", type=int, default=None, help="events per GPU (default: the size the config names)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--workload", default="config2", choices=["config0", "config1", "config2", "config3"],
+    ap.add_argument("--workload", default="config2", choices=["config0", "config1", "config2", "config3", "config3-k3",
+                                                               "config4"],
                     help="config2 (default) is the bench line; the others time the remaining BASELINE.json configs "
-                         "for BASELINE.md section 4 and give ncu a committed command for k1 / k1b / k3")
+                         "for BASELINE.md section 4 and give ncu a committed command for k1 / k1b / k3 / k4 "
+                         "(config3-k3 forces the unfactorised batched kernel; config4 is the size sweep)")
     return ap.parse_args()
 
 
@@ -187,6 +189,7 @@ def run_reference(args):
     }))
 
 
+K4_FLOP_PER_UNIT = 17.4       # all kernels of one factorised call, ncu (profiles/r1_launches_k4.md)
 # Per-config description of the secondary workloads: (events, units per event per step, bytes per unit, flop per unit)
 #   flop per unit: ncu-counted fp64 operations of the kernel that runs, bytes: algorithmic.
 OTHER = {
@@ -195,9 +198,14 @@ OTHER = {
     "config1": dict(n=10_000_000, kernel="prob_all_kernel (k1b)", bytes_per_unit=80.0, flop_per_unit=290.0,
                     what="configs[1]: 1e7 events, all 9 transitions for nu and nubar (2 osc_prob_all calls = "
                          "18 output arrays), delta_cp drawn per step, both hierarchies alternate"),
-    "config3": dict(n=1_000_000, kernel="reweight_batch_kernel (k3)", bytes_per_unit=25.0 / 1024, flop_per_unit=205.8,
+    # k4: fp64 operations the factorised path executes per (event, point), all its kernels together, counted by ncu
+    # (profiles/r1_k4_ops.md): the eigen-solve is shared by the 32 points of a dm2_32 group
+    "config3": dict(n=1_000_000, kernel="scan_main_kernel + sort/merge kernels (k4, factorised)",
+                    bytes_per_unit=25.0 / 1024, flop_per_unit=K4_FLOP_PER_UNIT,
                     what="configs[3]: 1e6 events x 1024 oscillation points (32x32 grid of sin2_th23 x dm2_32, "
-                         "delta_cp per point) in ONE osc_reweight_bin_batch call"),
+                         "delta_cp per point) in ONE osc_reweight_bin_batch call (factorised path k4)"),
+    "config3-k3": dict(n=1_000_000, kernel="reweight_batch_kernel (k3)", bytes_per_unit=25.0 / 1024, flop_per_unit=196.3,
+                       what="configs[3] with OSC_BATCH_PATH=k3: every (event, point) pair gets the full closed form"),
 }
 
 
@@ -241,7 +249,9 @@ def run_other(args):
         et, er, w0, ch = wl.events(n, seed=2)
         d_et, d_er, d_w0, d_ch = (torch.from_numpy(a).to(dev) for a in (et, er, w0, ch))
         d_edges = torch.from_numpy(wl.bin_edges()).to(dev)
-        pts = wl.scan_points()
+        if args.workload == "config3-k3":
+            os.environ["OSC_BATCH_PATH"] = "k3"
+        pts = osc.pack_params(wl.scan_points())                                 # marshalled once (binding only)
         out = torch.empty((len(pts), osc.N_CHANNELS, wl.N_BINS), dtype=torch.float64, device=dev)
         units = n * len(pts)
 
@@ -297,10 +307,98 @@ def run_other(args):
         "clocks": clocks, "e2e": None, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": None}))
 
 
+def run_sweep(args):
+    """configs[4]: size sweep N = 1e3 .. 1e9 on the configs[2] path (k2, one energy scale per launch, Table 1), plus
+    the 12 (rho, L, hierarchy) settings at N = 1e7.  One JSON line; `value` is the rate at the largest N."""
+    import torch
+
+    import paper_1311_7579_b200 as osc
+    from paper_1311_7579_b200 import build as _build
+
+    _build.build_library()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(0)
+    osc.osc_set_device(0)
+    dev = torch.device("cuda", 0)
+    stream = torch.cuda.current_stream()
+    d_edges = torch.from_numpy(wl.bin_edges()).to(dev)
+    hist = torch.zeros((osc.N_CHANNELS, wl.N_BINS), dtype=torch.float64, device=dev)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)       # > L2 (126 MB)
+    hbm_peak, peak_src = peaks()
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    n_max = args.events or 1_000_000_000
+    sizes = [10 ** k for k in range(3, 10) if 10 ** k <= n_max]
+    sampler = ClockSampler(0)
+    t0 = time.time()
+    launches0 = osc.osc_launch_count()
+
+    def time_k2(ev, par, reps):
+        """Mean duration of one k2 launch (ms).  Inputs below the L2 size are evicted before every launch."""
+        osc.osc_set_params(**par)
+        small = ev[0].numel() * BYTES_PER_EVENT < 200e6
+        for _ in range(3):
+            osc.osc_reweight_bin(*ev, 1.0, d_edges, hist_out=hist)
+        total = 0.0
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        if small:
+            for i in range(reps):
+                flush.fill_(i & 1)
+                a.record(stream)
+                osc.osc_reweight_bin(*ev, 1.0, d_edges, hist_out=hist)
+                b.record(stream)
+                torch.cuda.synchronize()
+                total += a.elapsed_time(b)
+            return total / reps
+        a.record(stream)
+        for _ in range(reps):
+            osc.osc_reweight_bin(*ev, 1.0, d_edges, hist_out=hist)
+        b.record(stream)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+
+    rows = []
+    ev = None
+    for n in sizes:
+        ev = wl.events_device(n, seed=4, device=dev)
+        ms = time_k2(ev, wl.table1(), max(3, min(args.steps, 20)))
+        rows.append({"N": n, "ms_per_launch": ms, "events_per_s": n / (ms * 1e-3)})
+        if n == 10_000_000:
+            settings = []
+            for par in wl.sweep_settings():
+                ms_s = time_k2(ev, par, 5)
+                settings.append({"rho": par["rho_g_cm3"], "L": par["L_km"], "hierarchy": par["hierarchy"],
+                                 "events_per_s": n / (ms_s * 1e-3)})
+            rows[-1]["settings"] = settings
+    torch.cuda.synchronize()
+    clocks = sampler.stop(t0, time.time())
+    sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
+    nominal = sm_count * FP64_LANES_PER_SM_CLK * 2 * sm_max * 1e6 / 1e12
+    for r in rows:
+        r["frac_fp64"] = r["events_per_s"] * FLOP_PER_EVENT / 1e12 / nominal
+        r["frac_hbm"] = r["events_per_s"] * BYTES_PER_EVENT / 1e9 / hbm_peak
+    last = rows[-1]
+    print(json.dumps({
+        "metric": METRIC, "value": last["events_per_s"], "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "warmup": 3, "ms_per_step": last["ms_per_launch"], "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic (drawn on the device with torch's generator, seed 4)",
+        "config": {"workload": "configs[4]: size sweep on the configs[2] path (k2, one launch per row), Table 1; "
+                               "rho x L x hierarchy settings at N = 1e7",
+                   "sizes": sizes, "l2": "inputs smaller than L2 are evicted (256 MB fill) before every timed launch"},
+        "clocks": clocks, "e2e": None, "gpu_launches": int(osc.osc_launch_count() - launches0),
+        "roofline": {"bound": "alu", "achieved": last["events_per_s"] * FLOP_PER_EVENT / 1e12, "peak": nominal,
+                     "unit": "TFLOP/s", "frac": last["frac_fp64"], "traffic": None, "kernel": "reweight_bin_kernel (k2)",
+                     "peak_source": "unit counts and clocks.max.sm (DESIGN.md section 6)",
+                     "hbm_peak": hbm_peak, "hbm_peak_source": peak_src},
+        "sweep": rows, "cpu_baseline": None}))
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.workload == "config4":
+        run_sweep(args)
         return
     if args.workload != "config2":
         run_other(args)
@@ -386,6 +484,29 @@ def main():
     torch.cuda.synchronize()
     k_ms = ks.elapsed_time(ke) / reps
 
+    # ---- the same step through the one-pass call (osc_reweight_bin_scales, NEXT-3): reported beside `value` --------
+    def step_fused():
+        osc.osc_set_params(**par)
+        osc.osc_reweight_bin_scales(d_et, d_er, d_w0, d_ch, SCALES, d_edges, hist_out=hist)
+        sharding.allreduce_hist(hist)
+
+    for _ in range(3):
+        step_fused()
+    barrier()
+    fs, fe = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    fs.record(stream)
+    for _ in range(args.steps):
+        step_fused()
+    fe.record(stream)
+    barrier()
+    f_ms = torch.tensor([fs.elapsed_time(fe)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(f_ms, op=dist.ReduceOp.MAX)
+    fused = {"value": world * n * len(SCALES) * args.steps / (float(f_ms.item()) * 1e-3), "unit": UNIT,
+             "ms_per_step": float(f_ms.item()) / args.steps,
+             "api": "osc_reweight_bin_scales: the three energy scales in one pass, closed form once per event; "
+                    "same three histograms as the step behind `value`"}
+
     # ---- fp64 peak probe in the same run (DFMA-only, register resident) ----------------------------------------
     probe_flops = osc.osc_fp64_peak_probe(1 << 14, 4)
     torch.cuda.synchronize()
@@ -463,6 +584,7 @@ def main():
                    "l2": "inputs (250 MB per pass) larger than L2 (126 MB); no explicit flush",
                    "parallelism": f"events sharded over {world} GPU(s); histogram all-reduce" if world > 1 else "1 GPU"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+        "fused_scales": fused,
     }
     print(json.dumps(out))
     if world > 1:

@@ -117,6 +117,24 @@ struct MergeScratch {
 
 constexpr int kGroup = 16; // blocks per first-level merge group
 
+// src[0] + src[stride] + ... (count terms, added in that order), read through L2.  The loads of eight terms are
+// issued together before they are added: the merge is a chain of dependent L2 round trips otherwise, and it sits
+// on the critical path of every call (the last block does it alone).
+__device__ __forceinline__ double ordered_sum_cg(const double* src, int count, int stride)
+{
+    double s = 0.0;
+    int b = 0;
+    for (; b + 8 <= count; b += 8) {
+        double v[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) v[k] = __ldcg(src + (size_t)(b + k) * stride);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) s += v[k];
+    }
+    for (; b < count; ++b) s += __ldcg(src + (size_t)b * stride);
+    return s;
+}
+
 // hist: [n_sub][nh] sub-histograms of this block in shared memory (n_sub = warps * kSlots).
 // Writes the block's sum to ms.partial, then the last block of each group sums the group and the last
 // group sums the groups into out[nh].  Must be called by all threads of the block.
@@ -141,12 +159,8 @@ __device__ __forceinline__ void block_merge(const double* hist, int n_sub, int n
     if (*s_ticket != (unsigned)(gsize - 1)) return;
     if (threadIdx.x == 0) ms.counters[group] = 0u;          // last of the group: nobody else reads it again
     __threadfence();
-    for (int i = threadIdx.x; i < nh; i += blockDim.x) {
-        const double* src = ms.partial + (size_t)gfirst * nh + i;
-        double s = __ldcg(src);
-        for (int b = 1; b < gsize; ++b) s += __ldcg(src + (size_t)b * nh);
-        ms.gpartial[(size_t)group * nh + i] = s;
-    }
+    for (int i = threadIdx.x; i < nh; i += blockDim.x)
+        ms.gpartial[(size_t)group * nh + i] = ordered_sum_cg(ms.partial + (size_t)gfirst * nh + i, gsize, nh);
     __threadfence();
     __syncthreads();
 
@@ -155,11 +169,7 @@ __device__ __forceinline__ void block_merge(const double* hist, int n_sub, int n
     if (*s_ticket != (unsigned)(ms.ngroups - 1)) return;
     if (threadIdx.x == 0) ms.counters[ms.ngroups] = 0u;
     __threadfence();
-    for (int i = threadIdx.x; i < nh; i += blockDim.x) {
-        double s = __ldcg(ms.gpartial + i);
-        for (int g = 1; g < ms.ngroups; ++g) s += __ldcg(ms.gpartial + (size_t)g * nh + i);
-        out[i] = s;
-    }
+    for (int i = threadIdx.x; i < nh; i += blockDim.x) out[i] = ordered_sum_cg(ms.gpartial + i, ms.ngroups, nh);
 }
 
 } // namespace oscb

@@ -650,6 +650,49 @@ def test_config2_full_size(osc):
     assert_hist_close(sub, ref, "config2 strided sample")
 
 
+def test_config3_full_size_sampled_points(osc):
+    """configs[3] at its full size in the launch configuration bench.py times (one factorised call, 1e6 events x
+    1024 points): three points against the oracle on all 1e6 events, every point against invariants."""
+    n = 1_000_000
+    et, er, w0, ch = wl.events(n, seed=2)
+    edges = wl.bin_edges()
+    pts = wl.scan_points()
+    d = [dev(a) for a in (et, er, w0, ch)]
+    got = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, dev(edges)))
+    assert got.shape == (1024, 4, 50)
+    for p in (0, 517, 1023):
+        ref = oracle.reweight_bin(oracle.Params(**pts[p]), et, er, w0, ch, 1.0, edges)
+        assert_hist_close(got[p], ref, f"config3 full size, point {p}")
+    # P(numu -> numu) + P(numu -> nue) <= 1, so channel sums are bounded by the unoscillated histogram of w0;
+    # empty cells are the same for every point
+    op0 = oracle.Params(**wl.table1(L_km=0.0))
+    unosc = oracle.reweight_bin(op0, et, er, w0, ch, 1.0, edges)            # L = 0: P(mu->mu) = 1, P(mu->e) = 0
+    assert np.all(got >= 0.0) and np.all(np.isfinite(got))
+    assert np.all(got[:, 0, :] <= unosc[0] * (1 + 1e-12)) and np.all(got[:, 2, :] <= unosc[2] * (1 + 1e-12))
+    empty = got[0] == 0.0
+    assert np.all((got == 0.0) == empty[None])
+
+
+def test_config4_large_n_properties(osc):
+    """configs[4] beyond what the oracle can redo: 1e8 device-drawn events (2.5 GB).  Additivity over chunks, and
+    the oracle on a 1e6-event chunk of the same arrays copied back to the host."""
+    n = 100_000_000
+    d = wl.events_device(n, seed=4, device=torch.device("cuda", 0))
+    edges = wl.bin_edges()
+    de = dev(edges)
+    op = set_params(osc, wl.table1(rho_g_cm3=5.0, L_km=1300.0, hierarchy=-1))
+    full = host(osc.osc_reweight_bin(*d, 1.0, de))
+    m = 12_500_000 + 2                                        # even: every chunk keeps 16-byte alignment
+    parts = sum(host(osc.osc_reweight_bin(*[t[i:i + m] for t in d], 1.0, de)) for i in range(0, n, m))
+    assert np.max(np.abs(parts - full) / np.maximum(full, 1e-300) * (full > 0)) < 1e-12
+    c = slice(77_000_001, 78_000_001)                         # odd offset: the 8-byte-aligned load path
+    chunk = [host(t[c]) for t in d]
+    got = host(osc.osc_reweight_bin(*[t[c] for t in d], 1.0, de))
+    assert_hist_close(got, oracle.reweight_bin(op, *chunk, 1.0, edges), "config4 chunk of 1e8")
+    again = host(osc.osc_reweight_bin(*d, 1.0, de))
+    assert np.array_equal(full, again)
+
+
 def test_paper_validation_replay(osc):
     """1e7 energies uniform in 0-30 GeV, residuals ~1e-12 in fp64 (A12: floored at 1e-3 GeV)."""
     n = 10_000_000

@@ -151,6 +151,20 @@ int osc_reweight_bin_batch(const osc_params *points, int n_points, const double 
 int osc_neg2lnl(const double *hist, int n_points, int n_cells, const double *data, double norm, double *out,
                 void *stream);
 
+/* Bin-centre reweighting against event-by-event reweighting ("calculate the
+ * effect of the variation at the center of each bin and apply it to the whole bin" versus "retain all of the
+ * simulated events", the comparison behind the paper's 2.6 % example).  Bins are in TRUE energy here:
+ *     hist_event_out[c][b]  = sum over events j of channel c with bin_edges[b] <= E_true[j] < bin_edges[b+1]
+ *                             of w0[j] * P_c(E_true[j])          (= osc_reweight_bin with E_reco := E_true, scale 1)
+ *     hist_centre_out[c][b] = P_c((bin_edges[b] + bin_edges[b+1]) / 2) * sum over the same events of w0[j]
+ * with the parameters of osc_set_params.  The binning bias of a cell is hist_centre / hist_event - 1.
+ *   E_true, w0 DEVICE [n] fp64; channel DEVICE [n] int8; bin_edges DEVICE [n_bins + 1] fp64, strictly increasing
+ *   hist_event_out, hist_centre_out  DEVICE [OSC_N_CHANNELS][n_bins] fp64, OVERWRITTEN
+ * A bin centre that is not a usable energy (<= 0 or non-finite) gives NaN in hist_centre_out. */
+int osc_bin_centre_compare(const double *E_true, const double *w0, const int8_t *channel, size_t n,
+                           const double *bin_edges, int n_bins, double *hist_event_out, double *hist_centre_out,
+                           void *stream);
+
 /* Debug/verification export of the integer binning decision of osc_reweight_bin (row a3c):
  *   bin_out  DEVICE [n] int32: the bin index b of event j, or -1 if the event is dropped. */
 int osc_bin_index(const double *E_true, const double *E_reco, const int8_t *channel, size_t n,

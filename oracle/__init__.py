@@ -77,6 +77,8 @@ def lib() -> ctypes.CDLL:
                                              _dp, ctypes.c_int, _dp]
         _lib.oracle_reweight_bin_batch.argtypes = [P, ctypes.c_int, _dp, _dp, _dp, _i8p, ctypes.c_size_t,
                                                    ctypes.c_double, _dp, ctypes.c_int, _dp]
+        _lib.oracle_bin_centre_compare.argtypes = [P, _dp, _dp, _i8p, ctypes.c_size_t, _dp, ctypes.c_int, _dp, _dp]
+        _lib.oracle_bin_centre_compare.restype = ctypes.c_int
         _lib.oracle_neg2lnl.argtypes = [_dp, ctypes.c_int, ctypes.c_int, _dp, ctypes.c_double, _dp]
         _lib.oracle_neg2lnl.restype = ctypes.c_int
         _lib.oracle_set_threads.argtypes = [ctypes.c_int]
@@ -191,3 +193,16 @@ def neg2lnl(hist, data, norm: float = 1.0) -> np.ndarray:
     _check(lib().oracle_neg2lnl(_ptr(hist), hist.shape[0], data.size, _ptr(data), float(norm), _ptr(out)),
            "oracle_neg2lnl")
     return out
+
+
+def bin_centre_compare(p: Params, E_true, w0, channel, edges):
+    """(hist_event, hist_centre), each [n_channels, n_bins], over TRUE-energy bins."""
+    E_true, w0, edges = _f64(E_true), _f64(w0), _f64(edges)
+    channel = np.ascontiguousarray(channel, dtype=np.int8)
+    nb = edges.size - 1
+    he = np.empty((n_channels(), nb), dtype=np.float64)
+    hc = np.empty_like(he)
+    c = p._c()
+    _check(lib().oracle_bin_centre_compare(ctypes.byref(c), _ptr(E_true), _ptr(w0), _ptr(channel, _i8p), E_true.size,
+                                           _ptr(edges), nb, _ptr(he), _ptr(hc)), "oracle_bin_centre_compare")
+    return he, hc

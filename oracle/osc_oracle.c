@@ -414,6 +414,37 @@ int oracle_neg2lnl(const double *hist, int n_points, int n_cells, const double *
     return 0;
 }
 
+/* Bin-centre reweighting beside event-by-event reweighting over TRUE-energy bins:
+ *   hist_event[c][b]  = sum_j w0_j P_c(E_j)          over the events of channel c with edges[b] <= E_j < edges[b+1]
+ *   hist_centre[c][b] = P_c((edges[b] + edges[b+1]) / 2) * sum_j w0_j   over the same events
+ * Events in index order, long double sums; the bin decision in IEEE double as in oracle_reweight_bin. */
+int oracle_bin_centre_compare(const oracle_params *p, const double *E_true, const double *w0, const int8_t *channel,
+                              size_t n, const double *edges, int n_bins, double *hist_event, double *hist_centre)
+{
+    if (!params_ok(p) || n_bins < 1) return -1;
+    const size_t nh = (size_t)ORACLE_N_CHANNELS * n_bins;
+    real *ev = (real *)calloc(nh, sizeof(real)), *un = (real *)calloc(nh, sizeof(real));
+    if (!ev || !un) { free(ev); free(un); return -2; }
+    for (size_t j = 0; j < n; ++j) {
+        const int c = channel[j];
+        if (c < 0 || c >= ORACLE_N_CHANNELS || !energy_ok(E_true[j])) continue;
+        const int b = bin_of(1.0, E_true[j], edges, n_bins);
+        if (b < 0) continue;
+        ev[(size_t)c * n_bins + b] += (real)w0[j] * prob_one(p, E_true[j], CH_IN[c], CH_OUT[c], CH_ANTI[c]);
+        un[(size_t)c * n_bins + b] += (real)w0[j];
+    }
+    for (int c = 0; c < ORACLE_N_CHANNELS; ++c)
+        for (int b = 0; b < n_bins; ++b) {
+            const double centre = 0.5 * (edges[b] + edges[b + 1]);
+            const size_t i = (size_t)c * n_bins + b;
+            hist_event[i] = (double)ev[i];
+            hist_centre[i] = energy_ok(centre) ? (double)(un[i] * prob_one(p, centre, CH_IN[c], CH_OUT[c], CH_ANTI[c])) : NAN;
+        }
+    free(ev);
+    free(un);
+    return 0;
+}
+
 int oracle_n_channels(void) { return ORACLE_N_CHANNELS; }
 
 #ifdef _OPENMP

@@ -24,7 +24,7 @@ PARAM_FIELDS = ("sin2_th12", "sin2_th23", "sin2_th13", "dm2_32", "dm2_21", "delt
 
 # every symbol include/osc.h declares (tests/test_abi.py checks the header against this list)
 EXPORTS = ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_scales", "osc_reweight_bin_batch",
-           "osc_neg2lnl", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_last_error", "osc_launch_count",
+           "osc_neg2lnl", "osc_bin_centre_compare", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_last_error", "osc_launch_count",
            "osc_version", "osc_set_device", "osc_get_device", "osc_fp64_peak_probe")
 
 
@@ -60,6 +60,7 @@ def lib() -> ctypes.CDLL:
     L.osc_reweight_bin_batch.argtypes = [ctypes.POINTER(osc_params), i, _dp, _dp, _dp, _dp, sz, d, _dp, i, _dp, vp]
     L.osc_bin_index.argtypes = [_dp, _dp, _dp, sz, d, _dp, i, _dp, vp]
     L.osc_neg2lnl.argtypes = [_dp, i, i, _dp, d, _dp, vp]
+    L.osc_bin_centre_compare.argtypes = [_dp, _dp, _dp, sz, _dp, i, _dp, _dp, vp]
     L.osc_prob_host.argtypes = [_dp, sz, i, i, i, _dp]
     L.osc_reweight_bin_host.argtypes = [_dp, _dp, _dp, _dp, sz, d, _dp, i, _dp]
     L.osc_set_device.argtypes = [i]
@@ -67,7 +68,7 @@ def lib() -> ctypes.CDLL:
     L.osc_fp64_peak_probe.argtypes = [i, i, ctypes.POINTER(d), vp]
     for name in ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_scales",
                  "osc_reweight_bin_batch",
-                 "osc_neg2lnl", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_set_device", "osc_get_device",
+                 "osc_neg2lnl", "osc_bin_centre_compare", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_set_device", "osc_get_device",
                  "osc_fp64_peak_probe"):
         getattr(L, name).restype = i
     L.osc_last_error.restype = ctypes.c_char_p
@@ -247,6 +248,20 @@ def osc_neg2lnl(hist, data, norm: float = 1.0, out=None, stream=None):
     _check(lib().osc_neg2lnl(_dev(hist, torch.float64, "hist"), npts, n_cells, _dev(data, torch.float64, "data"),
                              float(norm), _dev(out, torch.float64, "out"), _stream(stream)))
     return out
+
+
+def osc_bin_centre_compare(E_true, w0, channel, bin_edges, stream=None):
+    """(hist_event, hist_centre), each [N_CHANNELS, n_bins], over TRUE-energy bins (include/osc.h)."""
+    import torch
+
+    n, pt, _, pw, pc = _event_ptrs(E_true, E_true, w0, channel)
+    nb = bin_edges.numel() - 1
+    he = torch.empty((N_CHANNELS, nb), dtype=torch.float64, device=E_true.device)
+    hc = torch.empty_like(he)
+    _check(lib().osc_bin_centre_compare(pt, pw, pc, n, _dev(bin_edges, torch.float64, "bin_edges"), nb,
+                                        _dev(he, torch.float64, "hist_event_out"),
+                                        _dev(hc, torch.float64, "hist_centre_out"), _stream(stream)))
+    return he, hc
 
 
 def osc_bin_index(E_true, E_reco, channel, energy_scale: float, bin_edges, bin_out=None, stream=None):

@@ -804,6 +804,56 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
     return post_launch("osc_reweight_bin_batch merge");
 }
 
+int osc_bin_centre_compare(const double* E_true, const double* w0, const int8_t* channel, size_t n,
+                           const double* bin_edges, int n_bins, double* hist_event_out, double* hist_centre_out,
+                           void* stream)
+{
+    int rc = check_bin_args(E_true, E_true, w0, channel, n, 1.0, bin_edges, n_bins, hist_event_out);
+    if (rc) return rc;
+    if (!hist_centre_out) return fail(OSC_ERR_INVALID_ARG, "null hist_centre_out");
+    if (n > 0 && !w0) return fail(OSC_ERR_INVALID_ARG, "null w0 with n > 0");
+    if (!aligned(hist_event_out, 8) || !aligned(hist_centre_out, 8))
+        return fail(OSC_ERR_ALIGNMENT, "histogram not 8-byte aligned");
+    HostSet h;
+    if ((rc = snapshot(h))) return rc;
+    BinArgs args;
+    make_bin_args(h, args);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int nh = kChannels * n_bins;
+    // event by event: the fused kernel with the true energy in the role of the binned energy
+    if ((rc = launch_reweight(args, E_true, E_true, w0, channel, n, 1.0, bin_edges, n_bins, hist_event_out, st))) return rc;
+    // bin centre: unoscillated content of every true-energy bin, times the probability at the centre
+    if (n == 0) {
+        CUDA_TRY(cudaMemsetAsync(hist_centre_out, 0, (size_t)nh * sizeof(double), st));
+    } else {
+        int sms = 0;
+        if ((rc = sm_count(&sms))) return rc;
+        const size_t sub1 = sizeof(double) * (kBlock / 32) * kSlots * (size_t)nh;
+        const int n_sub = bin_table_bytes(n_bins) + 2 * sub1 <= 100 * 1024 ? 2 : 1;
+        const size_t smem = bin_table_bytes(n_bins) + n_sub * sub1;
+        if (smem > kSmemBudget) return fail(OSC_ERR_INVALID_ARG, "n_bins = %d needs more shared memory than one SM has", n_bins);
+        const size_t ntiles = (n + 2 * kBlock - 1) / (2 * (size_t)kBlock);
+        size_t g = (size_t)sms * (smem <= 100 * 1024 ? 2 : 1);
+        if (ntiles < g) g = ntiles;
+        const int grid = (int)g;
+        const int ngroups = (grid + kGroup - 1) / kGroup;
+        const size_t bytes_partial = (size_t)grid * nh * sizeof(double), bytes_gpartial = (size_t)ngroups * nh * sizeof(double);
+        char* scratch = nullptr;
+        if ((rc = stream_scratch(kCounterBytes + bytes_partial + bytes_gpartial, st, &scratch))) return rc;
+        MergeScratch ms;
+        ms.counters = reinterpret_cast<unsigned int*>(scratch);
+        ms.partial = reinterpret_cast<double*>(scratch + kCounterBytes);
+        ms.gpartial = reinterpret_cast<double*>(scratch + kCounterBytes + bytes_partial);
+        ms.ngroups = ngroups;
+        if (smem > 48 * 1024)
+            CUDA_TRY(cudaFuncSetAttribute(unit_hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        unit_hist_kernel<<<grid, kBlock, smem, st>>>(E_true, w0, channel, n, bin_edges, n_bins, n_sub, ms, hist_centre_out);
+        if ((rc = post_launch("osc_bin_centre_compare (unit histogram)"))) return rc;
+    }
+    centre_weight_kernel<<<(nh + 255) / 256, 256, 0, st>>>(args, bin_edges, n_bins, hist_centre_out);
+    return post_launch("osc_bin_centre_compare (centre weights)");
+}
+
 int osc_neg2lnl(const double* hist, int n_points, int n_cells, const double* data, double norm, double* out,
                 void* stream)
 {

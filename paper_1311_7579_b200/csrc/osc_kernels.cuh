@@ -419,6 +419,68 @@ reweight_bin_scales_kernel(const __grid_constant__ BinArgs a, const __grid_const
 }
 
 // ------------------------------------------------------------------------------------------------
+// Bin-centre comparator: the "quick" alternative the paper argues against
+// multiplies the unoscillated content of a TRUE-energy bin by the probability at the bin centre.
+// unit_hist_kernel fills hist[channel][bin] += w0 over true-energy bins (the machinery of k2 without the closed
+// form); centre_weight_kernel multiplies each cell by P_channel(centre of the bin).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kBlock)
+unit_hist_kernel(const double* __restrict__ E_true, const double* __restrict__ w0, const int8_t* __restrict__ channel,
+                 size_t n, const double* __restrict__ edges, int nb, int n_sub, MergeScratch ms,
+                 double* __restrict__ hist_out)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int WARPS = kBlock / 32;
+    const int nh = kChannels * nb;
+    double* hist = reinterpret_cast<double*>(smem_raw + bin_table_bytes(nb));
+    __shared__ unsigned int s_ticket;
+    const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    const int n_hist = WARPS * kSlots * n_sub;
+    for (int i = threadIdx.x; i < n_hist * nh; i += kBlock) hist[i] = 0.0;
+    build_bin_table(smem_raw, edges, nb);
+    const BinView bt = bin_view(smem_raw);
+    const LaneHist lh = lane_hist(hist, nh, n_sub, warp, lane);
+    const size_t ntiles = (n + 2 * kBlock - 1) / (2 * kBlock);
+    for (size_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const size_t j0 = t * (2 * kBlock) + threadIdx.x, j1 = j0 + kBlock;
+        int cell[2];
+        double w[2];
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            const size_t j = k ? j1 : j0;
+            cell[k] = -1;
+            w[k] = 0.0;
+            if (j < n) {
+                const double E = E_true[j];
+                const unsigned ch = (unsigned)(unsigned char)channel[j];
+                const int bin = find_bin<0>(bt, E);                      // true-energy bins: no energy scale
+                if (energy_ok(E) && ch < (unsigned)kChannels && bin >= 0) {
+                    cell[k] = (int)ch * nb + bin;
+                    w[k] = w0[j];
+                }
+            }
+        }
+        warp_hist_add2(lh, cell[0], w[0], cell[1], w[1], lt_mask);
+    }
+    block_merge(hist, n_hist, nh, ms, hist_out, &s_ticket);
+}
+
+// hist[ch][b] *= P_ch((edges[b] + edges[b+1]) / 2); a centre that is not a usable energy gives NaN.
+__global__ void __launch_bounds__(256)
+centre_weight_kernel(const __grid_constant__ BinArgs a, const double* __restrict__ edges, int nb,
+                     double* __restrict__ hist)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= kChannels * nb) return;
+    const int ch = i / nb, b = i - ch * nb;
+    const double c = 0.5 * (edges[b] + edges[b + 1]);
+    const bool ok = energy_ok(c);
+    const double P = prob_one(a.set, a.ch[ch], ok ? c : 1.0);
+    hist[i] = ok ? hist[i] * P : qnan();
+}
+
+// ------------------------------------------------------------------------------------------------
 // k3: batched parameter sets (row a4).  Block (c, g) owns event chunk c and point group g.  The chunk is
 // staged tile by tile in shared memory -- E_true, w0 and the histogram cell of every event, which does
 // not depend on the parameter set and is therefore decided once per tile -- and every staged tile is

@@ -570,6 +570,34 @@ def test_neg2lnl_edge_cases(osc):
 
 
 # ------------------------------------------------------------------------------------------------
+# NEXT-4: bin-centre against event-by-event reweighting over true-energy bins (osc_bin_centre_compare)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,nb", [(0, 5), (1, 1), (777, 13), (300_000, 200)])
+def test_bin_centre_compare(osc, n, nb):
+    et, _, w0, ch = wl.events(max(n, 1), seed=51)
+    et, w0, ch = et[:n].copy(), w0[:n], ch[:n].copy()
+    if n > 10:
+        et[3] = -1.0; ch[4] = 5; et[5] = 99.0
+    edges = wl.bin_edges(nb, 5.0) + 0.05                      # first centre > 0
+    op = set_params(osc, wl.table1(delta_cp=1.3, hierarchy=-1))
+    he, hc = osc.osc_bin_centre_compare(dev(et), dev(w0), dev(ch), dev(edges))
+    re, rc = oracle.bin_centre_compare(op, et, w0, ch, edges)
+    assert_hist_close(host(he), re, f"bin-centre compare, event-by-event n={n}")
+    assert_hist_close(host(hc), rc, f"bin-centre compare, centre n={n}")
+
+
+def test_bin_centre_compare_unusable_centre(osc):
+    et, _, w0, ch = wl.events(1000, seed=52)
+    edges = np.array([-1.0, 1.0, 3.0])                       # first centre is 0: not a usable energy
+    op = set_params(osc, wl.table1())
+    he, hc = osc.osc_bin_centre_compare(dev(et), dev(w0), dev(ch), dev(edges))
+    re, rc = oracle.bin_centre_compare(op, et, w0, ch, edges)
+    assert np.all(np.isnan(host(hc)[:, 0])) and np.all(np.isnan(rc[:, 0]))
+    assert_hist_close(host(hc)[:, 1], rc[:, 1], "centre, usable bin")
+    assert_hist_close(host(he), re, "event-by-event")
+
+
+# ------------------------------------------------------------------------------------------------
 # asynchrony: parameters are captured at enqueue time; work runs on the caller's stream
 # ------------------------------------------------------------------------------------------------
 def test_params_captured_at_enqueue_on_side_stream(osc):

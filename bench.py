@@ -193,9 +193,9 @@ K4_FLOP_PER_UNIT = 17.4       # all kernels of one factorised call, ncu (profile
 # Per-config description of the secondary workloads: (events, units per event per step, bytes per unit, flop per unit)
 #   flop per unit: ncu-counted fp64 operations of the kernel that runs, bytes: algorithmic.
 OTHER = {
-    "config0": dict(n=100_000, kernel="prob_kernel (k1)", bytes_per_unit=16.0, flop_per_unit=200.0,
+    "config0": dict(n=100_000, kernel="prob_kernel (k1)", bytes_per_unit=16.0, flop_per_unit=178.0,
                     what="configs[0]: 1e5 events, Table 1, P(numu->numu) and P(numu->nue) (2 osc_prob calls)"),
-    "config1": dict(n=10_000_000, kernel="prob_all_kernel (k1b)", bytes_per_unit=80.0, flop_per_unit=290.0,
+    "config1": dict(n=10_000_000, kernel="prob_all_kernel (k1b)", bytes_per_unit=80.0, flop_per_unit=241.0,
                     what="configs[1]: 1e7 events, all 9 transitions for nu and nubar (2 osc_prob_all calls = "
                          "18 output arrays), delta_cp drawn per step, both hierarchies alternate"),
     # k4: fp64 operations the factorised path executes per (event, point), all its kernels together, counted by ncu
@@ -204,7 +204,7 @@ OTHER = {
                     bytes_per_unit=25.0 / 1024, flop_per_unit=K4_FLOP_PER_UNIT,
                     what="configs[3]: 1e6 events x 1024 oscillation points (32x32 grid of sin2_th23 x dm2_32, "
                          "delta_cp per point) in ONE osc_reweight_bin_batch call (factorised path k4)"),
-    "config3-k3": dict(n=1_000_000, kernel="reweight_batch_kernel (k3)", bytes_per_unit=25.0 / 1024, flop_per_unit=196.3,
+    "config3-k3": dict(n=1_000_000, kernel="reweight_batch_kernel (k3)", bytes_per_unit=25.0 / 1024, flop_per_unit=203.5,
                        what="configs[3] with OSC_BATCH_PATH=k3: every (event, point) pair gets the full closed form"),
 }
 

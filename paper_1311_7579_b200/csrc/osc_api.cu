@@ -368,10 +368,20 @@ int osc_prob(const double* E_true, size_t n, int flavour_in, int flavour_out, in
     int grid = 1;
     if ((rc = grid_for((npairs + kBlock - 1) / kBlock, &grid))) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (aligned(E_true, 16) && aligned(P_out, 16))
-        prob_kernel<true><<<grid, kBlock, 0, st>>>(a, E_true, n, P_out);
-    else
-        prob_kernel<false><<<grid, kBlock, 0, st>>>(a, E_true, n, P_out);
+    // the element of S that is asked for is known here: 1 (e, e), 2 another diagonal element, 3 off-diagonal
+    const int kind = flavour_in != flavour_out ? 3 : (flavour_in == 0 ? 1 : 2);
+#define OSC_K1(VEC)                                                                       \
+    switch (kind) {                                                                       \
+    case 1: prob_kernel<VEC, 1><<<grid, kBlock, 0, st>>>(a, E_true, n, P_out); break;     \
+    case 2: prob_kernel<VEC, 2><<<grid, kBlock, 0, st>>>(a, E_true, n, P_out); break;     \
+    default: prob_kernel<VEC, 3><<<grid, kBlock, 0, st>>>(a, E_true, n, P_out); break;    \
+    }
+    if (aligned(E_true, 16) && aligned(P_out, 16)) {
+        OSC_K1(true)
+    } else {
+        OSC_K1(false)
+    }
+#undef OSC_K1
     return post_launch("osc_prob");
 }
 

@@ -114,6 +114,65 @@ __device__ __forceinline__ double assemble(const OscEig& e, double A, const OscT
     return fma(Zr, Zr, Zi * Zi);
 }
 
+// The same for a diagonal element (alpha == beta): T and T^2 are Hermitian, so the imaginary parts of the entry
+// vanish and delta = 1.  EE: the element is (e, e), the only one that carries the matter term.
+template <bool EE>
+__device__ __forceinline__ double assemble_diag(const OscEig& e, double A, const OscTrans& tr)
+{
+    const double Tr = EE ? A + tr.Tr0 : tr.Tr0;
+    const double T2r = EE ? fma(A, A + tr.T2r1, tr.T2r0) : fma(A, tr.T2r1, tr.T2r0);
+    const double N0r = e.prod12 + fma(-e.sum12, Tr, T2r);
+    const double N2r = e.prod01 + fma(-e.sum01, Tr, T2r);
+    const double kn = e.kap2 * N2r;
+    const double Zr = fma(-kn, e.s02, e.c1h);
+    const double Zi = fma(kn, e.c02, fma(-e.kap0, N0r, e.s1h));
+    return fma(Zr, Zr, Zi * Zi);
+}
+
+// ... and for the off-diagonal pair (alpha, beta), (beta, alpha) with neither index on (e, e)'s matter term twice:
+// delta = 0, ee = 0, and the two entries of T, T^2 are complex conjugates of each other, so N0, N2 of the second
+// element are the conjugates of the first.  tr describes alpha -> beta; P_ab = P(alpha -> beta), P_ba the reverse.
+__device__ __forceinline__ void assemble_offdiag_pair(const OscEig& e, double A, const OscTrans& tr, double& P_ab,
+                                                      double& P_ba)
+{
+    const double T2r = fma(A, tr.T2r1, tr.T2r0);
+    const double T2i = fma(A, tr.T2i1, tr.T2i0);
+    const double N0r = fma(-e.sum12, tr.Tr0, T2r), N0i = fma(-e.sum12, tr.Ti0, T2i);
+    const double N2r = fma(-e.sum01, tr.Tr0, T2r), N2i = fma(-e.sum01, tr.Ti0, T2i);
+    const double cr = e.c02 * N2r, sr = e.s02 * N2r;
+    const double Wr = fma(-e.s02, N2i, cr), Wi = fma(e.c02, N2i, sr);          // alpha -> beta
+    const double Vr = fma(e.s02, N2i, cr), Vi = fma(-e.c02, N2i, sr);          // beta -> alpha (N2i -> -N2i)
+    const double k0r = e.kap0 * N0r, k0i = e.kap0 * N0i;
+    const double Zr = fma(-e.kap2, Wi, k0i), Zi = fma(e.kap2, Wr, -k0r);
+    const double Yr = fma(-e.kap2, Vi, -k0i), Yi = fma(e.kap2, Vr, -k0r);
+    P_ab = fma(Zr, Zr, Zi * Zi);
+    P_ba = fma(Yr, Yr, Yi * Yi);
+}
+
+// One off-diagonal element alone (delta = 0, ee = 0).
+__device__ __forceinline__ double assemble_offdiag(const OscEig& e, double A, const OscTrans& tr)
+{
+    const double T2r = fma(A, tr.T2r1, tr.T2r0);
+    const double T2i = fma(A, tr.T2i1, tr.T2i0);
+    const double N0r = fma(-e.sum12, tr.Tr0, T2r), N0i = fma(-e.sum12, tr.Ti0, T2i);
+    const double N2r = fma(-e.sum01, tr.Tr0, T2r), N2i = fma(-e.sum01, tr.Ti0, T2i);
+    const double Wr = fma(e.c02, N2r, -(e.s02 * N2i));
+    const double Wi = fma(e.s02, N2r, e.c02 * N2i);
+    const double Zr = fma(e.kap0, N0i, -(e.kap2 * Wi));
+    const double Zi = fma(e.kap2, Wr, -(e.kap0 * N0r));
+    return fma(Zr, Zr, Zi * Zi);
+}
+
+// KIND: 0 any element (run-time delta / ee), 1 diagonal (e, e), 2 diagonal (mu, mu) or (tau, tau), 3 off-diagonal.
+template <int KIND>
+__device__ __forceinline__ double assemble_kind(const OscEig& e, double A, const OscTrans& tr)
+{
+    if (KIND == 1) return assemble_diag<true>(e, A, tr);
+    if (KIND == 2) return assemble_diag<false>(e, A, tr);
+    if (KIND == 3) return assemble_offdiag(e, A, tr);
+    return assemble(e, A, tr);
+}
+
 // A11: usable energy <=> finite and > 0 <=> 0 < bits < 0x7FF0000000000000 (integer pipe).
 __device__ __forceinline__ bool energy_ok(double E)
 {
@@ -121,13 +180,14 @@ __device__ __forceinline__ bool energy_ok(double E)
     return (b - 1ull) < 0x7FEFFFFFFFFFFFFFull;
 }
 
+template <int KIND = 0>
 __device__ __forceinline__ double prob_one(const OscSet& ps, const OscTrans& tr, double E)
 {
     double invE = rcp_pos(E);
     double A = tr.sa * E;
     OscEig e;
     eig_solve(ps, A, invE, e);
-    return assemble(e, A, tr);
+    return assemble_kind<KIND>(e, A, tr);
 }
 
 } // namespace oscb

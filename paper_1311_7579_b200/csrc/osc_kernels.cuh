@@ -32,35 +32,56 @@ __device__ __forceinline__ void st_stream2(double* p, double a, double b)
     __stcs(reinterpret_cast<double2*>(p), make_double2(a, b));
 }
 
+// The same load as ld_stream, pinned where it is written: ptxas is free to sink an ordinary load of a __restrict__
+// array down to its first use, which turns a prefetch issued at the top of a loop body into a load issued at its
+// bottom (seen in k1b: the loop then waits a full memory latency at its head in every iteration).
+__device__ __forceinline__ double ld_stream_pinned(const double* p)
+{
+    double v;
+    asm volatile("ld.global.cs.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
+    return v;
+}
+
 __device__ __forceinline__ double qnan() { return __longlong_as_double(0x7FF8000000000000LL); }
 
 // ------------------------------------------------------------------------------------------------
 // k1: P_out[j] = P(alpha -> beta)(E_true[j]).  VEC: pointers 16-byte aligned -> 128-bit accesses.
+// KIND: which element of S is asked for (assemble_kind): the launch knows it, so the assembly is specialised.
 // ------------------------------------------------------------------------------------------------
-template <bool VEC>
+template <bool VEC, int KIND>
 __global__ void __launch_bounds__(kBlock)
 prob_kernel(const __grid_constant__ ProbArgs a, const double* __restrict__ E_true, size_t n,
             double* __restrict__ P_out)
 {
-    // VEC: slot i holds events (2i, 2i+1); otherwise tile i / kBlock holds events j0 and j0 + kBlock
+    // VEC: slot i holds events (2i, 2i+1); otherwise tile i / kBlock holds events j0 and j0 + kBlock.
+    // The energies of the thread's next slot are loaded before the arithmetic of the current one.
     const size_t nslots = VEC ? (n + 1) / 2 : ((n + 2 * kBlock - 1) / (2 * kBlock)) * kBlock;
     const size_t stride = (size_t)gridDim.x * kBlock;
-    for (size_t i = (size_t)blockIdx.x * kBlock + threadIdx.x; i < nslots; i += stride) {
+    auto load = [&](size_t i, double& E0, double& E1) {
         const size_t j0 = VEC ? 2 * i : (i / kBlock) * (2 * kBlock) + (i % kBlock);
         const size_t j1 = VEC ? j0 + 1 : j0 + kBlock;
-        const bool has1 = j1 < n;
-        double E0, E1;
-        if (VEC && has1) {
-            double2 v = ld_stream2(E_true + j0);
+        if (VEC && j1 < n) {
+            const double2 v = ld_stream2(E_true + j0);
             E0 = v.x;
             E1 = v.y;
         } else {
             E0 = (j0 < n) ? ld_stream(E_true + j0) : 1.0;
-            E1 = has1 ? ld_stream(E_true + j1) : 1.0;
+            E1 = (j1 < n) ? ld_stream(E_true + j1) : 1.0;
         }
+    };
+    size_t i = (size_t)blockIdx.x * kBlock + threadIdx.x;
+    double N0 = 1.0, N1 = 1.0;
+    if (i < nslots) load(i, N0, N1);
+    while (i < nslots) {
+        const size_t j0 = VEC ? 2 * i : (i / kBlock) * (2 * kBlock) + (i % kBlock);
+        const size_t j1 = VEC ? j0 + 1 : j0 + kBlock;
+        const bool has1 = j1 < n;
+        const double E0 = N0, E1 = N1;
+        i += stride;
+        if (i < nslots) load(i, N0, N1);
         const bool ok0 = energy_ok(E0), ok1 = energy_ok(E1);
-        double P0 = prob_one(a.set, a.tr, ok0 ? E0 : 1.0);
-        double P1 = prob_one(a.set, a.tr, ok1 ? E1 : 1.0);
+        double P0 = prob_one<KIND>(a.set, a.tr, ok0 ? E0 : 1.0);
+        double P1 = prob_one<KIND>(a.set, a.tr, ok1 ? E1 : 1.0);
         P0 = ok0 ? P0 : qnan();
         P1 = ok1 ? P1 : qnan();
         if (VEC && has1) {
@@ -83,10 +104,10 @@ __device__ __forceinline__ void prob_nine(const ProbAllArgs& a, double E, bool o
     const double A = a.tr[0].sa * Es;
     OscEig e;
     eig_solve(a.set, A, invE, e);
-    const double p00 = assemble(e, A, a.tr[0]); // e  -> e
-    const double p01 = assemble(e, A, a.tr[1]); // mu -> e   (beta = e,  alpha = mu)
-    const double p10 = assemble(e, A, a.tr[2]); // e  -> mu  (beta = mu, alpha = e)
-    const double p11 = assemble(e, A, a.tr[3]); // mu -> mu
+    const double p00 = assemble_diag<true>(e, A, a.tr[0]);  // e  -> e
+    const double p11 = assemble_diag<false>(e, A, a.tr[3]); // mu -> mu
+    double p01, p10;                                        // p01: mu -> e (beta = e, alpha = mu); p10: e -> mu
+    assemble_offdiag_pair(e, A, a.tr[1], p01, p10);
     const double p20 = fmax((1.0 - p00) - p10, 0.0); // column alpha = e   sums to 1
     const double p21 = fmax((1.0 - p11) - p01, 0.0); // column alpha = mu
     const double p02 = fmax((1.0 - p00) - p01, 0.0); // row beta = e       sums to 1
@@ -108,13 +129,32 @@ __global__ void __launch_bounds__(kBlock)
 prob_all_kernel(const __grid_constant__ ProbAllArgs a, const double* __restrict__ E_true, size_t n,
                 double* __restrict__ P_out)
 {
+    // the energies are loaded two tiles ahead (ncu: 3.3 long-scoreboard stalls per issue without look-ahead, 1.9 with;
+    // ptxas still sinks the loads to the bottom of the body, so the rest of that stall is the store queue: with the
+    // stores removed the kernel takes 135 us per 1e7 events, with them 167 us)
     const size_t ntiles = (n + 2 * kBlock - 1) / (2 * kBlock);
-    for (size_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    auto load = [&](size_t tile, double& E0, double& E1) {
+        E0 = 1.0;
+        E1 = 1.0;
+        if (tile < ntiles) {
+            const size_t j0 = tile * (2 * kBlock) + threadIdx.x, j1 = j0 + kBlock;
+            if (j0 < n) E0 = ld_stream_pinned(E_true + j0);
+            if (j1 < n) E1 = ld_stream_pinned(E_true + j1);
+        }
+    };
+    size_t t = blockIdx.x;
+    double N0, N1, M0, M1;
+    load(t, N0, N1);
+    load(t + gridDim.x, M0, M1);
+    while (t < ntiles) {
         const size_t j0 = t * (2 * kBlock) + threadIdx.x;
         const size_t j1 = j0 + kBlock;
         const bool in0 = j0 < n, in1 = j1 < n;
-        const double E0 = in0 ? ld_stream(E_true + j0) : 1.0;
-        const double E1 = in1 ? ld_stream(E_true + j1) : 1.0;
+        const double E0 = N0, E1 = N1;
+        N0 = M0;
+        N1 = M1;
+        load(t + 2 * (size_t)gridDim.x, M0, M1);
+        t += gridDim.x;
         double P0[9], P1[9];
         prob_nine(a, E0, energy_ok(E0), P0);
         prob_nine(a, E1, energy_ok(E1), P1);

@@ -53,3 +53,31 @@ def sharded_reweight_bin(E_true, E_reco, w0, channel, energy_scale, bin_edges, r
     b, e = shard_bounds(E_true.shape[0], rank, world)
     part = reweight_fn(E_true[b:e], E_reco[b:e], w0[b:e], channel[b:e], energy_scale, bin_edges, hist_out=hist_out)
     return allreduce_hist(part, group)
+
+
+def sharded_scan(points, E_true, E_reco, w0, channel, energy_scale, bin_edges, rank: int, world: int, batch_fn,
+                 group=None):
+    """Parameter scan sharded by POINTS ("for scans, sharding parameter points instead needs no
+    collective (gather only)"): every rank holds all events, runs ``batch_fn`` (``osc_reweight_bin_batch`` of the
+    binding on GPUs) on its contiguous slice of the point list, and the slices are concatenated with one all-gather.
+
+    Slices are cut with ``align=32`` so that the groups of a scan grid (points that differ only in theta23 / delta_cp,
+    32 per dm2_32 value in configs[3]) stay whole on one rank and the factorised kernel keeps its full lanes.
+    Returns the [n_points, 4, n_bins] tensor on every rank.
+    """
+    import torch
+    import torch.distributed as dist
+
+    n_points = len(points)
+    b, e = shard_bounds(n_points, rank, world, align=32)
+    part = batch_fn(points[b:e], E_true, E_reco, w0, channel, energy_scale, bin_edges)
+    if not (dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1):
+        return part
+    # ranks may own different numbers of points and all_gather wants equal shapes: pad to the largest slice
+    sizes = [hi - lo for lo, hi in (shard_bounds(n_points, r, world, align=32) for r in range(world))]
+    tail = tuple(part.shape[1:])
+    padded = torch.zeros((max(sizes),) + tail, dtype=part.dtype, device=part.device)
+    padded[:e - b] = part
+    parts = [torch.empty_like(padded) for _ in range(world)]
+    dist.all_gather(parts, padded, group=group)
+    return torch.cat([q[:m] for q, m in zip(parts, sizes)], dim=0)

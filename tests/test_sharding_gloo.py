@@ -83,3 +83,44 @@ def test_world2_histogram_allreduce(tmp_path):
     assert np.array_equal(h0 == 0.0, ref == 0.0)
     nz = ref != 0.0
     assert np.max(np.abs(h0[nz] - ref[nz]) / ref[nz]) <= 1e-13
+
+
+def _scan_worker(rank: int, world: int, port: int, n: int, out_dir: str):
+    import torch.distributed as dist
+
+    import oracle
+
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        pts = wl.scan_points()[:80]                  # 2.5 groups of 32: the ranks own 64 and 16 points
+        et, er, w0, ch = wl.events(n, seed=3)
+        edges = wl.bin_edges()
+
+        def batch(p, a, b, c, d, s, e):              # stands in for osc_reweight_bin_batch on this rank's device
+            if len(p) == 0:
+                return torch.empty((0, 4, edges.size - 1), dtype=torch.float64)
+            return torch.from_numpy(oracle.reweight_bin_batch([oracle.Params(**q) for q in p], a, b, c, d, s, e))
+
+        h = sharding.sharded_scan(pts, et, er, w0, ch, 1.0, edges, rank, world, batch)
+        np.save(os.path.join(out_dir, f"scan_{rank}.npy"), h.numpy())
+    finally:
+        dist.destroy_process_group()
+
+
+def test_world2_scan_sharded_by_points(tmp_path):
+    import torch.multiprocessing as mp
+
+    import oracle
+
+    n, world = 501, 2
+    mp.spawn(_scan_worker, args=(world, _free_port(), n, str(tmp_path)), nprocs=world, join=True)
+    pts = wl.scan_points()[:80]
+    et, er, w0, ch = wl.events(n, seed=3)
+    ref = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 1.0, wl.bin_edges())
+    h0 = np.load(tmp_path / "scan_0.npy")
+    h1 = np.load(tmp_path / "scan_1.npy")
+    assert h0.shape == (80, 4, 50)
+    assert np.array_equal(h0, h1) and np.array_equal(h0, ref)    # no arithmetic across ranks: bit-identical
+    assert sharding.shard_bounds(80, 0, 2, align=32) == (0, 64) and sharding.shard_bounds(80, 1, 2, align=32) == (64, 80)

@@ -75,15 +75,6 @@ __device__ __forceinline__ double flip_sign_if(double v, int cond_bit31)
     return __hiloint2double(__double2hiint(v) ^ cond_bit31, __double2loint(v));
 }
 
-// max(v, 2^e) for v that is never NaN, decided on the upper word (integer pipe).  hi_floor is the upper
-// word of the power of two; values below it (including zero, denormals and negatives) are replaced.
-__device__ __forceinline__ double floor_at_pow2(double v, int hi_floor)
-{
-    const int hi = __double2hiint(v);
-    const bool small = hi < hi_floor;
-    return __hiloint2double(small ? hi_floor : hi, small ? 0 : __double2loint(v));
-}
-
 // v raised to at least 2^e by one integer max on the upper word (hi_floor = upper word of 2^e): zero, denormals,
 // negatives and anything else below 2^e come out in [2^e, 2^(e+1)) -- the low word is kept, the result is only used
 // where "some positive number of that size" is all that matters.  v must not be NaN.

@@ -32,7 +32,7 @@ def declared_symbols():
 
 def test_header_symbols_are_exported(L):
     names = declared_symbols()
-    assert len(names) >= 14
+    assert len(names) >= 17
     for name in names:
         assert hasattr(L, name), f"{name} declared in include/osc.h but not exported"
     assert set(names) == set(binding.EXPORTS)
@@ -110,6 +110,29 @@ def test_host_checkable_faults(L):
     assert L.osc_reweight_bin_batch(pts, -1, 16, 16, 16, 16, 3, 1.0, 16, 4, 16, None) == INVALID
     assert L.osc_get_device(None) == INVALID
     assert L.osc_fp64_peak_probe(0, 4, None, None) == INVALID
+    # several energy scales in one pass: count, null list, a bad scale in the list
+    sc = (ctypes.c_double * 4)(0.97, 1.0, 1.03, 1.06)
+    assert L.osc_reweight_bin_scales(None, None, None, None, 0, sc, 0, 8, 4, 8, None) == INVALID
+    assert L.osc_reweight_bin_scales(None, None, None, None, 0, sc, 5, 8, 4, 8, None) == INVALID
+    assert L.osc_reweight_bin_scales(None, None, None, None, 0, None, 3, 8, 4, 8, None) == INVALID
+    sc[1] = -1.0
+    assert L.osc_reweight_bin_scales(None, None, None, None, 0, sc, 3, 8, 4, 8, None) == INVALID
+    sc[1] = 1.0
+    assert L.osc_reweight_bin_scales(None, None, None, None, 3, sc, 3, 8, 4, 8, None) == INVALID   # null events, n > 0
+    assert L.osc_reweight_bin_scales(16, 16, 16, 16, 3, sc, 3, 12, 4, 8, None) == ALIGN
+    # likelihood: sizes, normalisation, null pointers; no points is a no-op
+    assert L.osc_neg2lnl(8, 4, 0, 8, 1.0, 8, None) == INVALID
+    assert L.osc_neg2lnl(8, -1, 10, 8, 1.0, 8, None) == INVALID
+    assert L.osc_neg2lnl(8, 4, 10, 8, 0.0, 8, None) == INVALID
+    assert L.osc_neg2lnl(8, 4, 10, 8, float("inf"), 8, None) == INVALID
+    assert L.osc_neg2lnl(None, 4, 10, 8, 1.0, 8, None) == INVALID
+    assert L.osc_neg2lnl(12, 4, 10, 8, 1.0, 8, None) == ALIGN
+    assert L.osc_neg2lnl(None, 0, 10, None, 1.0, None, None) == OK
+    # bin-centre comparator
+    assert L.osc_bin_centre_compare(None, None, None, 0, 8, 0, 8, 8, None) == INVALID          # n_bins < 1
+    assert L.osc_bin_centre_compare(None, None, None, 0, 8, 4, 8, None, None) == INVALID       # null second output
+    assert L.osc_bin_centre_compare(None, None, None, 3, 8, 4, 8, 8, None) == INVALID          # null events, n > 0
+    assert L.osc_bin_centre_compare(16, 16, 16, 3, 8, 4, 12, 8, None) == ALIGN
 
 
 def test_missing_library_fails_loudly(monkeypatch, tmp_path):

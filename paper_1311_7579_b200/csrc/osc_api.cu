@@ -464,7 +464,16 @@ struct PinnedRing {
         return OSC_OK;
     }
 };
-PinnedRing g_ring;
+PinnedRing g_rings[64];        // one per device: an event belongs to the device it was created on
+
+int ring_for_device(PinnedRing** out)
+{
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return fail(OSC_ERR_CUDA, "device index %d out of range", dev);
+    *out = &g_rings[dev];
+    return OSC_OK;
+}
 
 } // namespace
 
@@ -653,12 +662,14 @@ int launch_batch_scan(const ScanPlan& plan, int n_points, const double* E_true, 
     ScanSub* d_subs = reinterpret_cast<ScanSub*>(q); q += b_subs;
     double* partial = reinterpret_cast<double*>(q);
     // groups and sub-groups are contiguous on the device: one asynchronous copy from a pinned staging slot
+    PinnedRing* ring = nullptr;
+    if ((rc = ring_for_device(&ring))) return rc;
     PinnedRing::Slot* slot = nullptr;
-    if ((rc = g_ring.acquire(b_groups + b_subs, &slot))) return rc;
+    if ((rc = ring->acquire(b_groups + b_subs, &slot))) return rc;
     std::memcpy(slot->host, plan.groups.data(), plan.groups.size() * sizeof(ScanGroup));
     std::memcpy(static_cast<char*>(slot->host) + b_groups, plan.subs.data(), plan.subs.size() * sizeof(ScanSub));
     CUDA_TRY(cudaMemcpyAsync(d_groups, slot->host, b_groups + b_subs, cudaMemcpyHostToDevice, st));
-    if ((rc = g_ring.fence(slot, st))) return rc;
+    if ((rc = ring->fence(slot, st))) return rc;
 
     const unsigned sort_blocks = (geo.nranges + kScanWarps - 1) / kScanWarps;
     const size_t smem_cnt = sizeof(unsigned int) * kScanWarps * (size_t)geo.ncells;
@@ -800,11 +811,13 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
     double* d_points = reinterpret_cast<double*>(sc.p);
     double* partial = reinterpret_cast<double*>(sc.p + bytes_points);
     // asynchronous upload from a pinned staging slot (PinnedRing)
+    PinnedRing* ring = nullptr;
+    if ((rc = ring_for_device(&ring))) return rc;
     PinnedRing::Slot* slot = nullptr;
-    if ((rc = g_ring.acquire((size_t)n_points * sizeof(BinArgs), &slot))) return rc;
+    if ((rc = ring->acquire((size_t)n_points * sizeof(BinArgs), &slot))) return rc;
     std::memcpy(slot->host, blocks.data(), (size_t)n_points * sizeof(BinArgs));
     CUDA_TRY(cudaMemcpyAsync(d_points, slot->host, (size_t)n_points * sizeof(BinArgs), cudaMemcpyHostToDevice, st));
-    if ((rc = g_ring.fence(slot, st))) return rc;
+    if ((rc = ring->fence(slot, st))) return rc;
     const dim3 grid((unsigned)nchunks, (unsigned)ngroups);
     CUDA_TRY(cudaFuncSetAttribute(reweight_batch_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     reweight_batch_kernel<512><<<grid, 512, smem, st>>>(d_points, n_points, E_true, E_reco, w0, channel, n, geo,

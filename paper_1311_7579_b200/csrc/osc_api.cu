@@ -622,15 +622,18 @@ void build_scan_plan(const osc_params* points, int n_points, ScanPlan& plan)
     }
 }
 
-int launch_batch_scan(const ScanPlan& plan, int n_points, const double* E_true, const double* E_reco, const double* w0,
-                      const int8_t* channel, size_t n, double energy_scale, const double* bin_edges, int n_bins,
-                      double* hist_out, cudaStream_t st)
+// The sorted-event paths of the batched call: k4 (plan != nullptr: sub-groups of a scan grid) or k5 (full != nullptr:
+// one parameter block per point, every point its own eigen-problem).  Both sort the events by histogram cell, let
+// one warp own a piece of a cell, write partial[piece][point] and merge the pieces of every cell in order.
+int launch_batch_scan(const ScanPlan* plan, const std::vector<BinArgs>* full, int n_points, const double* E_true,
+                      const double* E_reco, const double* w0, const int8_t* channel, size_t n, double energy_scale,
+                      const double* bin_edges, int n_bins, double* hist_out, cudaStream_t st)
 {
     int rc;
     if (n >= 0xFFFFFFFFull - 64) return fail(OSC_ERR_INVALID_ARG, "osc_reweight_bin_batch: n = %zu is more than one call takes", n);
     ScanGeom geo;
     geo.ncells = kChannels * n_bins;
-    geo.nsubs = (int)plan.subs.size();
+    geo.nsubs = plan ? (int)plan->subs.size() : n_points;      // items a warp walks per piece: sub-groups or points
     geo.range = round_up(std::max<size_t>(1024, (n + 4095) / 4096), 32);
     geo.nranges = (unsigned)((n + geo.range - 1) / geo.range);
     int slots = geo.nsubs < 8 ? geo.nsubs : 8;
@@ -638,7 +641,7 @@ int launch_batch_scan(const ScanPlan& plan, int n_points, const double* E_true, 
     slots = (geo.nsubs + geo.subs_per_slot - 1) / geo.subs_per_slot;
     size_t piece = round_up(n * (size_t)slots / 16384 + 1, 64);
     if (piece < 128) piece = 128;
-    if (piece > 8192) piece = 8192;
+    if (piece > (plan ? 8192u : 512u)) piece = plan ? 8192 : 512;   // k5 stages the piece in shared memory
     geo.piece = (unsigned)piece;
     geo.max_units = (unsigned)(n / piece + (size_t)geo.ncells + 1);
 
@@ -646,8 +649,9 @@ int launch_batch_scan(const ScanPlan& plan, int n_points, const double* E_true, 
     const size_t b_count = round_up((size_t)geo.ncells * geo.nranges * sizeof(unsigned int), 256);
     const size_t b_cells = round_up((size_t)(geo.ncells + 1) * sizeof(unsigned int), 256);
     const size_t b_sorted = round_up(n * sizeof(double), 256);
-    const size_t b_groups = round_up(plan.groups.size() * sizeof(ScanGroup), 256);
-    const size_t b_subs = round_up(plan.subs.size() * sizeof(ScanSub), 256);
+    const size_t b_groups = plan ? round_up(plan->groups.size() * sizeof(ScanGroup), 256)
+                                 : round_up((size_t)n_points * sizeof(BinArgs), 256);
+    const size_t b_subs = plan ? round_up(plan->subs.size() * sizeof(ScanSub), 256) : 0;
     const size_t b_partial = round_up((size_t)geo.max_units * n_points * sizeof(double), 256);
     Scratch sc;
     if ((rc = sc.alloc(b_cellid + b_count + 2 * b_cells + 2 * b_sorted + b_groups + b_subs + b_partial, st))) return rc;
@@ -666,8 +670,12 @@ int launch_batch_scan(const ScanPlan& plan, int n_points, const double* E_true, 
     if ((rc = ring_for_device(&ring))) return rc;
     PinnedRing::Slot* slot = nullptr;
     if ((rc = ring->acquire(b_groups + b_subs, &slot))) return rc;
-    std::memcpy(slot->host, plan.groups.data(), plan.groups.size() * sizeof(ScanGroup));
-    std::memcpy(static_cast<char*>(slot->host) + b_groups, plan.subs.data(), plan.subs.size() * sizeof(ScanSub));
+    if (plan) {
+        std::memcpy(slot->host, plan->groups.data(), plan->groups.size() * sizeof(ScanGroup));
+        std::memcpy(static_cast<char*>(slot->host) + b_groups, plan->subs.data(), plan->subs.size() * sizeof(ScanSub));
+    } else {
+        std::memcpy(slot->host, full->data(), (size_t)n_points * sizeof(BinArgs));
+    }
     CUDA_TRY(cudaMemcpyAsync(d_groups, slot->host, b_groups + b_subs, cudaMemcpyHostToDevice, st));
     if ((rc = ring->fence(slot, st))) return rc;
 
@@ -689,9 +697,23 @@ int launch_batch_scan(const ScanPlan& plan, int n_points, const double* E_true, 
                                                                         sEt, sW);
     if ((rc = post_launch("osc_reweight_bin_batch (sort: scatter)"))) return rc;
     const dim3 grid((geo.max_units + kScanWarps - 1) / kScanWarps, (unsigned)slots);
-    scan_main_kernel<<<grid, 32 * kScanWarps, 0, st>>>(d_groups, d_subs, sEt, sW, cell_begin, unit_begin, geo, n_bins,
-                                                       n_points, partial);
-    if ((rc = post_launch("osc_reweight_bin_batch (scan)"))) return rc;
+    if (plan) {
+        scan_main_kernel<<<grid, 32 * kScanWarps, 0, st>>>(d_groups, d_subs, sEt, sW, cell_begin, unit_begin, geo, n_bins,
+                                                           n_points, partial);
+        if ((rc = post_launch("osc_reweight_bin_batch (scan, factorised)"))) return rc;
+    } else {
+        ChannelKinds kinds;
+        for (int c = 0; c < kChannels; ++c) {
+            int fin, fout, anti;
+            channel_def(c, fin, fout, anti);
+            kinds.k[c] = fin != fout ? 3 : (fin == 0 ? 1 : 2);
+        }
+        const size_t smem_ev = sizeof(double) * kScanWarps * 3 * (size_t)geo.piece;      // <= 48 kB at piece = 512
+        scan_full_kernel<<<grid, 32 * kScanWarps, smem_ev, st>>>(reinterpret_cast<const double*>(d_groups), n_points,
+                                                                 geo.subs_per_slot, kinds, sEt, sW, cell_begin,
+                                                                 unit_begin, geo, n_bins, partial);
+        if ((rc = post_launch("osc_reweight_bin_batch (scan, one eigen-problem per point)"))) return rc;
+    }
     scan_merge_kernel<<<geo.ncells, 256, 0, st>>>(partial, unit_begin, geo.ncells, n_points, hist_out);
     return post_launch("osc_reweight_bin_batch (merge)");
 }
@@ -755,10 +777,12 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
         ScanPlan plan;
         build_scan_plan(points, n_points, plan);
         bool use_scan = (size_t)n_points >= 8 * plan.subs.size();
-        if (const char* e = getenv("OSC_BATCH_PATH")) use_scan = (std::strcmp(e, "k4") == 0) || (use_scan && std::strcmp(e, "k3") != 0);
+        const char* e = getenv("OSC_BATCH_PATH");
+        if (e && !std::strcmp(e, "k4")) use_scan = true;
+        if (e && (!std::strcmp(e, "k3") || !std::strcmp(e, "k5"))) use_scan = false;
         if (use_scan)
-            return launch_batch_scan(plan, n_points, E_true, E_reco, w0, channel, n, energy_scale, bin_edges, n_bins,
-                                     hist_out, st);
+            return launch_batch_scan(&plan, nullptr, n_points, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
+                                     n_bins, hist_out, st);
     }
     // a1 for every point (host), packed as BinArgs
     std::vector<BinArgs> blocks((size_t)n_points);
@@ -766,6 +790,17 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
         HostSet h;
         precompute(points[p], h);
         make_bin_args(h, blocks[(size_t)p]);
+    }
+    // Point lists without scan structure: from 8 points on the sort of the events pays for itself (kernel k5 on
+    // the sorted events); below that the events are taken in their own order (kernel k3).
+    {
+        bool use_full = n_points >= 8;
+        const char* e = getenv("OSC_BATCH_PATH");
+        if (e && !std::strcmp(e, "k5")) use_full = true;
+        if (e && !std::strcmp(e, "k3")) use_full = false;
+        if (use_full)
+            return launch_batch_scan(nullptr, &blocks, n_points, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
+                                     n_bins, hist_out, st);
     }
     int sms = 0;
     if ((rc = sm_count(&sms))) return rc;

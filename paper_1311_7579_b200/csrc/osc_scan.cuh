@@ -415,6 +415,110 @@ scan_main_kernel(const ScanGroup* __restrict__ groups, const ScanSub* __restrict
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// k5: the batched call for point lists WITHOUT scan structure (every point its own eigen-problem, e.g. a batch of
+// Markov-chain proposals), on the sorted events of k4.  Warp (blockIdx.x * kScanWarps + warp) owns one piece of one
+// sorted cell and stages its events (E_true, 1/E_true, w0) in shared memory once; blockIdx.y selects the slot of
+// points it walks.  Lane = event throughout.  What the sort buys over k3:
+//   * every event of the piece has the same histogram cell: the weights are summed in a register and reduced over
+//     the warp once per (piece, point) -- no bin search, no MATCH, no shared-memory histogram in the point loop;
+//   * every event of the piece has the same channel: the transition block is loaded once per (piece, point) and the
+//     amplitude assembly is the one specialised for the kind of element (assemble_kind), chosen by a uniform branch;
+//   * 1/E is taken once per event, not once per event and point.
+// partial[piece][point] and scan_merge are those of k4.  kinds[c] is the element kind of channel c (osc_core.cuh).
+// Shared memory (dynamic): ev[kScanWarps][3][piece]
+// ------------------------------------------------------------------------------------------------
+struct ChannelKinds {
+    int k[kChannels];
+};
+
+template <int KIND>
+__device__ __forceinline__ double full_piece_sum(const OscSet& set, const OscTrans& tr, const double* sE,
+                                                 const double* sI, const double* sW, int len, unsigned lane)
+{
+    double acc0 = 0.0, acc1 = 0.0;
+    for (int i = lane; i < len; i += 64) {
+        const int i1 = i + 32;
+        const bool has1 = i1 < len;
+        const double E0 = sE[i], E1 = has1 ? sE[i1] : 1.0;
+        const double I0 = sI[i], I1 = has1 ? sI[i1] : 1.0;
+        const double w0v = sW[i], w1v = has1 ? sW[i1] : 0.0;
+        const double A0 = tr.sa * E0, A1 = tr.sa * E1;
+        OscEig e0, e1;
+        eig_solve(set, A0, I0, e0);
+        eig_solve(set, A1, I1, e1);
+        acc0 = fma(w0v, assemble_kind<KIND>(e0, A0, tr), acc0);
+        acc1 = fma(w1v, assemble_kind<KIND>(e1, A1, tr), acc1);
+    }
+    double s = acc0 + acc1;
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+    return s;
+}
+
+__global__ void __launch_bounds__(32 * kScanWarps)
+scan_full_kernel(const double* __restrict__ points, int npoints, int pts_per_slot, const ChannelKinds kinds,
+                 const double* __restrict__ sEt, const double* __restrict__ sW,
+                 const unsigned int* __restrict__ cell_begin, const unsigned int* __restrict__ unit_begin, ScanGeom geo,
+                 int nb, double* __restrict__ partial)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const unsigned u = blockIdx.x * kScanWarps + warp;
+    if (u >= __ldg(unit_begin + geo.ncells)) return;
+    int lo = 0, hi = geo.ncells - 1;                         // cell of piece u, as in scan_main_kernel
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (__ldg(unit_begin + mid) <= u) lo = mid; else hi = mid - 1;
+    }
+    const int cell = lo;
+    const unsigned cb = __ldg(cell_begin + cell), ce = __ldg(cell_begin + cell + 1);
+    const unsigned begin = cb + (u - __ldg(unit_begin + cell)) * geo.piece;
+    const int len = (int)(min(ce, begin + geo.piece) - begin);
+    const int ch = cell / nb;
+
+    double* sE = reinterpret_cast<double*>(smem_raw) + (size_t)warp * 3 * geo.piece;
+    double* sI = sE + geo.piece;
+    double* sWt = sI + geo.piece;
+    for (int i = lane; i < len; i += 32) {
+        const double E = __ldg(sEt + begin + i);
+        sE[i] = E;
+        sI[i] = rcp_pos(E);
+        sWt[i] = __ldg(sW + begin + i);
+    }
+    __syncwarp();
+
+    const int p_begin = blockIdx.y * pts_per_slot, p_end = min(npoints, p_begin + pts_per_slot);
+    const int kind = kinds.k[ch];
+    for (int p = p_begin; p < p_end; ++p) {
+        const double* pb = points + (size_t)p * kBinArgsDoubles;
+        OscSet set;
+        set.xq23 = __ldg(pb + 0);
+        set.tr = __ldg(pb + 1);
+        set.dd = __ldg(pb + 2);
+        set.k1 = __ldg(pb + 3);
+        set.k0_27 = __ldg(pb + 4);
+        const double* tb = pb + 6 + ch * kTransDoubles;
+        OscTrans tr;
+        tr.sa = __ldg(tb + 0);
+        tr.delta = __ldg(tb + 1);
+        tr.ee = __ldg(tb + 2);
+        tr.Tr0 = __ldg(tb + 3);
+        tr.Ti0 = __ldg(tb + 4);
+        tr.T2r0 = __ldg(tb + 5);
+        tr.T2i0 = __ldg(tb + 6);
+        tr.T2r1 = __ldg(tb + 7);
+        tr.T2i1 = __ldg(tb + 8);
+        tr.pad = 0.0;
+        double s;
+        if (kind == 2) s = full_piece_sum<2>(set, tr, sE, sI, sWt, len, lane);
+        else if (kind == 3) s = full_piece_sum<3>(set, tr, sE, sI, sWt, len, lane);
+        else if (kind == 1) s = full_piece_sum<1>(set, tr, sE, sI, sWt, len, lane);
+        else s = full_piece_sum<0>(set, tr, sE, sI, sWt, len, lane);
+        if (lane == 0) partial[(size_t)u * npoints + p] = s;
+    }
+}
+
 // out[p][cell] = sum over the pieces of the cell, in order, of partial[piece][p]; 0 for an empty cell.
 __global__ void __launch_bounds__(256)
 scan_merge_kernel(const double* __restrict__ partial, const unsigned int* __restrict__ unit_begin, int ncells,

@@ -435,9 +435,12 @@ def test_k4_ragged_groups_vs_oracle(osc):
         got4 = host(osc.osc_reweight_bin_batch(pts, *d, 1.03, dev(edges)))
     with batch_path("k3"):
         got3 = host(osc.osc_reweight_bin_batch(pts, *d, 1.03, dev(edges)))
+    with batch_path("k5"):
+        got5 = host(osc.osc_reweight_bin_batch(pts, *d, 1.03, dev(edges)))
     assert_hist_close(got4, ref, "k4 ragged groups")
     assert_hist_close(got3, ref, "k3 ragged groups")
-    assert np.array_equal(got4 == 0.0, got3 == 0.0)
+    assert_hist_close(got5, ref, "k5 ragged groups")
+    assert np.array_equal(got4 == 0.0, got3 == 0.0) and np.array_equal(got5 == 0.0, got3 == 0.0)
 
 
 def test_k4_equals_k3_on_the_grid_with_more_events(osc):
@@ -452,17 +455,23 @@ def test_k4_equals_k3_on_the_grid_with_more_events(osc):
         b = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, de))
     with batch_path("k3"):
         c = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, de))
+    with batch_path("k5"):
+        e = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, de))
+        f = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, de))
     assert np.array_equal(a, b), "k4 is not bit-reproducible"
+    assert np.array_equal(e, f), "k5 is not bit-reproducible"
     assert_hist_close(a, c, "k4 vs k3")
+    assert_hist_close(e, c, "k5 vs k3")
     # the oracle on a sample of points (full 200k events each)
     pick = [0, 37, 95]
     ref = oracle.reweight_bin_batch([oracle.Params(**pts[i]) for i in pick], et, er, w0, ch, 1.0, edges)
     assert_hist_close(a[pick], ref, "k4 vs oracle")
 
 
+@pytest.mark.parametrize("path", ["k4", "k5"])
 @pytest.mark.parametrize("n", [0, 1, 31, 64, 65, 129, 1000])
 @pytest.mark.parametrize("nb,kind", [(1, "uniform"), (7, "random"), (50, "uniform")])
-def test_k4_small_and_ragged_sizes(osc, n, nb, kind):
+def test_k4_small_and_ragged_sizes(osc, n, nb, kind, path):
     rng = np.random.default_rng(100 + n + nb)
     if kind == "uniform":
         edges = wl.bin_edges(nb, 5.0)
@@ -471,11 +480,11 @@ def test_k4_small_and_ragged_sizes(osc, n, nb, kind):
     pts = [wl.table1(sin2_th23=0.3 + 0.05 * k, delta_cp=-3.0 + 0.7 * k) for k in range(9)]
     et, er, w0, ch = wl.events(max(n, 1), seed=24)
     et, er, w0, ch = et[:n], er[:n], w0[:n], ch[:n]
-    with batch_path("k4"):
+    with batch_path(path):
         got = host(osc.osc_reweight_bin_batch(pts, dev(et), dev(er), dev(w0), dev(ch), 0.97, dev(edges)))
     ref = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 0.97, edges)
     assert got.shape == (9, 4, nb)
-    assert_hist_close(got, ref, f"k4 n={n} nb={nb}")
+    assert_hist_close(got, ref, f"{path} n={n} nb={nb}")
 
 
 def test_k4_all_events_dropped(osc):

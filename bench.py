@@ -57,10 +57,10 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--workload", default="config2", choices=["config0", "config1", "config2", "config3", "config3-k3",
-                                                               "config4"],
+                                                               "config3-k5", "config4"],
                     help="config2 (default) is the bench line; the others time the remaining BASELINE.json configs "
                          "for BASELINE.md section 4 and give ncu a committed command for k1 / k1b / k3 / k4 "
-                         "(config3-k3 forces the unfactorised batched kernel; config4 is the size sweep)")
+                         "(config3-k3 / config3-k5 force the unfactorised batched kernels; config4 is the size sweep)")
     return ap.parse_args()
 
 
@@ -189,6 +189,7 @@ def run_reference(args):
     }))
 
 
+K5_FLOP_PER_UNIT = 175.6      # all kernels of one k5 call, ncu (profiles/r1_k5.md)
 K4_FLOP_PER_UNIT = 17.4       # all kernels of one factorised call, ncu (profiles/r1_launches_k4.md)
 # Per-config description of the secondary workloads: (events, units per event per step, bytes per unit, flop per unit)
 #   flop per unit: ncu-counted fp64 operations of the kernel that runs, bytes: algorithmic.
@@ -204,6 +205,10 @@ OTHER = {
                     bytes_per_unit=25.0 / 1024, flop_per_unit=K4_FLOP_PER_UNIT,
                     what="configs[3]: 1e6 events x 1024 oscillation points (32x32 grid of sin2_th23 x dm2_32, "
                          "delta_cp per point) in ONE osc_reweight_bin_batch call (factorised path k4)"),
+    "config3-k5": dict(n=1_000_000, kernel="scan_full_kernel + sort/merge kernels (k5)", bytes_per_unit=25.0 / 1024,
+                       flop_per_unit=K5_FLOP_PER_UNIT,
+                       what="configs[3] with OSC_BATCH_PATH=k5: every (event, point) pair gets the full closed form, on "
+                            "events sorted by histogram cell (the path of point lists without scan structure)"),
     "config3-k3": dict(n=1_000_000, kernel="reweight_batch_kernel (k3)", bytes_per_unit=25.0 / 1024, flop_per_unit=203.5,
                        what="configs[3] with OSC_BATCH_PATH=k3: every (event, point) pair gets the full closed form"),
 }
@@ -249,8 +254,8 @@ def run_other(args):
         et, er, w0, ch = wl.events(n, seed=2)
         d_et, d_er, d_w0, d_ch = (torch.from_numpy(a).to(dev) for a in (et, er, w0, ch))
         d_edges = torch.from_numpy(wl.bin_edges()).to(dev)
-        if args.workload == "config3-k3":
-            os.environ["OSC_BATCH_PATH"] = "k3"
+        if args.workload in ("config3-k3", "config3-k5"):
+            os.environ["OSC_BATCH_PATH"] = args.workload[-2:]
         pts = osc.pack_params(wl.scan_points())                                 # marshalled once (binding only)
         out = torch.empty((len(pts), osc.N_CHANNELS, wl.N_BINS), dtype=torch.float64, device=dev)
         units = n * len(pts)

@@ -432,31 +432,42 @@ struct ChannelKinds {
     int k[kChannels];
 };
 
+// Sum of w0 P over the events of the staged piece for one point; lane = event, kFullUnroll events per lane and step
+// (independent dependency chains: the kernel runs few warps per SM, so the instruction-level parallelism has to come
+// from inside the warp); padding slots carry E = 1, w0 = 0.  Fixed summation order: deterministic.
+constexpr int kFullUnroll = 4;
+
 template <int KIND>
 __device__ __forceinline__ double full_piece_sum(const OscSet& set, const OscTrans& tr, const double* sE,
                                                  const double* sI, const double* sW, int len, unsigned lane)
 {
-    double acc0 = 0.0, acc1 = 0.0;
-    for (int i = lane; i < len; i += 64) {
-        const int i1 = i + 32;
-        const bool has1 = i1 < len;
-        const double E0 = sE[i], E1 = has1 ? sE[i1] : 1.0;
-        const double I0 = sI[i], I1 = has1 ? sI[i1] : 1.0;
-        const double w0v = sW[i], w1v = has1 ? sW[i1] : 0.0;
-        const double A0 = tr.sa * E0, A1 = tr.sa * E1;
-        OscEig e0, e1;
-        eig_solve(set, A0, I0, e0);
-        eig_solve(set, A1, I1, e1);
-        acc0 = fma(w0v, assemble_kind<KIND>(e0, A0, tr), acc0);
-        acc1 = fma(w1v, assemble_kind<KIND>(e1, A1, tr), acc1);
+    double acc[kFullUnroll];
+#pragma unroll
+    for (int k = 0; k < kFullUnroll; ++k) acc[k] = 0.0;
+    for (int i = lane; i < len; i += 32 * kFullUnroll) {
+        double E[kFullUnroll], I[kFullUnroll], w[kFullUnroll], A[kFullUnroll];
+        OscEig e[kFullUnroll];
+#pragma unroll
+        for (int k = 0; k < kFullUnroll; ++k) {
+            const int j = i + 32 * k;
+            const bool has = j < len;
+            E[k] = has ? sE[j] : 1.0;
+            I[k] = has ? sI[j] : 1.0;
+            w[k] = has ? sW[j] : 0.0;
+            A[k] = tr.sa * E[k];
+        }
+#pragma unroll
+        for (int k = 0; k < kFullUnroll; ++k) eig_solve(set, A[k], I[k], e[k]);
+#pragma unroll
+        for (int k = 0; k < kFullUnroll; ++k) acc[k] = fma(w[k], assemble_kind<KIND>(e[k], A[k], tr), acc[k]);
     }
-    double s = acc0 + acc1;
+    double s = (acc[0] + acc[1]) + (acc[2] + acc[3]);
 #pragma unroll
     for (int d = 16; d >= 1; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
     return s;
 }
 
-__global__ void __launch_bounds__(32 * kScanWarps)
+__global__ void __launch_bounds__(32 * kScanWarps, 3)
 scan_full_kernel(const double* __restrict__ points, int npoints, int pts_per_slot, const ChannelKinds kinds,
                  const double* __restrict__ sEt, const double* __restrict__ sW,
                  const unsigned int* __restrict__ cell_begin, const unsigned int* __restrict__ unit_begin, ScanGeom geo,

@@ -125,16 +125,17 @@ int osc_reweight_bin_scales(const double *E_true, const double *E_reco, const do
  * the state set by osc_set_params.
  *   points    HOST [n_points]; validated and copied before the call returns
  *   hist_out  DEVICE [n_points][OSC_N_CHANNELS][n_bins] fp64, OVERWRITTEN
- * Two code paths, chosen per call from the point list (results agree to rounding, both are
+ * Three code paths, chosen per call from the point list (results agree to rounding, each is
  * bit-reproducible from run to run):
  *   - points that differ only in sin2_th23 and delta_cp share the matter eigen-problem.  When the list has
  *     at least 8 points per such group on average (a scan grid: "only theta23 and dm2_32
  *     float"), the events are sorted by histogram cell once and the eigen-solve is done once per (event,
  *     group); a point then costs 4 to 6 fused multiply-adds per event (kernel k4, csrc/osc_scan.cuh);
- *   - otherwise every (event, point) pair gets the full closed form from event tiles staged in shared
- *     memory (kernel k3).
- * The environment variable OSC_BATCH_PATH = k3 | k4, read at every call, forces one path (tests use it
- * to check both paths on the same inputs); any other value, or none, leaves the choice to the library. */
+ *   - otherwise every (event, point) pair gets the full closed form: from 8 points on, on the events
+ *     sorted by histogram cell, with the weights of a cell summed in registers (kernel k5); below 8 points on
+ *     event tiles staged in shared memory in the caller's order (kernel k3).
+ * The environment variable OSC_BATCH_PATH = k3 | k4 | k5, read at every call, forces one path (tests use
+ * it to check the paths on the same inputs); any other value, or none, leaves the choice to the library. */
 int osc_reweight_bin_batch(const osc_params *points, int n_points, const double *E_true,
                            const double *E_reco, const double *w0, const int8_t *channel, size_t n,
                            double energy_scale, const double *bin_edges, int n_bins, double *hist_out,

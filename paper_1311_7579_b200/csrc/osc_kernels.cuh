@@ -97,9 +97,15 @@ prob_kernel(const __grid_constant__ ProbArgs a, const double* __restrict__ E_tru
 // k1b: all nine transitions.  One eigen-solve, four assembled amplitudes (alpha, beta in {e, mu});
 // the remaining five probabilities are the unitarity complements.  Row 3*beta + alpha of P_out.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void prob_nine(const ProbAllArgs& a, double E, bool ok, double P[9])
+// max(x, 0) that lets NaN through (fmax would turn it into 0): the complements below are differences of numbers near
+// 1 and may come out as -1e-17.
+__device__ __forceinline__ double clamp0_keep_nan(double x) { return x < 0.0 ? 0.0 : x; }
+
+// A11: an unusable energy is replaced by NaN, which then propagates through the closed form into all nine outputs
+// (two selects instead of nine).
+__device__ __forceinline__ void prob_nine(const ProbAllArgs& a, double E, double P[9])
 {
-    const double Es = ok ? E : 1.0;
+    const double Es = energy_ok(E) ? E : qnan();
     const double invE = rcp_pos(Es);
     const double A = a.tr[0].sa * Es;
     OscEig e;
@@ -108,21 +114,20 @@ __device__ __forceinline__ void prob_nine(const ProbAllArgs& a, double E, bool o
     const double p11 = assemble_diag<false>(e, A, a.tr[3]); // mu -> mu
     double p01, p10;                                        // p01: mu -> e (beta = e, alpha = mu); p10: e -> mu
     assemble_offdiag_pair(e, A, a.tr[1], p01, p10);
-    const double p20 = fmax((1.0 - p00) - p10, 0.0); // column alpha = e   sums to 1
-    const double p21 = fmax((1.0 - p11) - p01, 0.0); // column alpha = mu
-    const double p02 = fmax((1.0 - p00) - p01, 0.0); // row beta = e       sums to 1
-    const double p12 = fmax((1.0 - p11) - p10, 0.0); // row beta = mu
-    const double p22 = fmax((1.0 - p20) - p21, 0.0); // row beta = tau
-    const double nn = qnan();
-    P[0] = ok ? p00 : nn;
-    P[1] = ok ? p01 : nn;
-    P[2] = ok ? p02 : nn;
-    P[3] = ok ? p10 : nn;
-    P[4] = ok ? p11 : nn;
-    P[5] = ok ? p12 : nn;
-    P[6] = ok ? p20 : nn;
-    P[7] = ok ? p21 : nn;
-    P[8] = ok ? p22 : nn;
+    const double p20 = clamp0_keep_nan((1.0 - p00) - p10); // column alpha = e   sums to 1
+    const double p21 = clamp0_keep_nan((1.0 - p11) - p01); // column alpha = mu
+    const double p02 = clamp0_keep_nan((1.0 - p00) - p01); // row beta = e       sums to 1
+    const double p12 = clamp0_keep_nan((1.0 - p11) - p10); // row beta = mu
+    const double p22 = clamp0_keep_nan((1.0 - p20) - p21); // row beta = tau
+    P[0] = p00;
+    P[1] = p01;
+    P[2] = p02;
+    P[3] = p10;
+    P[4] = p11;
+    P[5] = p12;
+    P[6] = p20;
+    P[7] = p21;
+    P[8] = p22;
 }
 
 __global__ void __launch_bounds__(kBlock)
@@ -156,12 +161,18 @@ prob_all_kernel(const __grid_constant__ ProbAllArgs a, const double* __restrict_
         load(t + 2 * (size_t)gridDim.x, M0, M1);
         t += gridDim.x;
         double P0[9], P1[9];
-        prob_nine(a, E0, energy_ok(E0), P0);
-        prob_nine(a, E1, energy_ok(E1), P1);
+        prob_nine(a, E0, P0);
+        prob_nine(a, E1, P1);
+        // one running pointer per event, advanced by the row stride: nine row bases would not fit the uniform
+        // registers next to the constants of the closed form (ptxas spilled them and refilled them every iteration)
+        double* q0 = P_out + j0;
+        double* q1 = P_out + j1;
 #pragma unroll
         for (int k = 0; k < 9; ++k) {
-            if (in0) st_stream(P_out + (size_t)k * n + j0, P0[k]);
-            if (in1) st_stream(P_out + (size_t)k * n + j1, P1[k]);
+            if (in0) st_stream(q0, P0[k]);
+            if (in1) st_stream(q1, P1[k]);
+            q0 += n;
+            q1 += n;
         }
     }
 }

@@ -634,7 +634,10 @@ int launch_batch_scan(const ScanPlan* plan, const std::vector<BinArgs>* full, in
     ScanGeom geo;
     geo.ncells = kChannels * n_bins;
     geo.nsubs = plan ? (int)plan->subs.size() : n_points;      // items a warp walks per piece: sub-groups or points
-    geo.range = round_up(std::max<size_t>(1024, (n + 4095) / 4096), 32);
+    // warp ranges of the sort passes: short enough to give every SM dozens of warps (the passes are latency-bound),
+    // long enough to keep the [ncells][nranges] count table below 64 MB
+    const size_t max_ranges = std::min<size_t>(16384, (64u << 20) / (sizeof(unsigned int) * (size_t)geo.ncells));
+    geo.range = round_up(std::max<size_t>(256, (n + max_ranges - 1) / max_ranges), 32);
     geo.nranges = (unsigned)((n + geo.range - 1) / geo.range);
     int slots = geo.nsubs < 8 ? geo.nsubs : 8;
     geo.subs_per_slot = (geo.nsubs + slots - 1) / slots;
@@ -714,7 +717,8 @@ int launch_batch_scan(const ScanPlan* plan, const std::vector<BinArgs>* full, in
                                                                  unit_begin, geo, n_bins, partial);
         if ((rc = post_launch("osc_reweight_bin_batch (scan, one eigen-problem per point)"))) return rc;
     }
-    scan_merge_kernel<<<geo.ncells, 256, 0, st>>>(partial, unit_begin, geo.ncells, n_points, hist_out);
+    scan_merge_kernel<<<dim3((unsigned)geo.ncells, (unsigned)((n_points + 255) / 256)), 256, 0, st>>>(
+        partial, unit_begin, geo.ncells, n_points, hist_out);
     return post_launch("osc_reweight_bin_batch (merge)");
 }
 

@@ -531,17 +531,27 @@ scan_full_kernel(const double* __restrict__ points, int npoints, int pts_per_slo
 }
 
 // out[p][cell] = sum over the pieces of the cell, in order, of partial[piece][p]; 0 for an empty cell.
+// grid (ncells, ceil(npoints / 256)); the loads of eight pieces are issued together before they are added.
 __global__ void __launch_bounds__(256)
 scan_merge_kernel(const double* __restrict__ partial, const unsigned int* __restrict__ unit_begin, int ncells,
                   int npoints, double* __restrict__ out)
 {
     const int cell = blockIdx.x;
+    const int p = blockIdx.y * blockDim.x + threadIdx.x;
+    if (p >= npoints) return;
     const unsigned u0 = unit_begin[cell], u1 = unit_begin[cell + 1];
-    for (int p = threadIdx.x; p < npoints; p += blockDim.x) {
-        double s = 0.0;
-        for (unsigned u = u0; u < u1; ++u) s += partial[(size_t)u * npoints + p];
-        out[(size_t)p * ncells + cell] = s;
+    const double* src = partial + (size_t)u0 * npoints + p;
+    double s = 0.0;
+    unsigned u = u0;
+    for (; u + 8 <= u1; u += 8, src += (size_t)8 * npoints) {
+        double v[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) v[k] = __ldg(src + (size_t)k * npoints);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) s += v[k];
     }
+    for (; u < u1; ++u, src += npoints) s += __ldg(src);
+    out[(size_t)p * ncells + cell] = s;
 }
 
 } // namespace oscb

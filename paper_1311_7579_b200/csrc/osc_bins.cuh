@@ -117,6 +117,28 @@ __device__ __forceinline__ int find_bin(const BinView& t, double x)
     return (lo < t.nb && t.key0 <= kx) ? lo : -1;
 }
 
+// The same search with the validity as a predicate instead of a -1 return value: `lo` is always a cell index that can
+// be used in address arithmetic, the return value says whether x lies inside the binning.  Saves the select chain
+// that the -1 convention forces on a caller which goes on to form an address.
+template <int STEPS>
+__device__ __forceinline__ bool find_bin_pred(const BinView& t, double x, int& lo_out)
+{
+    const long long kx = order_key(x);
+    const int khi = (int)(kx >> 32);
+    const unsigned int rel = (unsigned int)max(khi, t.base) - (unsigned int)t.base;
+    const unsigned int cell = min(rel >> t.shift, (unsigned int)(kLutCells - 1));
+    int lo = (int)lds_u16(t.lut + 2u * cell);
+    lo += ((long long)lds_u64(t.ekey + 8u * (unsigned)(lo + 1)) <= kx) ? 1 : 0;
+    if (STEPS != 1) {
+        lo += ((long long)lds_u64(t.ekey + 8u * (unsigned)(lo + 1)) <= kx) ? 1 : 0;
+        if (t.steps > 2u) {
+            while (lo < t.nb && (long long)lds_u64(t.ekey + 8u * (unsigned)(lo + 1)) <= kx) ++lo;
+        }
+    }
+    lo_out = lo;
+    return lo < t.nb && t.key0 <= kx;
+}
+
 // Builds the table for `edges` in shared memory.  Called by all threads of the block (it contains
 // barriers); about 2 us per block, once per kernel.
 __device__ __forceinline__ void build_bin_table(unsigned char* smem_table, const double* __restrict__ edges, int nb)

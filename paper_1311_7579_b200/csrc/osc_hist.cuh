@@ -62,6 +62,17 @@ __device__ __forceinline__ void warp_hist_match(HistPlan& p, const LaneHist& lh,
     p.m1 = __match_any_sync(FULL, p.a1);
 }
 
+// The same with the validity of each event as a predicate (cell may be anything for a dropped event).
+__device__ __forceinline__ void warp_hist_match_pred(HistPlan& p, const LaneHist& lh, bool ok0, int cell0, bool ok1,
+                                                     int cell1)
+{
+    const unsigned FULL = 0xffffffffu;
+    p.a0 = ok0 ? lh.h0 + 8u * (unsigned)cell0 : 0xFFFFFFFFu;
+    p.a1 = ok1 ? lh.h1 + 8u * (unsigned)cell1 : 0xFFFFFFFFu;
+    p.m0 = __match_any_sync(FULL, p.a0);
+    p.m1 = __match_any_sync(FULL, p.a1);
+}
+
 // Step 2 (once MATCH has had time to come back): ranks and the pre-read of the rank-0 lanes.
 __device__ __forceinline__ void warp_hist_rank(HistPlan& p, unsigned lt_mask)
 {

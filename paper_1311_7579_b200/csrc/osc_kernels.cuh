@@ -237,15 +237,17 @@ __device__ __forceinline__ OscSet load_set(const double* pb)
 // ch is the channel byte zero-extended: 0..3 are valid, every other code (negative int8 values, the 0xFF that
 // load_pair puts in for events past the end) is not.
 template <int STEPS>
-__device__ __forceinline__ void locate_one(const BinView& bt, double energy_scale, double Et, double Er, unsigned ch,
+__device__ __forceinline__ bool locate_one(const BinView& bt, double energy_scale, double Et, double Er, unsigned ch,
                                            int& cell, unsigned& c, double& Es)
 {
     const double x = scaled_energy(energy_scale, Er);       // a3b: one rounded fp64 multiply
-    const int bin = find_bin<STEPS>(bt, x);                 // a3c: bit-exact index
-    const bool ok = energy_ok(Et) && ch < (unsigned)kChannels && bin >= 0;
+    int bin;
+    const bool inside = find_bin_pred<STEPS>(bt, x, bin);   // a3c: bit-exact index
+    const bool ok = energy_ok(Et) && ch < (unsigned)kChannels && inside;
     c = ok ? ch : 0u;
     Es = ok ? Et : 1.0;
-    cell = ok ? (int)c * bt.nb + bin : -1;
+    cell = (int)c * bt.nb + bin;                            // only used when ok
+    return ok;
 }
 
 // Two events of one thread as they come from global memory (VEC: events 2i, 2i+1 by 128-bit loads).  The two channel
@@ -297,10 +299,10 @@ __device__ __forceinline__ void k2_loop(const BinArgs& a, const double* __restri
         int cell0, cell1;
         unsigned c0, c1;
         double Es0, Es1;
-        locate_one<STEPS>(bt, energy_scale, cur.Et0, cur.Er0, cur.chp & 0xFFu, cell0, c0, Es0);
-        locate_one<STEPS>(bt, energy_scale, cur.Et1, cur.Er1, cur.chp >> 8, cell1, c1, Es1);
+        const bool ok0 = locate_one<STEPS>(bt, energy_scale, cur.Et0, cur.Er0, cur.chp & 0xFFu, cell0, c0, Es0);
+        const bool ok1 = locate_one<STEPS>(bt, energy_scale, cur.Et1, cur.Er1, cur.chp >> 8, cell1, c1, Es1);
         HistPlan plan;
-        warp_hist_match(plan, lh, cell0, cell1);
+        warp_hist_match_pred(plan, lh, ok0, cell0, ok1, cell1);
         const double wp0 = cur.wp0, wp1 = cur.wp1;
         // prefetch: E_true, E_reco and channel of the current pair are dead from here on
         t += gridDim.x;

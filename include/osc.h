@@ -179,6 +179,11 @@ int osc_prob_host(const double *E_true_host, size_t n, int flavour_in, int flavo
 int osc_reweight_bin_host(const double *E_true_host, const double *E_reco_host, const double *w0_host,
                           const int8_t *channel_host, size_t n, double energy_scale,
                           const double *bin_edges_host, int n_bins, double *hist_out_host);
+/* The same for several energy-scale values (osc_reweight_bin_scales): the events cross PCIe once for all scales.
+ *   energy_scales  HOST [n_scales], 1 <= n_scales <= 4;   hist_out_host  HOST [n_scales][OSC_N_CHANNELS][n_bins] */
+int osc_reweight_bin_scales_host(const double *E_true_host, const double *E_reco_host, const double *w0_host,
+                                 const int8_t *channel_host, size_t n, const double *energy_scales, int n_scales,
+                                 const double *bin_edges_host, int n_bins, double *hist_out_host);
 
 /* Message of the calling thread's most recent error ("" if none).  Never NULL. */
 const char *osc_last_error(void);

@@ -24,7 +24,7 @@ PARAM_FIELDS = ("sin2_th12", "sin2_th23", "sin2_th13", "dm2_32", "dm2_21", "delt
 
 # every symbol include/osc.h declares (tests/test_abi.py checks the header against this list)
 EXPORTS = ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_scales", "osc_reweight_bin_batch",
-           "osc_neg2lnl", "osc_bin_centre_compare", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_last_error", "osc_launch_count",
+           "osc_neg2lnl", "osc_bin_centre_compare", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_reweight_bin_scales_host", "osc_last_error", "osc_launch_count",
            "osc_version", "osc_set_device", "osc_get_device", "osc_fp64_peak_probe")
 
 
@@ -63,12 +63,14 @@ def lib() -> ctypes.CDLL:
     L.osc_bin_centre_compare.argtypes = [_dp, _dp, _dp, sz, _dp, i, _dp, _dp, vp]
     L.osc_prob_host.argtypes = [_dp, sz, i, i, i, _dp]
     L.osc_reweight_bin_host.argtypes = [_dp, _dp, _dp, _dp, sz, d, _dp, i, _dp]
+    L.osc_reweight_bin_scales_host.argtypes = [_dp, _dp, _dp, _dp, sz, ctypes.POINTER(d), i, _dp, i, _dp]
     L.osc_set_device.argtypes = [i]
     L.osc_get_device.argtypes = [ctypes.POINTER(i)]
     L.osc_fp64_peak_probe.argtypes = [i, i, ctypes.POINTER(d), vp]
     for name in ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_scales",
                  "osc_reweight_bin_batch",
-                 "osc_neg2lnl", "osc_bin_centre_compare", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_set_device", "osc_get_device",
+                 "osc_neg2lnl", "osc_bin_centre_compare", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_reweight_bin_scales_host", "osc_set_device",
+                 "osc_get_device",
                  "osc_fp64_peak_probe"):
         getattr(L, name).restype = i
     L.osc_last_error.restype = ctypes.c_char_p
@@ -328,3 +330,19 @@ def osc_fp64_peak_probe(iters: int, blocks_per_sm: int = 4, stream=None) -> floa
     flops = ctypes.c_double(0.0)
     _check(lib().osc_fp64_peak_probe(int(iters), int(blocks_per_sm), ctypes.byref(flops), _stream(stream)))
     return flops.value
+
+
+def osc_reweight_bin_scales_host(E_true: np.ndarray, E_reco: np.ndarray, w0: np.ndarray, channel: np.ndarray,
+                                 energy_scales: Sequence[float], bin_edges: np.ndarray,
+                                 hist_out: Optional[np.ndarray] = None) -> np.ndarray:
+    """Host buffers in and out, several energy scales, one trip of the events over PCIe."""
+    nb = bin_edges.size - 1
+    ns = len(energy_scales)
+    if hist_out is None:
+        hist_out = np.empty((ns, N_CHANNELS, nb), dtype=np.float64)
+    arr = (ctypes.c_double * max(ns, 1))(*[float(v) for v in energy_scales])
+    _check(lib().osc_reweight_bin_scales_host(_host(E_true, np.float64, "E_true"), _host(E_reco, np.float64, "E_reco"),
+                                              _host(w0, np.float64, "w0"), _host(channel, np.int8, "channel"),
+                                              E_true.size, arr, ns, _host(bin_edges, np.float64, "bin_edges"), nb,
+                                              _host(hist_out, np.float64, "hist_out")))
+    return hist_out

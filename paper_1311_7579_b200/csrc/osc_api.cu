@@ -963,19 +963,23 @@ int osc_prob_host(const double* E_true_host, size_t n, int flavour_in, int flavo
     return OSC_OK;
 }
 
-int osc_reweight_bin_host(const double* E_true_host, const double* E_reco_host, const double* w0_host,
-                          const int8_t* channel_host, size_t n, double energy_scale, const double* bin_edges_host,
-                          int n_bins, double* hist_out_host)
+int osc_reweight_bin_scales_host(const double* E_true_host, const double* E_reco_host, const double* w0_host,
+                                 const int8_t* channel_host, size_t n, const double* energy_scales, int n_scales,
+                                 const double* bin_edges_host, int n_bins, double* hist_out_host)
 {
     if (n_bins < 1 || n_bins > kMaxBins) return fail(OSC_ERR_INVALID_ARG, "n_bins = %d outside [1, %d]", n_bins, kMaxBins);
-    if (!bin_edges_host || !hist_out_host) return fail(OSC_ERR_INVALID_ARG, "null bin_edges or hist_out");
+    if (n_scales < 1 || n_scales > kMaxScales)
+        return fail(OSC_ERR_INVALID_ARG, "n_scales = %d outside [1, %d]", n_scales, kMaxScales);
+    if (!energy_scales || !bin_edges_host || !hist_out_host)
+        return fail(OSC_ERR_INVALID_ARG, "null energy_scales, bin_edges or hist_out");
     if (n > 0 && (!E_true_host || !E_reco_host || !w0_host || !channel_host))
         return fail(OSC_ERR_INVALID_ARG, "null host array with n > 0");
     std::lock_guard<std::mutex> lk(g_host.mu);
+    const size_t nh = (size_t)kChannels * n_bins;
     const size_t b8 = round_up(n * sizeof(double), 256);
     const size_t b1 = round_up(n, 256);
     const size_t be = round_up((size_t)(n_bins + 1) * sizeof(double), 256);
-    const size_t bh = round_up((size_t)kChannels * n_bins * sizeof(double), 256);
+    const size_t bh = round_up((size_t)n_scales * nh * sizeof(double), 256);
     int rc = g_host.ensure(3 * b8 + b1 + be + bh + 256);
     if (rc) return rc;
     char* p = g_host.buf;
@@ -993,11 +997,19 @@ int osc_reweight_bin_host(const double* E_true_host, const double* E_reco_host, 
         CUDA_TRY(cudaMemcpyAsync(dC, channel_host, n, cudaMemcpyHostToDevice, st));
     }
     CUDA_TRY(cudaMemcpyAsync(dEdges, bin_edges_host, (size_t)(n_bins + 1) * sizeof(double), cudaMemcpyHostToDevice, st));
-    rc = osc_reweight_bin(dEt, dEr, dW, dC, n, energy_scale, dEdges, n_bins, dH, st);
+    rc = osc_reweight_bin_scales(dEt, dEr, dW, dC, n, energy_scales, n_scales, dEdges, n_bins, dH, st);
     if (rc) return rc;
-    CUDA_TRY(cudaMemcpyAsync(hist_out_host, dH, (size_t)kChannels * n_bins * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(hist_out_host, dH, (size_t)n_scales * nh * sizeof(double), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     return OSC_OK;
+}
+
+int osc_reweight_bin_host(const double* E_true_host, const double* E_reco_host, const double* w0_host,
+                          const int8_t* channel_host, size_t n, double energy_scale, const double* bin_edges_host,
+                          int n_bins, double* hist_out_host)
+{
+    return osc_reweight_bin_scales_host(E_true_host, E_reco_host, w0_host, channel_host, n, &energy_scale, 1,
+                                        bin_edges_host, n_bins, hist_out_host);
 }
 
 const char* osc_last_error(void) { return t_err; }

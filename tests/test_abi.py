@@ -120,6 +120,9 @@ def test_host_checkable_faults(L):
     sc[1] = 1.0
     assert L.osc_reweight_bin_scales(None, None, None, None, 3, sc, 3, 8, 4, 8, None) == INVALID   # null events, n > 0
     assert L.osc_reweight_bin_scales(16, 16, 16, 16, 3, sc, 3, 12, 4, 8, None) == ALIGN
+    assert L.osc_reweight_bin_scales_host(None, None, None, None, 0, sc, 0, 8, 4, 8) == INVALID
+    assert L.osc_reweight_bin_scales_host(None, None, None, None, 0, None, 3, 8, 4, 8) == INVALID
+    assert L.osc_reweight_bin_scales_host(None, None, None, None, 3, sc, 3, 8, 4, 8) == INVALID
     # likelihood: sizes, normalisation, null pointers; no points is a no-op
     assert L.osc_neg2lnl(8, 4, 0, 8, 1.0, 8, None) == INVALID
     assert L.osc_neg2lnl(8, -1, 10, 8, 1.0, 8, None) == INVALID

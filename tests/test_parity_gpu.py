@@ -635,6 +635,10 @@ def test_host_entry_points(osc):
     assert_prob_close(osc.osc_prob_host(et, 1, 0, 1), oracle.prob(op, et, 1, 0, 1), "osc_prob_host")
     assert_hist_close(osc.osc_reweight_bin_host(et, er, w0, ch, 1.03, edges),
                       oracle.reweight_bin(op, et, er, w0, ch, 1.03, edges), "osc_reweight_bin_host")
+    hs = osc.osc_reweight_bin_scales_host(et, er, w0, ch, wl.ENERGY_SCALES, edges)
+    assert hs.shape == (3, 4, 50)
+    for k, s in enumerate(wl.ENERGY_SCALES):
+        assert_hist_close(hs[k], oracle.reweight_bin(op, et, er, w0, ch, s, edges), f"osc_reweight_bin_scales_host {s}")
 
 
 # ------------------------------------------------------------------------------------------------

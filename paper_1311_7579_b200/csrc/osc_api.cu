@@ -797,12 +797,16 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
     }
     // Point lists without scan structure: from 8 points on the sort of the events pays for itself (kernel k5 on
     // the sorted events); below that the events are taken in their own order (kernel k3).
+    // k3 keeps 32 sub-histograms per block in shared memory and takes binnings up to about 190 bins; finer ones
+    // always go through the sorted events, which have no histogram in shared memory at all.
+    const bool k3_fits = sizeof(double) * kBinArgsDoubles + bin_table_bytes(n_bins) + sizeof(double) * 16 * kSlots * nh +
+                             (size_t)kBatchBytesPerEvent * 2 * 512 <= kSmemBudget;
     {
         bool use_full = n_points >= 8;
         const char* e = getenv("OSC_BATCH_PATH");
         if (e && !std::strcmp(e, "k5")) use_full = true;
         if (e && !std::strcmp(e, "k3")) use_full = false;
-        if (use_full)
+        if (use_full || !k3_fits)
             return launch_batch_scan(nullptr, &blocks, n_points, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
                                      n_bins, hist_out, st);
     }
@@ -817,8 +821,7 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
     const int n_sub = (2 * hist1 <= 64 * 1024) ? 2 : 1;
     const size_t fixed = sizeof(double) * kBinArgsDoubles + bin_table_bytes(n_bins) + n_sub * hist1;
     if (fixed + (size_t)kBatchBytesPerEvent * 2 * threads > budget)
-        return fail(OSC_ERR_INVALID_ARG, "osc_reweight_bin_batch: n_bins = %d needs more shared memory than one SM has "
-                                         "(limit for the batched call: about 380 bins)", n_bins);
+        return fail(OSC_ERR_INVALID_ARG, "osc_reweight_bin_batch: n_bins = %d does not fit kernel k3's shared memory", n_bins);
     const int blocks_per_sm = 512 / threads;
     const int tile_quant = 2 * threads;
     int te = (int)((budget - fixed) / kBatchBytesPerEvent / tile_quant * tile_quant);

@@ -487,6 +487,34 @@ def test_k4_small_and_ragged_sizes(osc, n, nb, kind, path):
     assert_hist_close(got, ref, f"{path} n={n} nb={nb}")
 
 
+@pytest.mark.parametrize("path", ["k3", "k4", "k5"])
+def test_batch_paths_with_many_bins(osc, path):
+    """350 bins x 4 channels = 1400 cells: the per-warp counters of the sort passes and the cell search of the piece
+    kernels at a size well beyond configs[3]'s 200 cells.  k3's shared-memory histograms stop fitting near 190 bins:
+    forcing k3 here must still give the right answer (the library falls back to the sorted events)."""
+    n = 30_000 + 5
+    et, er, w0, ch = wl.events(n, seed=26)
+    edges = wl.bin_edges(350, 5.0)
+    pts = [wl.table1(sin2_th23=0.35 + 0.02 * k, delta_cp=-2.0 + 0.3 * k) for k in range(12)]
+    with batch_path(path):
+        got = host(osc.osc_reweight_bin_batch(pts, dev(et), dev(er), dev(w0), dev(ch), 1.0, dev(edges)))
+    ref = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 1.0, edges)
+    assert_hist_close(got, ref, f"{path} with 350 bins")
+
+
+def test_batch_sorted_paths_with_768_bins(osc):
+    """The largest binning the library accepts (768 bins, 3072 cells): only the sorted paths take it in a batch."""
+    n = 10_000
+    et, er, w0, ch = wl.events(n, seed=27)
+    edges = wl.bin_edges(768, 5.0)
+    pts = [wl.table1(sin2_th23=0.3 + 0.04 * k, dm2_32=2.2e-3 + 1e-5 * (k // 5)) for k in range(10)]
+    ref = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 1.0, edges)
+    for path in ("k4", "k5"):
+        with batch_path(path):
+            got = host(osc.osc_reweight_bin_batch(pts, dev(et), dev(er), dev(w0), dev(ch), 1.0, dev(edges)))
+        assert_hist_close(got, ref, f"{path} with 768 bins")
+
+
 def test_k4_all_events_dropped(osc):
     n = 500
     et, er, w0, ch = wl.events(n, seed=25)

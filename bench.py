@@ -56,11 +56,11 @@ def parse():
     ap.add_argument("--events", type=int, default=None, help="events per GPU (default: the size the config names)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--workload", default="config2", choices=["config0", "config1", "config2", "config3", "config3-k3",
-                                                               "config3-k5", "config4"],
+    ap.add_argument("--workload", default="config2", choices=["config0", "config1", "config2", "config3", "config3-k5",
+                                                               "config4"],
                     help="config2 (default) is the bench line; the others time the remaining BASELINE.json configs "
-                         "for BASELINE.md section 4 and give ncu a committed command for k1 / k1b / k3 / k4 "
-                         "(config3-k3 / config3-k5 force the unfactorised batched kernels; config4 is the size sweep)")
+                         "for BASELINE.md section 4 and give ncu a committed command for k1 / k1b / k4 / k5 "
+                         "(config3-k5 forces the unfactorised batched kernel; config4 is the size sweep)")
     return ap.parse_args()
 
 
@@ -209,8 +209,6 @@ OTHER = {
                        flop_per_unit=K5_FLOP_PER_UNIT,
                        what="configs[3] with OSC_BATCH_PATH=k5: every (event, point) pair gets the full closed form, on "
                             "events sorted by histogram cell (the path of point lists without scan structure)"),
-    "config3-k3": dict(n=1_000_000, kernel="reweight_batch_kernel (k3)", bytes_per_unit=25.0 / 1024, flop_per_unit=203.5,
-                       what="configs[3] with OSC_BATCH_PATH=k3: every (event, point) pair gets the full closed form"),
 }
 
 
@@ -254,8 +252,8 @@ def run_other(args):
         et, er, w0, ch = wl.events(n, seed=2)
         d_et, d_er, d_w0, d_ch = (torch.from_numpy(a).to(dev) for a in (et, er, w0, ch))
         d_edges = torch.from_numpy(wl.bin_edges()).to(dev)
-        if args.workload in ("config3-k3", "config3-k5"):
-            os.environ["OSC_BATCH_PATH"] = args.workload[-2:]
+        if args.workload == "config3-k5":
+            os.environ["OSC_BATCH_PATH"] = "k5"
         pts = osc.pack_params(wl.scan_points())                                 # marshalled once (binding only)
         out = torch.empty((len(pts), osc.N_CHANNELS, wl.N_BINS), dtype=torch.float64, device=dev)
         units = n * len(pts)

@@ -776,14 +776,14 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
     }
     // Points that differ only in theta23 and delta_cp share the eigen-problem: when the list has enough of that
     // structure (a scan grid), the factorised path k4 does the eigen-solve once per group (osc_scan.cuh).
-    // OSC_BATCH_PATH = k3 | k4 overrides the choice (tests exercise both paths on the same inputs).
+    // OSC_BATCH_PATH = k2 | k4 | k5 overrides the choice (tests exercise all paths on the same inputs).
     {
         ScanPlan plan;
         build_scan_plan(points, n_points, plan);
         bool use_scan = (size_t)n_points >= 8 * plan.subs.size();
         const char* e = getenv("OSC_BATCH_PATH");
         if (e && !std::strcmp(e, "k4")) use_scan = true;
-        if (e && (!std::strcmp(e, "k3") || !std::strcmp(e, "k5"))) use_scan = false;
+        if (e && (!std::strcmp(e, "k2") || !std::strcmp(e, "k5"))) use_scan = false;
         if (use_scan)
             return launch_batch_scan(&plan, nullptr, n_points, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
                                      n_bins, hist_out, st);
@@ -795,78 +795,22 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
         precompute(points[p], h);
         make_bin_args(h, blocks[(size_t)p]);
     }
-    // Point lists without scan structure: from 8 points on the sort of the events pays for itself (kernel k5 on
-    // the sorted events); below that the events are taken in their own order (kernel k3).
-    // k3 keeps 32 sub-histograms per block in shared memory and takes binnings up to about 190 bins; finer ones
-    // always go through the sorted events, which have no histogram in shared memory at all.
-    const bool k3_fits = sizeof(double) * kBinArgsDoubles + bin_table_bytes(n_bins) + sizeof(double) * 16 * kSlots * nh +
-                             (size_t)kBatchBytesPerEvent * 2 * 512 <= kSmemBudget;
-    {
-        bool use_full = n_points >= 8;
-        const char* e = getenv("OSC_BATCH_PATH");
-        if (e && !std::strcmp(e, "k5")) use_full = true;
-        if (e && !std::strcmp(e, "k3")) use_full = false;
-        if (use_full || !k3_fits)
-            return launch_batch_scan(nullptr, &blocks, n_points, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
-                                     n_bins, hist_out, st);
+    // Point lists without scan structure.  The sort of the events pays for itself from four points on (measured on
+    // 1e6 and 1e7 events: the sorted kernel k5 is ahead of one k2 pass per point from 4 points, behind it at 2);
+    // below that every point gets its own pass of the fused single-set kernel k2.
+    bool use_full = n_points >= 4;
+    if (const char* e = getenv("OSC_BATCH_PATH")) {
+        if (!std::strcmp(e, "k5")) use_full = true;
+        if (!std::strcmp(e, "k2")) use_full = false;
     }
-    int sms = 0;
-    if ((rc = sm_count(&sms))) return rc;
-
-    // geometry: 1 block of 512 threads per SM (shared-memory bound; two blocks of 256 measured 2 % slower on
-    // configs[3]); blocks = nchunks x ngroups ~ 4 waves
-    const int threads = 512;
-    const size_t budget = kSmemBudget;
-    const size_t hist1 = sizeof(double) * (threads / 32) * kSlots * nh;
-    const int n_sub = (2 * hist1 <= 64 * 1024) ? 2 : 1;
-    const size_t fixed = sizeof(double) * kBinArgsDoubles + bin_table_bytes(n_bins) + n_sub * hist1;
-    if (fixed + (size_t)kBatchBytesPerEvent * 2 * threads > budget)
-        return fail(OSC_ERR_INVALID_ARG, "osc_reweight_bin_batch: n_bins = %d does not fit kernel k3's shared memory", n_bins);
-    const int blocks_per_sm = 512 / threads;
-    const int tile_quant = 2 * threads;
-    int te = (int)((budget - fixed) / kBatchBytesPerEvent / tile_quant * tile_quant);
-    if (te > 8192) te = 8192;
-    BatchGeom geo;
-    const int target_blocks = 4 * sms * blocks_per_sm;
-    int ngroups = n_points < 16 ? n_points : 16;
-    size_t max_chunks = (n + tile_quant - 1) / tile_quant;          // at least one thread-pair row per chunk
-    size_t nchunks = (size_t)(target_blocks + ngroups - 1) / ngroups;
-    if (nchunks > max_chunks) {
-        nchunks = max_chunks;
-        // few events: spread the points over more groups instead
-        size_t want = ((size_t)target_blocks + nchunks - 1) / nchunks;
-        ngroups = (int)(want < (size_t)n_points ? want : (size_t)n_points);
-    }
-    geo.chunk_events = round_up((n + nchunks - 1) / nchunks, 2);
-    nchunks = (n + geo.chunk_events - 1) / geo.chunk_events;
-    geo.nchunks = (int)nchunks;
-    geo.pts_per_group = (n_points + ngroups - 1) / ngroups;
-    ngroups = (n_points + geo.pts_per_group - 1) / geo.pts_per_group;
-    if ((size_t)te > round_up(geo.chunk_events, tile_quant)) te = (int)round_up(geo.chunk_events, tile_quant);
-    geo.te = te;
-    const size_t smem = fixed + (size_t)kBatchBytesPerEvent * te;
-
-    const size_t bytes_points = round_up((size_t)n_points * sizeof(BinArgs), 256);
-    const size_t bytes_partial = (size_t)n_points * nchunks * nh * sizeof(double);
-    Scratch sc;
-    if ((rc = sc.alloc(bytes_points + bytes_partial, st))) return rc;
-    double* d_points = reinterpret_cast<double*>(sc.p);
-    double* partial = reinterpret_cast<double*>(sc.p + bytes_points);
-    // asynchronous upload from a pinned staging slot (PinnedRing)
-    PinnedRing* ring = nullptr;
-    if ((rc = ring_for_device(&ring))) return rc;
-    PinnedRing::Slot* slot = nullptr;
-    if ((rc = ring->acquire((size_t)n_points * sizeof(BinArgs), &slot))) return rc;
-    std::memcpy(slot->host, blocks.data(), (size_t)n_points * sizeof(BinArgs));
-    CUDA_TRY(cudaMemcpyAsync(d_points, slot->host, (size_t)n_points * sizeof(BinArgs), cudaMemcpyHostToDevice, st));
-    if ((rc = ring->fence(slot, st))) return rc;
-    const dim3 grid((unsigned)nchunks, (unsigned)ngroups);
-    CUDA_TRY(cudaFuncSetAttribute(reweight_batch_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    reweight_batch_kernel<512><<<grid, 512, smem, st>>>(d_points, n_points, E_true, E_reco, w0, channel, n, geo,
-                                                        energy_scale, bin_edges, n_bins, n_sub, partial);
-    if ((rc = post_launch("osc_reweight_bin_batch"))) return rc;
-    merge_chunks_kernel<<<n_points, 256, 0, st>>>(partial, (int)nchunks, (int)nh, hist_out);
-    return post_launch("osc_reweight_bin_batch merge");
+    if (use_full)
+        return launch_batch_scan(nullptr, &blocks, n_points, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
+                                 n_bins, hist_out, st);
+    for (int p = 0; p < n_points; ++p)
+        if ((rc = launch_reweight(blocks[(size_t)p], E_true, E_reco, w0, channel, n, energy_scale, bin_edges, n_bins,
+                                  hist_out + (size_t)p * nh, st)))
+            return rc;
+    return OSC_OK;
 }
 
 int osc_bin_centre_compare(const double* E_true, const double* w0, const int8_t* channel, size_t n,

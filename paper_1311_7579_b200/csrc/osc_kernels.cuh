@@ -3,10 +3,8 @@
 //   prob_kernel            k1   one transition per event                        (osc_prob)
 //   prob_all_kernel        k1b  nine transitions from one eigen-solve           (osc_prob_all)
 //   reweight_bin_kernel    k2   fused probability -> weight -> bin -> histogram  (osc_reweight_bin)
-//   reweight_batch_kernel  k3   event tiles resident in shared memory, reused across many
-//                               parameter sets                                   (osc_reweight_bin_batch)
-//   merge_chunks_kernel         fixed-order sum of k3's per-chunk histograms
-//   bin_index_kernel            the integer binning decision of k2/k3, exported  (osc_bin_index)
+//   (the batched call, osc_reweight_bin_batch, lives in osc_scan.cuh: k4 and k5 on events sorted by histogram cell)
+//   bin_index_kernel            the integer binning decision of k2, exported  (osc_bin_index)
 //
 // k1, k1b and k2 are persistent grid-stride kernels sized from the SM count; every thread carries two
 // events per iteration (two independent fp64 dependency chains) and the parameter block arrives as a
@@ -531,158 +529,6 @@ centre_weight_kernel(const __grid_constant__ BinArgs a, const double* __restrict
     const bool ok = energy_ok(c);
     const double P = prob_one(a.set, a.ch[ch], ok ? c : 1.0);
     hist[i] = ok ? hist[i] * P : qnan();
-}
-
-// ------------------------------------------------------------------------------------------------
-// k3: batched parameter sets (row a4).  Block (c, g) owns event chunk c and point group g.  The chunk is
-// staged tile by tile in shared memory -- E_true, w0 and the histogram cell of every event, which does
-// not depend on the parameter set and is therefore decided once per tile -- and every staged tile is
-// reused for all points of the group.  Per point the block fills per-warp sub-histograms, sums them in a
-// fixed order and adds the result to its own slice partial[p][c][:] in global memory; merge_chunks_kernel
-// then sums the chunks of each point in chunk order.
-//
-// Shared memory: param block | bin table | hist[warps][kSlots][n_sub][4 nb] | Et[te] | w0[te] | plan[te]
-// plan (32 bit) = cell | channel << 12 | rank << 16 (cell < 4 * 768 = 3072), 0xFFFFFFFF for a dropped or padding event.
-// The rank of an event among the lanes of its warp that hit the same histogram word (osc_hist.cuh) depends on the
-// cells only, not on the parameter set: MATCH runs once per staged tile, not once per point.
-// ------------------------------------------------------------------------------------------------
-constexpr unsigned kDropped = 0xFFFFFFFFu;
-constexpr int kBatchBytesPerEvent = 20;   // E_true + w0 (fp64) + plan (u32)
-
-struct BatchGeom {
-    size_t chunk_events;  // events per chunk (multiple of 2)
-    int te;               // tile capacity in events (multiple of 2 * THREADS)
-    int nchunks;
-    int pts_per_group;
-};
-
-// Launched with 512 threads, one block per SM.
-template <int kBatchThreads>
-__global__ void __launch_bounds__(kBatchThreads, 512 / kBatchThreads)
-reweight_batch_kernel(const double* __restrict__ points, int npts, const double* __restrict__ E_true,
-                      const double* __restrict__ E_reco, const double* __restrict__ w0,
-                      const int8_t* __restrict__ channel, size_t n, BatchGeom geo, double energy_scale,
-                      const double* __restrict__ edges, int nb, int n_sub, double* __restrict__ partial)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int WARPS = kBatchThreads / 32;
-    const int nh = kChannels * nb;
-    const int n_hist = WARPS * kSlots * n_sub;
-    double* pbuf = reinterpret_cast<double*>(smem_raw);
-    unsigned char* tab = smem_raw + sizeof(double) * kBinArgsDoubles;
-    double* hist = reinterpret_cast<double*>(tab + bin_table_bytes(nb));
-    double* sEt = hist + (size_t)n_hist * nh;
-    double* sW = sEt + geo.te;
-    unsigned* sPlan = reinterpret_cast<unsigned*>(sW + geo.te);
-
-    const unsigned lane = threadIdx.x & 31u;
-    const unsigned warp = threadIdx.x >> 5;
-    const unsigned lt_mask = (1u << lane) - 1u;
-    const uint32_t pb = smem_u32(pbuf);
-    const LaneHist lh = lane_hist(hist, nh, n_sub, warp, lane);
-
-    const int chunk = blockIdx.x;
-    const size_t ev_begin = (size_t)chunk * geo.chunk_events;
-    const size_t ev_end = min(n, ev_begin + geo.chunk_events);
-    const int p_begin = blockIdx.y * geo.pts_per_group;
-    const int p_end = min(npts, p_begin + geo.pts_per_group);
-
-    for (int i = threadIdx.x; i < n_hist * nh; i += kBatchThreads) hist[i] = 0.0;
-    build_bin_table(tab, edges, nb);
-    const BinView bt = bin_view(tab);
-
-    bool first_tile = true;
-    for (size_t tile = ev_begin; tile < ev_end || first_tile; tile += geo.te) {
-        // ---- stage one tile: E_true, w0, cell (a3b, a3c taken once per event) -------------------
-        const int m = tile < ev_end ? (int)min((size_t)geo.te, ev_end - tile) : 0;
-        const int m_pad = (m + 2 * kBatchThreads - 1) / (2 * kBatchThreads) * (2 * kBatchThreads);
-        for (int j = threadIdx.x; j < m_pad; j += kBatchThreads) {
-            double Et = 1.0, wv = 0.0;
-            unsigned cc = kDropped;
-            if (j < m) {
-                const size_t g = tile + j;
-                const double e = ld_stream(E_true + g);
-                const double x = scaled_energy(energy_scale, ld_stream(E_reco + g));
-                const int ch = channel[g];
-                const int bin = find_bin<0>(bt, x);
-                if (energy_ok(e) && (unsigned)ch < (unsigned)kChannels && bin >= 0) {
-                    Et = e;
-                    wv = ld_stream(w0 + g);
-                    cc = (unsigned)((ch * nb + bin) | (ch << 12));
-                }
-            }
-            sEt[j] = Et;
-            sW[j] = wv;
-            sPlan[j] = cc;
-        }
-        __syncthreads();
-        // ---- rank the events of every warp iteration once (same thread -> event map as the point loop) ----
-        for (int j = threadIdx.x; j < m_pad; j += 2 * kBatchThreads) {
-            const int j1 = j + kBatchThreads;
-            const unsigned cc0 = sPlan[j], cc1 = sPlan[j1];
-            HistPlan pl;
-            warp_hist_match(pl, lh, cc0 == kDropped ? -1 : (int)(cc0 & 0xFFFu), cc1 == kDropped ? -1 : (int)(cc1 & 0xFFFu));
-            if (cc0 != kDropped) sPlan[j] = cc0 | ((unsigned)__popc(pl.m0 & lt_mask) << 16);
-            if (cc1 != kDropped) sPlan[j1] = cc1 | ((unsigned)__popc(pl.m1 & lt_mask) << 16);
-        }
-        // (every thread re-reads only the words it wrote itself: no barrier needed before the point loop)
-
-        // ---- all points of the group over the staged tile ----------------------------------------
-        for (int p = p_begin; p < p_end; ++p) {
-            if (threadIdx.x < kBinArgsDoubles)
-                pbuf[threadIdx.x] = __ldg(points + (size_t)p * kBinArgsDoubles + threadIdx.x);
-            __syncthreads();
-            const OscSet set = load_set(pbuf);
-            for (int j = threadIdx.x; j < m_pad; j += 2 * kBatchThreads) {
-                const int j1 = j + kBatchThreads;
-                const unsigned cc0 = sPlan[j], cc1 = sPlan[j1];
-                const double Et0 = sEt[j], Et1 = sEt[j1];
-                HistPlan pl;
-                pl.r0 = (int)cc0 >> 16;                                  // -1 for a dropped event
-                pl.r1 = (int)cc1 >> 16;
-                pl.a0 = lh.h0 + 8u * (cc0 & 0xFFFu);
-                pl.a1 = lh.h1 + 8u * (cc1 & 0xFFFu);
-                pl.rmax = __reduce_max_sync(0xffffffffu, max(pl.r0, pl.r1));
-                pl.v0 = 0.0;
-                pl.v1 = 0.0;
-                if (pl.r0 == 0) pl.v0 = lds_f64_volatile(pl.a0);
-                if (pl.r1 == 0) pl.v1 = lds_f64_volatile(pl.a1);
-                const OscTrans tr0 = load_trans(pb, (cc0 >> 12) & 3u);
-                const OscTrans tr1 = load_trans(pb, (cc1 >> 12) & 3u);
-                const double P0 = prob_one(set, tr0, Et0);
-                const double P1 = prob_one(set, tr1, Et1);
-                warp_hist_commit(pl, __dmul_rn(sW[j], P0), __dmul_rn(sW[j1], P1));
-            }
-            __syncthreads();
-            // sub-histograms summed in (warp, slot) order, cleared for the next point
-            double* dst = partial + ((size_t)p * geo.nchunks + chunk) * nh;
-            for (int i = threadIdx.x; i < nh; i += kBatchThreads) {
-                double s = 0.0;
-                for (int w = 0; w < n_hist; ++w) {
-                    s += hist[(size_t)w * nh + i];
-                    hist[(size_t)w * nh + i] = 0.0;
-                }
-                dst[i] = first_tile ? s : dst[i] + s;
-            }
-            // no barrier needed here: the parameter block and the tile arrays were last read before the
-            // barrier above, and the cleared histogram is next touched after the barrier that follows the
-            // next parameter-block load (or the next tile's staging barrier)
-        }
-        first_tile = false;
-    }
-}
-
-// out[p][i] = sum over chunks c (in order) of partial[p][c][i]
-__global__ void __launch_bounds__(256)
-merge_chunks_kernel(const double* __restrict__ partial, int nchunks, int nh, double* __restrict__ out)
-{
-    const size_t p = blockIdx.x;
-    const double* src = partial + p * (size_t)nchunks * nh;
-    for (int i = threadIdx.x; i < nh; i += blockDim.x) {
-        double s = src[i];
-        for (int c = 1; c < nchunks; ++c) s += src[(size_t)c * nh + i];
-        out[p * (size_t)nh + i] = s;
-    }
 }
 
 // Peak-rate probe for the roofline denominator: a chain-parallel DFMA loop, 8 independent chains per

@@ -419,7 +419,7 @@ scan_main_kernel(const ScanGroup* __restrict__ groups, const ScanSub* __restrict
 // k5: the batched call for point lists WITHOUT scan structure (every point its own eigen-problem, e.g. a batch of
 // Markov-chain proposals), on the sorted events of k4.  Warp (blockIdx.x * kScanWarps + warp) owns one piece of one
 // sorted cell and stages its events (E_true, 1/E_true, w0) in shared memory once; blockIdx.y selects the slot of
-// points it walks.  Lane = event throughout.  What the sort buys over k3:
+// points it walks.  Lane = event throughout.  What the sort buys over one pass of k2 per point:
 //   * every event of the piece has the same histogram cell: the weights are summed in a register and reduced over
 //     the warp once per (piece, point) -- no bin search, no MATCH, no shared-memory histogram in the point loop;
 //   * every event of the piece has the same channel: the transition block is loaded once per (piece, point) and the

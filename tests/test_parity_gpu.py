@@ -433,12 +433,12 @@ def test_k4_ragged_groups_vs_oracle(osc):
     ref = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 1.03, edges)
     with batch_path("k4"):
         got4 = host(osc.osc_reweight_bin_batch(pts, *d, 1.03, dev(edges)))
-    with batch_path("k3"):
+    with batch_path("k2"):
         got3 = host(osc.osc_reweight_bin_batch(pts, *d, 1.03, dev(edges)))
     with batch_path("k5"):
         got5 = host(osc.osc_reweight_bin_batch(pts, *d, 1.03, dev(edges)))
     assert_hist_close(got4, ref, "k4 ragged groups")
-    assert_hist_close(got3, ref, "k3 ragged groups")
+    assert_hist_close(got3, ref, "k2-per-point ragged groups")
     assert_hist_close(got5, ref, "k5 ragged groups")
     assert np.array_equal(got4 == 0.0, got3 == 0.0) and np.array_equal(got5 == 0.0, got3 == 0.0)
 
@@ -453,15 +453,15 @@ def test_k4_equals_k3_on_the_grid_with_more_events(osc):
     with batch_path("k4"):
         a = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, de))
         b = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, de))
-    with batch_path("k3"):
+    with batch_path("k2"):
         c = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, de))
     with batch_path("k5"):
         e = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, de))
         f = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, de))
     assert np.array_equal(a, b), "k4 is not bit-reproducible"
     assert np.array_equal(e, f), "k5 is not bit-reproducible"
-    assert_hist_close(a, c, "k4 vs k3")
-    assert_hist_close(e, c, "k5 vs k3")
+    assert_hist_close(a, c, "k4 vs k2 per point")
+    assert_hist_close(e, c, "k5 vs k2 per point")
     # the oracle on a sample of points (full 200k events each)
     pick = [0, 37, 95]
     ref = oracle.reweight_bin_batch([oracle.Params(**pts[i]) for i in pick], et, er, w0, ch, 1.0, edges)
@@ -487,11 +487,10 @@ def test_k4_small_and_ragged_sizes(osc, n, nb, kind, path):
     assert_hist_close(got, ref, f"{path} n={n} nb={nb}")
 
 
-@pytest.mark.parametrize("path", ["k3", "k4", "k5"])
+@pytest.mark.parametrize("path", ["k2", "k4", "k5"])
 def test_batch_paths_with_many_bins(osc, path):
     """350 bins x 4 channels = 1400 cells: the per-warp counters of the sort passes and the cell search of the piece
-    kernels at a size well beyond configs[3]'s 200 cells.  k3's shared-memory histograms stop fitting near 190 bins:
-    forcing k3 here must still give the right answer (the library falls back to the sorted events)."""
+    kernels at a size well beyond configs[3]'s 200 cells; "k2" is one pass of the single-set kernel per point."""
     n = 30_000 + 5
     et, er, w0, ch = wl.events(n, seed=26)
     edges = wl.bin_edges(350, 5.0)

@@ -682,7 +682,9 @@ int launch_batch_scan(const ScanPlan* plan, const std::vector<BinArgs>* full, in
     CUDA_TRY(cudaMemcpyAsync(d_groups, slot->host, b_groups + b_subs, cudaMemcpyHostToDevice, st));
     if ((rc = ring->fence(slot, st))) return rc;
 
-    const unsigned sort_blocks = (geo.nranges + kScanWarps - 1) / kScanWarps;
+    int sms = 0;
+    if ((rc = sm_count(&sms))) return rc;
+    const unsigned sort_blocks = std::min<unsigned>((geo.nranges + kScanWarps - 1) / kScanWarps, (unsigned)sms * 8u);
     const size_t smem_cnt = sizeof(unsigned int) * kScanWarps * (size_t)geo.ncells;
     const size_t smem_count = bin_table_bytes(n_bins) + smem_cnt;
     if (smem_count > 48 * 1024)
@@ -795,10 +797,11 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
         precompute(points[p], h);
         make_bin_args(h, blocks[(size_t)p]);
     }
-    // Point lists without scan structure.  The sort of the events pays for itself from four points on (measured on
-    // 1e6 and 1e7 events: the sorted kernel k5 is ahead of one k2 pass per point from 4 points, behind it at 2);
-    // below that every point gets its own pass of the fused single-set kernel k2.
-    bool use_full = n_points >= 4;
+    // Point lists without scan structure.  The sort of the events costs about 45 ps per event and then a point costs
+    // 9 ps per event in k5 against 14 ps (plus 20 us per launch) for a pass of the fused single-set kernel k2: measured
+    // on a B200, k5 is ahead from 4 points on at 1e6 events and from 10 points on at 1e7.  Below that every point gets
+    // its own k2 pass.
+    bool use_full = n_points >= (n <= 2000000 ? 4 : 10);
     if (const char* e = getenv("OSC_BATCH_PATH")) {
         if (!std::strcmp(e, "k5")) use_full = true;
         if (!std::strcmp(e, "k2")) use_full = false;

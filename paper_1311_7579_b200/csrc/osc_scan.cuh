@@ -100,26 +100,29 @@ scan_count_kernel(const double* __restrict__ E_true, const double* __restrict__ 
     const BinView bt = bin_view(smem_raw);
     const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     unsigned int* wcnt = reinterpret_cast<unsigned int*>(smem_raw + bin_table_bytes(nb)) + (size_t)warp * geo.ncells;
-    const unsigned r = blockIdx.x * kScanWarps + warp;
-    if (r >= geo.nranges) return;
-    for (int c = lane; c < geo.ncells; c += 32) wcnt[c] = 0u;
-    __syncwarp();
-    const size_t begin = (size_t)r * geo.range, end = min(n, begin + geo.range);
-    for (size_t j0 = begin; j0 < end; j0 += 32) {
-        const size_t j = j0 + lane;
-        unsigned cell = kNoCell;
-        if (j < end) {
-            const double x = scaled_energy(energy_scale, E_reco[j]);
-            const int bin = find_bin<0>(bt, x);
-            const unsigned ch = (unsigned)(unsigned char)channel[j];
-            if (energy_ok(E_true[j]) && ch < (unsigned)kChannels && bin >= 0) cell = ch * (unsigned)nb + (unsigned)bin;
-            cellid[j] = (unsigned short)cell;
+    // the grid is a few blocks per SM and every warp walks ranges r, r + warps of the grid, ...: the bin table is
+    // built once per block, not once per 4 ranges (it was two thirds of this kernel's instructions)
+    for (unsigned r = blockIdx.x * kScanWarps + warp; r < geo.nranges; r += gridDim.x * kScanWarps) {
+        for (int c = lane; c < geo.ncells; c += 32) wcnt[c] = 0u;
+        __syncwarp();
+        const size_t begin = (size_t)r * geo.range, end = min(n, begin + geo.range);
+        for (size_t j0 = begin; j0 < end; j0 += 32) {
+            const size_t j = j0 + lane;
+            unsigned cell = kNoCell;
+            if (j < end) {
+                const double x = scaled_energy(energy_scale, E_reco[j]);
+                const int bin = find_bin<0>(bt, x);
+                const unsigned ch = (unsigned)(unsigned char)channel[j];
+                if (energy_ok(E_true[j]) && ch < (unsigned)kChannels && bin >= 0) cell = ch * (unsigned)nb + (unsigned)bin;
+                cellid[j] = (unsigned short)cell;
+            }
+            const unsigned m = __match_any_sync(0xffffffffu, cell);
+            if (cell != kNoCell && lane == 31u - (unsigned)__clz((int)m)) wcnt[cell] += (unsigned)__popc(m);
+            __syncwarp();
         }
-        const unsigned m = __match_any_sync(0xffffffffu, cell);
-        if (cell != kNoCell && lane == 31u - (unsigned)__clz((int)m)) wcnt[cell] += (unsigned)__popc(m);
+        for (int c = lane; c < geo.ncells; c += 32) count[(size_t)c * geo.nranges + r] = wcnt[c];
         __syncwarp();
     }
-    for (int c = lane; c < geo.ncells; c += 32) count[(size_t)c * geo.nranges + r] = wcnt[c];
 }
 
 // Block-wide exclusive scan of one value per thread (1024 threads); returns the prefix, *total gets the sum.
@@ -212,26 +215,26 @@ scan_scatter_kernel(const double* __restrict__ E_true, const double* __restrict_
     const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const unsigned lt_mask = (1u << lane) - 1u;
     unsigned int* wcnt = reinterpret_cast<unsigned int*>(smem_raw) + (size_t)warp * geo.ncells;
-    const unsigned r = blockIdx.x * kScanWarps + warp;
-    if (r >= geo.nranges) return;
-    for (int c = lane; c < geo.ncells; c += 32) wcnt[c] = 0u;
-    __syncwarp();
-    const size_t begin = (size_t)r * geo.range, end = min(n, begin + geo.range);
-    for (size_t j0 = begin; j0 < end; j0 += 32) {
-        const size_t j = j0 + lane;
-        const unsigned cell = j < end ? (unsigned)cellid[j] : (unsigned)kNoCell;
-        const unsigned m = __match_any_sync(0xffffffffu, cell);
-        unsigned before = 0;
-        if (cell != kNoCell) before = wcnt[cell];
+    for (unsigned r = blockIdx.x * kScanWarps + warp; r < geo.nranges; r += gridDim.x * kScanWarps) {
+        for (int c = lane; c < geo.ncells; c += 32) wcnt[c] = 0u;
         __syncwarp();
-        if (cell != kNoCell) {
-            const size_t dst = (size_t)cell_begin[cell] + offsets[(size_t)cell * geo.nranges + r] + before +
-                               (unsigned)__popc(m & lt_mask);
-            sEt[dst] = E_true[j];
-            sW[dst] = w0[j];
-            if (lane == 31u - (unsigned)__clz((int)m)) wcnt[cell] = before + (unsigned)__popc(m);
+        const size_t begin = (size_t)r * geo.range, end = min(n, begin + geo.range);
+        for (size_t j0 = begin; j0 < end; j0 += 32) {
+            const size_t j = j0 + lane;
+            const unsigned cell = j < end ? (unsigned)cellid[j] : (unsigned)kNoCell;
+            const unsigned m = __match_any_sync(0xffffffffu, cell);
+            unsigned before = 0;
+            if (cell != kNoCell) before = wcnt[cell];
+            __syncwarp();
+            if (cell != kNoCell) {
+                const size_t dst = (size_t)cell_begin[cell] + offsets[(size_t)cell * geo.nranges + r] + before +
+                                   (unsigned)__popc(m & lt_mask);
+                sEt[dst] = E_true[j];
+                sW[dst] = w0[j];
+                if (lane == 31u - (unsigned)__clz((int)m)) wcnt[cell] = before + (unsigned)__popc(m);
+            }
+            __syncwarp();
         }
-        __syncwarp();
     }
 }
 

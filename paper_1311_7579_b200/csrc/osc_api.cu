@@ -684,14 +684,18 @@ int launch_batch_scan(const ScanPlan* plan, const std::vector<BinArgs>* full, in
 
     int sms = 0;
     if ((rc = sm_count(&sms))) return rc;
-    const unsigned sort_blocks = std::min<unsigned>((geo.nranges + kScanWarps - 1) / kScanWarps, (unsigned)sms * 8u);
+    // blocks per SM of the two event-ordered passes (measured at 1e7 events): the count pass is latency-bound and wants
+    // all the warps an SM holds, the scatter pass is bound by its write pattern and gets slower with more of them
+    const unsigned range_blocks = (geo.nranges + kScanWarps - 1) / kScanWarps;
+    const unsigned count_blocks = std::min<unsigned>(range_blocks, (unsigned)sms * 16u);
+    const unsigned sort_blocks = std::min<unsigned>(range_blocks, (unsigned)sms * 8u);
     const size_t smem_cnt = sizeof(unsigned int) * kScanWarps * (size_t)geo.ncells;
     const size_t smem_count = bin_table_bytes(n_bins) + smem_cnt;
     if (smem_count > 48 * 1024)
         CUDA_TRY(cudaFuncSetAttribute(scan_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_count));
     if (smem_cnt > 48 * 1024)
         CUDA_TRY(cudaFuncSetAttribute(scan_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cnt));
-    scan_count_kernel<<<sort_blocks, 32 * kScanWarps, smem_count, st>>>(E_true, E_reco, channel, n, energy_scale, bin_edges,
+    scan_count_kernel<<<count_blocks, 32 * kScanWarps, smem_count, st>>>(E_true, E_reco, channel, n, energy_scale, bin_edges,
                                                                         n_bins, geo, cellid, count);
     if ((rc = post_launch("osc_reweight_bin_batch (sort: count)"))) return rc;
     scan_offsets_cell_kernel<<<geo.ncells, 1024, 0, st>>>(count, geo, cell_begin);

@@ -622,53 +622,98 @@ void build_scan_plan(const osc_params* points, int n_points, ScanPlan& plan)
     }
 }
 
-// The sorted-event paths of the batched call: k4 (plan != nullptr: sub-groups of a scan grid) or k5 (full != nullptr:
-// one parameter block per point, every point its own eigen-problem).  Both sort the events by histogram cell, let
-// one warp own a piece of a cell, write partial[piece][point] and merge the pieces of every cell in order.
-int launch_batch_scan(const ScanPlan* plan, const std::vector<BinArgs>* full, int n_points, const double* E_true,
-                      const double* E_reco, const double* w0, const int8_t* channel, size_t n, double energy_scale,
-                      const double* bin_edges, int n_bins, double* hist_out, cudaStream_t st)
+// Events sorted by histogram cell and cut into pieces (osc_scan.cuh): what k4 and k5 work on.  The buffers belong
+// either to the stream-ordered scratch of one batched call or to an osc_plan.
+struct SortedEvents {
+    ScanGeom geo;              // range, nranges, piece, max_units, ncells (nsubs / subs_per_slot are set per run)
+    int n_bins = 0;
+    size_t n = 0;
+    unsigned int* cell_begin = nullptr;
+    unsigned int* unit_begin = nullptr;
+    double* sEt = nullptr;
+    double* sW = nullptr;
+};
+
+size_t sorted_bytes_cells(int ncells) { return round_up((size_t)(ncells + 1) * sizeof(unsigned int), 256); }
+size_t sorted_bytes_events(size_t n) { return round_up(n * sizeof(double), 256); }
+
+// Geometry of the sort for n events; `piece` as the caller wants it (multiple of 64).
+int sorted_geometry(size_t n, int n_bins, size_t piece, ScanGeom& geo)
 {
-    int rc;
-    if (n >= 0xFFFFFFFFull - 64) return fail(OSC_ERR_INVALID_ARG, "osc_reweight_bin_batch: n = %zu is more than one call takes", n);
-    ScanGeom geo;
+    if (n >= 0xFFFFFFFFull - 64) return fail(OSC_ERR_INVALID_ARG, "n = %zu events is more than one batched call takes", n);
     geo.ncells = kChannels * n_bins;
-    geo.nsubs = plan ? (int)plan->subs.size() : n_points;      // items a warp walks per piece: sub-groups or points
+    geo.nsubs = 0;
+    geo.subs_per_slot = 0;
     // warp ranges of the sort passes: short enough to give every SM dozens of warps (the passes are latency-bound),
     // long enough to keep the [ncells][nranges] count table below 64 MB
     const size_t max_ranges = std::min<size_t>(16384, (64u << 20) / (sizeof(unsigned int) * (size_t)geo.ncells));
     geo.range = round_up(std::max<size_t>(256, (n + max_ranges - 1) / max_ranges), 32);
     geo.nranges = (unsigned)((n + geo.range - 1) / geo.range);
+    geo.piece = (unsigned)piece;
+    geo.max_units = (unsigned)(n / piece + (size_t)geo.ncells + 1);
+    return OSC_OK;
+}
+
+// The three sort passes.  se's buffers are assigned by the caller; the temporaries come from a stream-ordered scratch.
+int scan_sort(const SortedEvents& se, const double* E_true, const double* E_reco, const double* w0, const int8_t* channel,
+              double energy_scale, const double* bin_edges, cudaStream_t st)
+{
+    int rc;
+    const ScanGeom& geo = se.geo;
+    const size_t b_cellid = round_up(se.n * sizeof(unsigned short), 256);
+    const size_t b_count = round_up((size_t)geo.ncells * geo.nranges * sizeof(unsigned int), 256);
+    Scratch tmp;
+    if ((rc = tmp.alloc(b_cellid + b_count, st))) return rc;
+    unsigned short* cellid = reinterpret_cast<unsigned short*>(tmp.p);
+    unsigned int* count = reinterpret_cast<unsigned int*>(tmp.p + b_cellid);
+    int sms = 0;
+    if ((rc = sm_count(&sms))) return rc;
+    // blocks per SM of the two event-ordered passes (measured at 1e7 events): the count pass is latency-bound and wants
+    // all the warps an SM holds, the scatter pass is bound by its write pattern and gets slower with more of them
+    const unsigned range_blocks = (geo.nranges + kScanWarps - 1) / kScanWarps;
+    const unsigned count_blocks = std::min<unsigned>(range_blocks, (unsigned)sms * 16u);
+    const unsigned sort_blocks = std::min<unsigned>(range_blocks, (unsigned)sms * 8u);
+    const size_t smem_cnt = sizeof(unsigned int) * kScanWarps * (size_t)geo.ncells;
+    const size_t smem_count = bin_table_bytes(se.n_bins) + smem_cnt;
+    if (smem_count > 48 * 1024)
+        CUDA_TRY(cudaFuncSetAttribute(scan_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_count));
+    if (smem_cnt > 48 * 1024)
+        CUDA_TRY(cudaFuncSetAttribute(scan_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cnt));
+    scan_count_kernel<<<count_blocks, 32 * kScanWarps, smem_count, st>>>(E_true, E_reco, channel, se.n, energy_scale,
+                                                                         bin_edges, se.n_bins, geo, cellid, count);
+    if ((rc = post_launch("sort of the events: count"))) return rc;
+    scan_offsets_cell_kernel<<<geo.ncells, 1024, 0, st>>>(count, geo, se.cell_begin);
+    if ((rc = post_launch("sort of the events: offsets per cell"))) return rc;
+    scan_offsets_kernel<<<1, 1024, 0, st>>>(geo, se.cell_begin, se.unit_begin);
+    if ((rc = post_launch("sort of the events: offsets"))) return rc;
+    scan_scatter_kernel<<<sort_blocks, 32 * kScanWarps, smem_cnt, st>>>(E_true, w0, cellid, se.n, geo, count, se.cell_begin,
+                                                                        se.sEt, se.sW);
+    return post_launch("sort of the events: scatter");
+}
+
+// The point kernels on sorted events: k4 (plan != nullptr: sub-groups of a scan grid) or k5 (full != nullptr: one
+// parameter block per point, every point its own eigen-problem), then the ordered merge of the pieces of every cell.
+int scan_run(const SortedEvents& se, const ScanPlan* plan, const std::vector<BinArgs>* full, int n_points,
+             double* hist_out, cudaStream_t st)
+{
+    int rc;
+    ScanGeom geo = se.geo;
+    geo.nsubs = plan ? (int)plan->subs.size() : n_points;      // items a warp walks per piece: sub-groups or points
     int slots = geo.nsubs < 8 ? geo.nsubs : 8;
     geo.subs_per_slot = (geo.nsubs + slots - 1) / slots;
     slots = (geo.nsubs + geo.subs_per_slot - 1) / geo.subs_per_slot;
-    size_t piece = round_up(n * (size_t)slots / 16384 + 1, 64);
-    if (piece < 128) piece = 128;
-    if (piece > (plan ? 8192u : 512u)) piece = plan ? 8192 : 512;   // k5 stages the piece in shared memory
-    geo.piece = (unsigned)piece;
-    geo.max_units = (unsigned)(n / piece + (size_t)geo.ncells + 1);
+    if (!plan && geo.piece > 512) return fail(OSC_ERR_INVALID_ARG, "internal: piece of %u events is too long for k5", geo.piece);
 
-    const size_t b_cellid = round_up(n * sizeof(unsigned short), 256);
-    const size_t b_count = round_up((size_t)geo.ncells * geo.nranges * sizeof(unsigned int), 256);
-    const size_t b_cells = round_up((size_t)(geo.ncells + 1) * sizeof(unsigned int), 256);
-    const size_t b_sorted = round_up(n * sizeof(double), 256);
     const size_t b_groups = plan ? round_up(plan->groups.size() * sizeof(ScanGroup), 256)
                                  : round_up((size_t)n_points * sizeof(BinArgs), 256);
     const size_t b_subs = plan ? round_up(plan->subs.size() * sizeof(ScanSub), 256) : 0;
     const size_t b_partial = round_up((size_t)geo.max_units * n_points * sizeof(double), 256);
     Scratch sc;
-    if ((rc = sc.alloc(b_cellid + b_count + 2 * b_cells + 2 * b_sorted + b_groups + b_subs + b_partial, st))) return rc;
-    char* q = sc.p;
-    unsigned short* cellid = reinterpret_cast<unsigned short*>(q); q += b_cellid;
-    unsigned int* count = reinterpret_cast<unsigned int*>(q); q += b_count;
-    unsigned int* cell_begin = reinterpret_cast<unsigned int*>(q); q += b_cells;
-    unsigned int* unit_begin = reinterpret_cast<unsigned int*>(q); q += b_cells;
-    double* sEt = reinterpret_cast<double*>(q); q += b_sorted;
-    double* sW = reinterpret_cast<double*>(q); q += b_sorted;
-    ScanGroup* d_groups = reinterpret_cast<ScanGroup*>(q); q += b_groups;
-    ScanSub* d_subs = reinterpret_cast<ScanSub*>(q); q += b_subs;
-    double* partial = reinterpret_cast<double*>(q);
-    // groups and sub-groups are contiguous on the device: one asynchronous copy from a pinned staging slot
+    if ((rc = sc.alloc(b_groups + b_subs + b_partial, st))) return rc;
+    ScanGroup* d_groups = reinterpret_cast<ScanGroup*>(sc.p);
+    ScanSub* d_subs = reinterpret_cast<ScanSub*>(sc.p + b_groups);
+    double* partial = reinterpret_cast<double*>(sc.p + b_groups + b_subs);
+    // the host-built tables are contiguous on the device: one asynchronous copy from a pinned staging slot
     PinnedRing* ring = nullptr;
     if ((rc = ring_for_device(&ring))) return rc;
     PinnedRing::Slot* slot = nullptr;
@@ -682,34 +727,11 @@ int launch_batch_scan(const ScanPlan* plan, const std::vector<BinArgs>* full, in
     CUDA_TRY(cudaMemcpyAsync(d_groups, slot->host, b_groups + b_subs, cudaMemcpyHostToDevice, st));
     if ((rc = ring->fence(slot, st))) return rc;
 
-    int sms = 0;
-    if ((rc = sm_count(&sms))) return rc;
-    // blocks per SM of the two event-ordered passes (measured at 1e7 events): the count pass is latency-bound and wants
-    // all the warps an SM holds, the scatter pass is bound by its write pattern and gets slower with more of them
-    const unsigned range_blocks = (geo.nranges + kScanWarps - 1) / kScanWarps;
-    const unsigned count_blocks = std::min<unsigned>(range_blocks, (unsigned)sms * 16u);
-    const unsigned sort_blocks = std::min<unsigned>(range_blocks, (unsigned)sms * 8u);
-    const size_t smem_cnt = sizeof(unsigned int) * kScanWarps * (size_t)geo.ncells;
-    const size_t smem_count = bin_table_bytes(n_bins) + smem_cnt;
-    if (smem_count > 48 * 1024)
-        CUDA_TRY(cudaFuncSetAttribute(scan_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_count));
-    if (smem_cnt > 48 * 1024)
-        CUDA_TRY(cudaFuncSetAttribute(scan_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cnt));
-    scan_count_kernel<<<count_blocks, 32 * kScanWarps, smem_count, st>>>(E_true, E_reco, channel, n, energy_scale, bin_edges,
-                                                                        n_bins, geo, cellid, count);
-    if ((rc = post_launch("osc_reweight_bin_batch (sort: count)"))) return rc;
-    scan_offsets_cell_kernel<<<geo.ncells, 1024, 0, st>>>(count, geo, cell_begin);
-    if ((rc = post_launch("osc_reweight_bin_batch (sort: offsets per cell)"))) return rc;
-    scan_offsets_kernel<<<1, 1024, 0, st>>>(geo, cell_begin, unit_begin);
-    if ((rc = post_launch("osc_reweight_bin_batch (sort: offsets)"))) return rc;
-    scan_scatter_kernel<<<sort_blocks, 32 * kScanWarps, smem_cnt, st>>>(E_true, w0, cellid, n, geo, count, cell_begin,
-                                                                        sEt, sW);
-    if ((rc = post_launch("osc_reweight_bin_batch (sort: scatter)"))) return rc;
     const dim3 grid((geo.max_units + kScanWarps - 1) / kScanWarps, (unsigned)slots);
     if (plan) {
-        scan_main_kernel<<<grid, 32 * kScanWarps, 0, st>>>(d_groups, d_subs, sEt, sW, cell_begin, unit_begin, geo, n_bins,
-                                                           n_points, partial);
-        if ((rc = post_launch("osc_reweight_bin_batch (scan, factorised)"))) return rc;
+        scan_main_kernel<<<grid, 32 * kScanWarps, 0, st>>>(d_groups, d_subs, se.sEt, se.sW, se.cell_begin, se.unit_begin,
+                                                           geo, se.n_bins, n_points, partial);
+        if ((rc = post_launch("batched reweighting on sorted events (k4, factorised)"))) return rc;
     } else {
         ChannelKinds kinds;
         for (int c = 0; c < kChannels; ++c) {
@@ -719,13 +741,39 @@ int launch_batch_scan(const ScanPlan* plan, const std::vector<BinArgs>* full, in
         }
         const size_t smem_ev = sizeof(double) * kScanWarps * 3 * (size_t)geo.piece;      // <= 48 kB at piece = 512
         scan_full_kernel<<<grid, 32 * kScanWarps, smem_ev, st>>>(reinterpret_cast<const double*>(d_groups), n_points,
-                                                                 geo.subs_per_slot, kinds, sEt, sW, cell_begin,
-                                                                 unit_begin, geo, n_bins, partial);
-        if ((rc = post_launch("osc_reweight_bin_batch (scan, one eigen-problem per point)"))) return rc;
+                                                                 geo.subs_per_slot, kinds, se.sEt, se.sW, se.cell_begin,
+                                                                 se.unit_begin, geo, se.n_bins, partial);
+        if ((rc = post_launch("batched reweighting on sorted events (k5, one eigen-problem per point)"))) return rc;
     }
     scan_merge_kernel<<<dim3((unsigned)geo.ncells, (unsigned)((n_points + 255) / 256)), 256, 0, st>>>(
-        partial, unit_begin, geo.ncells, n_points, hist_out);
-    return post_launch("osc_reweight_bin_batch (merge)");
+        partial, se.unit_begin, geo.ncells, n_points, hist_out);
+    return post_launch("batched reweighting on sorted events (merge)");
+}
+
+// One batched call: sort into a stream-ordered scratch, then run.
+int launch_batch_scan(const ScanPlan* plan, const std::vector<BinArgs>* full, int n_points, const double* E_true,
+                      const double* E_reco, const double* w0, const int8_t* channel, size_t n, double energy_scale,
+                      const double* bin_edges, int n_bins, double* hist_out, cudaStream_t st)
+{
+    int rc;
+    const int nsubs = plan ? (int)plan->subs.size() : n_points;
+    const int slots = nsubs < 8 ? nsubs : 8;
+    size_t piece = round_up(n * (size_t)slots / 16384 + 1, 64);
+    if (piece < 128) piece = 128;
+    if (piece > (plan ? 8192u : 512u)) piece = plan ? 8192 : 512;   // k5 stages the piece in shared memory
+    SortedEvents se;
+    se.n = n;
+    se.n_bins = n_bins;
+    if ((rc = sorted_geometry(n, n_bins, piece, se.geo))) return rc;
+    const size_t b_cells = sorted_bytes_cells(se.geo.ncells), b_ev = sorted_bytes_events(n);
+    Scratch sc;
+    if ((rc = sc.alloc(2 * b_cells + 2 * b_ev, st))) return rc;
+    se.cell_begin = reinterpret_cast<unsigned int*>(sc.p);
+    se.unit_begin = reinterpret_cast<unsigned int*>(sc.p + b_cells);
+    se.sEt = reinterpret_cast<double*>(sc.p + 2 * b_cells);
+    se.sW = reinterpret_cast<double*>(sc.p + 2 * b_cells + b_ev);
+    if ((rc = scan_sort(se, E_true, E_reco, w0, channel, energy_scale, bin_edges, st))) return rc;
+    return scan_run(se, plan, full, n_points, hist_out, st);
 }
 
 } // namespace

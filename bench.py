@@ -510,6 +510,36 @@ def main():
              "api": "osc_reweight_bin_scales: the three energy scales in one pass, closed form once per event; "
                     "same three histograms as the step behind `value`"}
 
+    # ---- the same three histograms from plans (osc_plan_*): events sorted by cell once per (sample, scale), outside
+    # the timed region; a step is osc_set_params + one osc_plan_reweight_bin per scale.  This is the Markov-chain use
+    # of the paper (same events, new parameters every step), reported beside `value`, not instead of it. ------------
+    plans = [osc.osc_plan_create(d_et, d_er, d_w0, d_ch, s, d_edges) for s in SCALES]
+
+    def step_plan():
+        osc.osc_set_params(**par)
+        for k, pl in enumerate(plans):
+            osc.osc_plan_reweight_bin(pl, hist_out=hist[k])
+        sharding.allreduce_hist(hist)
+
+    for _ in range(3):
+        step_plan()
+    barrier()
+    qs, qe = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    qs.record(stream)
+    for _ in range(args.steps):
+        step_plan()
+    qe.record(stream)
+    barrier()
+    p_ms = torch.tensor([qs.elapsed_time(qe)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(p_ms, op=dist.ReduceOp.MAX)
+    planned = {"value": world * n * len(SCALES) * args.steps / (float(p_ms.item()) * 1e-3), "unit": UNIT,
+               "ms_per_step": float(p_ms.item()) / args.steps,
+               "api": "osc_plan_reweight_bin on three plans (one per energy scale) built before the timed region: "
+                      "events pre-sorted by histogram cell, kernel k5 for one parameter set"}
+    for pl in plans:
+        osc.osc_plan_destroy(pl)
+
     # ---- fp64 peak probe in the same run (DFMA-only, register resident) ----------------------------------------
     probe_flops = osc.osc_fp64_peak_probe(1 << 14, 4)
     torch.cuda.synchronize()
@@ -598,7 +628,7 @@ def main():
                    "l2": "inputs (250 MB per pass) larger than L2 (126 MB); no explicit flush",
                    "parallelism": f"events sharded over {world} GPU(s); histogram all-reduce" if world > 1 else "1 GPU"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
-        "fused_scales": fused,
+        "fused_scales": fused, "planned": planned,
     }
     print(json.dumps(out))
     if world > 1:

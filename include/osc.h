@@ -142,6 +142,28 @@ int osc_reweight_bin_batch(const osc_params *points, int n_points, const double 
                            double energy_scale, const double *bin_edges, int n_bins, double *hist_out,
                            void *stream);
 
+/* Plans: the same histograms for callers that keep the event sample, the energy scale and the binning fixed
+ * over many calls -- the Markov chain of the paper's toy fit proposes new oscillation parameters at every step
+ * and rebuilds the PDF from the same simulated events.  osc_plan_create sorts the events by
+ * histogram cell once (the sort of osc_reweight_bin_batch, kept on the device: 16 bytes per event); the
+ * reweight calls then run the sorted-event kernels only: no bin search and no shared-memory histogram per
+ * call, the weights of a cell are summed in registers.
+ *   osc_plan_create              arguments as osc_reweight_bin; *plan_out receives the plan.  The caller's event
+ *                                arrays are not needed once the work enqueued on `stream` has run.
+ *   osc_plan_reweight_bin        hist_out DEVICE [OSC_N_CHANNELS][n_bins], OVERWRITTEN; parameters of osc_set_params;
+ *                                equals osc_reweight_bin on the planned events to rounding (order of additions)
+ *   osc_plan_reweight_bin_batch  hist_out DEVICE [n_points][OSC_N_CHANNELS][n_bins]; as osc_reweight_bin_batch
+ *   osc_plan_destroy             frees the plan (synchronises with work that still reads it); NULL is a no-op
+ * A plan belongs to the device that was current at creation.  Calls that use a plan must be ordered after its
+ * creation (same stream, or a synchronisation in between).  Results are bit-reproducible from run to run. */
+typedef struct osc_plan osc_plan;
+int osc_plan_create(const double *E_true, const double *E_reco, const double *w0, const int8_t *channel, size_t n,
+                    double energy_scale, const double *bin_edges, int n_bins, void *stream, osc_plan **plan_out);
+int osc_plan_reweight_bin(const osc_plan *plan, double *hist_out, void *stream);
+int osc_plan_reweight_bin_batch(const osc_plan *plan, const osc_params *points, int n_points, double *hist_out,
+                                void *stream);
+int osc_plan_destroy(osc_plan *plan);
+
 /* Binned Poisson likelihood of rebuilt PDFs against a data histogram (PAPER.md:125-128,
  * eq. 2.1, read as a product of Poisson probabilities of the bin contents -- DESIGN.md R5):
  *     out[p] = -2 ln lambda_p = 2 sum_i [ mu - D_i + D_i ln(D_i / mu) ],   mu = norm * hist[p][i],

@@ -24,6 +24,7 @@ PARAM_FIELDS = ("sin2_th12", "sin2_th23", "sin2_th13", "dm2_32", "dm2_21", "delt
 
 # every symbol include/osc.h declares (tests/test_abi.py checks the header against this list)
 EXPORTS = ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_scales", "osc_reweight_bin_batch",
+           "osc_plan_create", "osc_plan_reweight_bin", "osc_plan_reweight_bin_batch", "osc_plan_destroy",
            "osc_neg2lnl", "osc_bin_centre_compare", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_reweight_bin_scales_host", "osc_last_error", "osc_launch_count",
            "osc_version", "osc_set_device", "osc_get_device", "osc_fp64_peak_probe")
 
@@ -60,6 +61,10 @@ def lib() -> ctypes.CDLL:
     L.osc_reweight_bin_batch.argtypes = [ctypes.POINTER(osc_params), i, _dp, _dp, _dp, _dp, sz, d, _dp, i, _dp, vp]
     L.osc_bin_index.argtypes = [_dp, _dp, _dp, sz, d, _dp, i, _dp, vp]
     L.osc_neg2lnl.argtypes = [_dp, i, i, _dp, d, _dp, vp]
+    L.osc_plan_create.argtypes = [_dp, _dp, _dp, _dp, sz, d, _dp, i, vp, ctypes.POINTER(vp)]
+    L.osc_plan_reweight_bin.argtypes = [vp, _dp, vp]
+    L.osc_plan_reweight_bin_batch.argtypes = [vp, ctypes.POINTER(osc_params), i, _dp, vp]
+    L.osc_plan_destroy.argtypes = [vp]
     L.osc_bin_centre_compare.argtypes = [_dp, _dp, _dp, sz, _dp, i, _dp, _dp, vp]
     L.osc_prob_host.argtypes = [_dp, sz, i, i, i, _dp]
     L.osc_reweight_bin_host.argtypes = [_dp, _dp, _dp, _dp, sz, d, _dp, i, _dp]
@@ -69,6 +74,7 @@ def lib() -> ctypes.CDLL:
     L.osc_fp64_peak_probe.argtypes = [i, i, ctypes.POINTER(d), vp]
     for name in ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_scales",
                  "osc_reweight_bin_batch",
+                 "osc_plan_create", "osc_plan_reweight_bin", "osc_plan_reweight_bin_batch", "osc_plan_destroy",
                  "osc_neg2lnl", "osc_bin_centre_compare", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_reweight_bin_scales_host", "osc_set_device",
                  "osc_get_device",
                  "osc_fp64_peak_probe"):
@@ -233,6 +239,64 @@ def osc_reweight_bin_batch(points: Sequence, E_true, E_reco, w0, channel, energy
                                         _dev(bin_edges, torch.float64, "bin_edges"), nb,
                                         _dev(hist_out, torch.float64, "hist_out"), _stream(stream)))
     return hist_out
+
+
+class OscPlan:
+    """Handle of an ``osc_plan`` (include/osc.h) plus what the binding needs to size outputs.  Destroyed with
+    ``osc_plan_destroy`` (or when the object is collected)."""
+
+    def __init__(self, ptr: int, n_bins: int, device):
+        self.ptr, self.n_bins, self.device = ptr, n_bins, device
+
+    def __del__(self):
+        try:
+            osc_plan_destroy(self)
+        except Exception:
+            pass
+
+
+def osc_plan_create(E_true, E_reco, w0, channel, energy_scale: float, bin_edges, stream=None) -> OscPlan:
+    import torch
+
+    n, pt, pr, pw, pc = _event_ptrs(E_true, E_reco, w0, channel)
+    nb = bin_edges.numel() - 1
+    out = ctypes.c_void_p()
+    _check(lib().osc_plan_create(pt, pr, pw, pc, n, float(energy_scale), _dev(bin_edges, torch.float64, "bin_edges"), nb,
+                                 _stream(stream), ctypes.byref(out)))
+    return OscPlan(out.value, nb, E_true.device)
+
+
+def osc_plan_reweight_bin(plan: OscPlan, hist_out=None, stream=None):
+    """[N_CHANNELS, n_bins] histogram of the planned events with the parameters of osc_set_params."""
+    import torch
+
+    if hist_out is None:
+        hist_out = torch.empty((N_CHANNELS, plan.n_bins), dtype=torch.float64, device=plan.device)
+    if hist_out.numel() != N_CHANNELS * plan.n_bins:
+        raise ValueError("hist_out must hold N_CHANNELS * n_bins values")
+    _check(lib().osc_plan_reweight_bin(plan.ptr, _dev(hist_out, torch.float64, "hist_out"), _stream(stream)))
+    return hist_out
+
+
+def osc_plan_reweight_bin_batch(plan: OscPlan, points: Sequence, hist_out=None, stream=None):
+    """[n_points, N_CHANNELS, n_bins] histograms of the planned events, one slice per parameter set."""
+    import torch
+
+    npts = len(points)
+    arr = points if isinstance(points, ctypes.Array) else pack_params(points)
+    if hist_out is None:
+        hist_out = torch.empty((npts, N_CHANNELS, plan.n_bins), dtype=torch.float64, device=plan.device)
+    if hist_out.numel() != npts * N_CHANNELS * plan.n_bins:
+        raise ValueError("hist_out must hold n_points * N_CHANNELS * n_bins values")
+    _check(lib().osc_plan_reweight_bin_batch(plan.ptr, arr, npts, _dev(hist_out, torch.float64, "hist_out"),
+                                             _stream(stream)))
+    return hist_out
+
+
+def osc_plan_destroy(plan: OscPlan) -> None:
+    if plan is not None and plan.ptr:
+        ptr, plan.ptr = plan.ptr, None
+        _check(lib().osc_plan_destroy(ptr))
 
 
 def osc_neg2lnl(hist, data, norm: float = 1.0, out=None, stream=None):

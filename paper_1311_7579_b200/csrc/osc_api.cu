@@ -11,6 +11,7 @@
 #include <complex>
 #include <map>
 #include <mutex>
+#include <new>
 #include <utility>
 #include <vector>
 
@@ -630,12 +631,14 @@ struct SortedEvents {
     size_t n = 0;
     unsigned int* cell_begin = nullptr;
     unsigned int* unit_begin = nullptr;
+    unsigned short* unit_cell = nullptr;   // [max_units]
     double* sEt = nullptr;
     double* sW = nullptr;
 };
 
 size_t sorted_bytes_cells(int ncells) { return round_up((size_t)(ncells + 1) * sizeof(unsigned int), 256); }
 size_t sorted_bytes_events(size_t n) { return round_up(n * sizeof(double), 256); }
+size_t sorted_bytes_units(unsigned max_units) { return round_up((size_t)max_units * sizeof(unsigned short), 256); }
 
 // Geometry of the sort for n events; `piece` as the caller wants it (multiple of 64).
 int sorted_geometry(size_t n, int n_bins, size_t piece, ScanGeom& geo)
@@ -684,7 +687,7 @@ int scan_sort(const SortedEvents& se, const double* E_true, const double* E_reco
     if ((rc = post_launch("sort of the events: count"))) return rc;
     scan_offsets_cell_kernel<<<geo.ncells, 1024, 0, st>>>(count, geo, se.cell_begin);
     if ((rc = post_launch("sort of the events: offsets per cell"))) return rc;
-    scan_offsets_kernel<<<1, 1024, 0, st>>>(geo, se.cell_begin, se.unit_begin);
+    scan_offsets_kernel<<<1, 1024, 0, st>>>(geo, se.cell_begin, se.unit_begin, se.unit_cell);
     if ((rc = post_launch("sort of the events: offsets"))) return rc;
     scan_scatter_kernel<<<sort_blocks, 32 * kScanWarps, smem_cnt, st>>>(E_true, w0, cellid, se.n, geo, count, se.cell_begin,
                                                                         se.sEt, se.sW);
@@ -730,7 +733,7 @@ int scan_run(const SortedEvents& se, const ScanPlan* plan, const std::vector<Bin
     const dim3 grid((geo.max_units + kScanWarps - 1) / kScanWarps, (unsigned)slots);
     if (plan) {
         scan_main_kernel<<<grid, 32 * kScanWarps, 0, st>>>(d_groups, d_subs, se.sEt, se.sW, se.cell_begin, se.unit_begin,
-                                                           geo, se.n_bins, n_points, partial);
+                                                           se.unit_cell, geo, se.n_bins, n_points, partial);
         if ((rc = post_launch("batched reweighting on sorted events (k4, factorised)"))) return rc;
     } else {
         ChannelKinds kinds;
@@ -739,14 +742,23 @@ int scan_run(const SortedEvents& se, const ScanPlan* plan, const std::vector<Bin
             channel_def(c, fin, fout, anti);
             kinds.k[c] = fin != fout ? 3 : (fin == 0 ? 1 : 2);
         }
-        const size_t smem_ev = sizeof(double) * kScanWarps * 3 * (size_t)geo.piece;      // <= 48 kB at piece = 512
-        scan_full_kernel<<<grid, 32 * kScanWarps, smem_ev, st>>>(reinterpret_cast<const double*>(d_groups), n_points,
-                                                                 geo.subs_per_slot, kinds, se.sEt, se.sW, se.cell_begin,
-                                                                 se.unit_begin, geo, se.n_bins, partial);
+        if (geo.subs_per_slot > 2) {          // a piece is staged in shared memory once and walked by many points
+            const size_t smem_ev = sizeof(double) * kScanWarps * 3 * (size_t)geo.piece;  // <= 48 kB at piece = 512
+            scan_full_kernel<true><<<grid, 32 * kScanWarps, smem_ev, st>>>(
+                reinterpret_cast<const double*>(d_groups), n_points, geo.subs_per_slot, kinds, se.sEt, se.sW,
+                se.cell_begin, se.unit_begin, se.unit_cell, geo, se.n_bins, partial);
+        } else {                              // one or two points per piece: straight from the sorted arrays
+            scan_full_kernel<false><<<grid, 32 * kScanWarps, 0, st>>>(
+                reinterpret_cast<const double*>(d_groups), n_points, geo.subs_per_slot, kinds, se.sEt, se.sW,
+                se.cell_begin, se.unit_begin, se.unit_cell, geo, se.n_bins, partial);
+        }
         if ((rc = post_launch("batched reweighting on sorted events (k5, one eigen-problem per point)"))) return rc;
     }
-    scan_merge_kernel<<<dim3((unsigned)geo.ncells, (unsigned)((n_points + 255) / 256)), 256, 0, st>>>(
-        partial, se.unit_begin, geo.ncells, n_points, hist_out);
+    if (n_points < 32)
+        scan_merge_few_kernel<<<geo.ncells, 256, 0, st>>>(partial, se.unit_begin, geo.ncells, n_points, hist_out);
+    else
+        scan_merge_kernel<<<dim3((unsigned)geo.ncells, (unsigned)((n_points + 255) / 256)), 256, 0, st>>>(
+            partial, se.unit_begin, geo.ncells, n_points, hist_out);
     return post_launch("batched reweighting on sorted events (merge)");
 }
 
@@ -766,14 +778,30 @@ int launch_batch_scan(const ScanPlan* plan, const std::vector<BinArgs>* full, in
     se.n_bins = n_bins;
     if ((rc = sorted_geometry(n, n_bins, piece, se.geo))) return rc;
     const size_t b_cells = sorted_bytes_cells(se.geo.ncells), b_ev = sorted_bytes_events(n);
+    const size_t b_units = sorted_bytes_units(se.geo.max_units);
     Scratch sc;
-    if ((rc = sc.alloc(2 * b_cells + 2 * b_ev, st))) return rc;
+    if ((rc = sc.alloc(2 * b_cells + 2 * b_ev + b_units, st))) return rc;
     se.cell_begin = reinterpret_cast<unsigned int*>(sc.p);
     se.unit_begin = reinterpret_cast<unsigned int*>(sc.p + b_cells);
     se.sEt = reinterpret_cast<double*>(sc.p + 2 * b_cells);
     se.sW = reinterpret_cast<double*>(sc.p + 2 * b_cells + b_ev);
+    se.unit_cell = reinterpret_cast<unsigned short*>(sc.p + 2 * b_cells + 2 * b_ev);
     if ((rc = scan_sort(se, E_true, E_reco, w0, channel, energy_scale, bin_edges, st))) return rc;
     return scan_run(se, plan, full, n_points, hist_out, st);
+}
+
+// An osc_plan: the sorted events of one (event sample, energy scale, binning), kept on the device.
+struct PlanImpl {
+    unsigned long long magic = 0x6F73635F706C616EULL;   // "osc_plan"
+    int device = 0;
+    SortedEvents se;
+    char* buf = nullptr;
+};
+
+PlanImpl* plan_cast(const void* p)
+{
+    PlanImpl* q = static_cast<PlanImpl*>(const_cast<void*>(p));
+    return (q && q->magic == 0x6F73635F706C616EULL) ? q : nullptr;
 }
 
 } // namespace
@@ -866,6 +894,136 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
                                   hist_out + (size_t)p * nh, st)))
             return rc;
     return OSC_OK;
+}
+
+int osc_plan_create(const double* E_true, const double* E_reco, const double* w0, const int8_t* channel, size_t n,
+                    double energy_scale, const double* bin_edges, int n_bins, void* stream, osc_plan** plan_out)
+{
+    if (!plan_out) return fail(OSC_ERR_INVALID_ARG, "null plan_out");
+    *plan_out = nullptr;
+    double dummy;
+    int rc = check_bin_args(E_true, E_reco, w0, channel, n, energy_scale, bin_edges, n_bins, &dummy);
+    if (rc) return rc;
+    if (n > 0 && !w0) return fail(OSC_ERR_INVALID_ARG, "null w0 with n > 0");
+    PlanImpl* pl = new (std::nothrow) PlanImpl;
+    if (!pl) return fail(OSC_ERR_CUDA, "out of host memory");
+    cudaError_t e = cudaGetDevice(&pl->device);
+    if (e != cudaSuccess) {
+        delete pl;
+        return fail(OSC_ERR_CUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+    }
+    SortedEvents& se = pl->se;
+    se.n = n;
+    se.n_bins = n_bins;
+    // pieces short enough for k5 (it stages a piece in shared memory) and for a single parameter set to fill the GPU
+    size_t piece = round_up(n / 16384 + 1, 64);
+    if (piece < 128) piece = 128;
+    if (piece > 512) piece = 512;
+    if ((rc = sorted_geometry(n, n_bins, piece, se.geo))) {
+        delete pl;
+        return rc;
+    }
+    const size_t b_cells = sorted_bytes_cells(se.geo.ncells), b_ev = sorted_bytes_events(n);
+    const size_t b_units = sorted_bytes_units(se.geo.max_units);
+    e = cudaMalloc((void**)&pl->buf, 2 * b_cells + 2 * b_ev + b_units + 256);
+    if (e != cudaSuccess) {
+        delete pl;
+        return fail(OSC_ERR_CUDA, "cudaMalloc of the plan (%zu bytes): %s", 2 * b_cells + 2 * b_ev, cudaGetErrorString(e));
+    }
+    se.cell_begin = reinterpret_cast<unsigned int*>(pl->buf);
+    se.unit_begin = reinterpret_cast<unsigned int*>(pl->buf + b_cells);
+    se.sEt = reinterpret_cast<double*>(pl->buf + 2 * b_cells);
+    se.sW = reinterpret_cast<double*>(pl->buf + 2 * b_cells + b_ev);
+    se.unit_cell = reinterpret_cast<unsigned short*>(pl->buf + 2 * b_cells + 2 * b_ev);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (n == 0) {
+        e = cudaMemsetAsync(pl->buf, 0, 2 * b_cells, st);       // no event, no piece
+        rc = e == cudaSuccess ? OSC_OK : fail(OSC_ERR_CUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e));
+    } else {
+        rc = scan_sort(se, E_true, E_reco, w0, channel, energy_scale, bin_edges, st);
+    }
+    if (rc) {
+        cudaFree(pl->buf);
+        delete pl;
+        return rc;
+    }
+    *plan_out = reinterpret_cast<osc_plan*>(pl);
+    return OSC_OK;
+}
+
+int osc_plan_destroy(osc_plan* plan)
+{
+    if (!plan) return OSC_OK;
+    PlanImpl* pl = plan_cast(plan);
+    if (!pl) return fail(OSC_ERR_INVALID_ARG, "not an osc_plan");
+    pl->magic = 0;
+    cudaError_t e = cudaFree(pl->buf);              // synchronises with the work that still reads the plan
+    delete pl;
+    if (e != cudaSuccess) return fail(OSC_ERR_CUDA, "cudaFree: %s", cudaGetErrorString(e));
+    return OSC_OK;
+}
+
+int osc_plan_reweight_bin_batch(const osc_plan* plan, const osc_params* points, int n_points, double* hist_out,
+                                void* stream)
+{
+    PlanImpl* pl = plan_cast(plan);
+    if (!pl) return fail(OSC_ERR_INVALID_ARG, "not an osc_plan");
+    if (n_points < 0) return fail(OSC_ERR_INVALID_ARG, "n_points < 0");
+    if (n_points == 0) return OSC_OK;
+    if (!points || !hist_out) return fail(OSC_ERR_INVALID_ARG, "null points or hist_out");
+    if (!aligned(hist_out, 8)) return fail(OSC_ERR_ALIGNMENT, "hist_out not 8-byte aligned");
+    for (int p = 0; p < n_points; ++p)
+        if (const char* msg = check_params(points[p]))
+            return fail(OSC_ERR_INVALID_ARG, "osc_plan_reweight_bin_batch: point %d: %s", p, msg);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    // same choice between the factorised kernel k4 and the one-eigen-problem-per-point kernel k5 as in
+    // osc_reweight_bin_batch; the sort is already paid for, so there is no k2 branch
+    ScanPlan sp;
+    build_scan_plan(points, n_points, sp);
+    bool use_scan = (size_t)n_points >= 8 * sp.subs.size();
+    if (const char* e = getenv("OSC_BATCH_PATH")) {
+        if (!std::strcmp(e, "k4")) use_scan = true;
+        if (!std::strcmp(e, "k5")) use_scan = false;
+    }
+    if (use_scan) return scan_run(pl->se, &sp, nullptr, n_points, hist_out, st);
+    std::vector<BinArgs> blocks((size_t)n_points);
+    for (int p = 0; p < n_points; ++p) {
+        HostSet h;
+        precompute(points[p], h);
+        make_bin_args(h, blocks[(size_t)p]);
+    }
+    return scan_run(pl->se, nullptr, &blocks, n_points, hist_out, st);
+}
+
+int osc_plan_reweight_bin(const osc_plan* plan, double* hist_out, void* stream)
+{
+    PlanImpl* pl = plan_cast(plan);
+    if (!pl) return fail(OSC_ERR_INVALID_ARG, "not an osc_plan");
+    if (!hist_out) return fail(OSC_ERR_INVALID_ARG, "null hist_out");
+    if (!aligned(hist_out, 8)) return fail(OSC_ERR_ALIGNMENT, "hist_out not 8-byte aligned");
+    HostSet h;
+    int rc = snapshot(h);
+    if (rc) return rc;
+    BinArgs args;
+    make_bin_args(h, args);
+    // one parameter set: parameter block by value, partial sums in the per-stream scratch of the library -- two
+    // launches and nothing else on the stream
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const SortedEvents& se = pl->se;
+    char* scratch = nullptr;
+    if ((rc = stream_scratch(kCounterBytes + (size_t)se.geo.max_units * sizeof(double), st, &scratch))) return rc;
+    double* partial = reinterpret_cast<double*>(scratch + kCounterBytes);
+    ChannelKinds kinds;
+    for (int c = 0; c < kChannels; ++c) {
+        int fin, fout, anti;
+        channel_def(c, fin, fout, anti);
+        kinds.k[c] = fin != fout ? 3 : (fin == 0 ? 1 : 2);
+    }
+    scan_full_one_kernel<<<(se.geo.max_units + kScanWarps - 1) / kScanWarps, 32 * kScanWarps, 0, st>>>(
+        args, kinds, se.sEt, se.sW, se.cell_begin, se.unit_begin, se.unit_cell, se.geo, se.n_bins, partial);
+    if ((rc = post_launch("osc_plan_reweight_bin (k5, one parameter set)"))) return rc;
+    scan_merge_few_kernel<<<se.geo.ncells, 256, 0, st>>>(partial, se.unit_begin, se.geo.ncells, 1, hist_out);
+    return post_launch("osc_plan_reweight_bin (merge)");
 }
 
 int osc_bin_centre_compare(const double* E_true, const double* w0, const int8_t* channel, size_t n,

@@ -174,9 +174,11 @@ scan_offsets_cell_kernel(unsigned int* __restrict__ count, ScanGeom geo, unsigne
 
 // Sort pass 2b (one block of 1024 threads): cell_begin[c] = first sorted position of cell c (cell_begin[ncells] =
 // number of kept events; on entry cell_begin[c] holds the cell's total); unit_begin[c] = index of the first piece of
-// cell c (unit_begin[ncells] = number of pieces).  At most 3 cells per thread (ncells <= 4 * 768).
+// cell c (unit_begin[ncells] = number of pieces), unit_cell[u] = cell of piece u.  At most 3 cells per thread
+// (ncells <= 4 * 768).
 __global__ void __launch_bounds__(1024)
-scan_offsets_kernel(ScanGeom geo, unsigned int* __restrict__ cell_begin, unsigned int* __restrict__ unit_begin)
+scan_offsets_kernel(ScanGeom geo, unsigned int* __restrict__ cell_begin, unsigned int* __restrict__ unit_begin,
+                    unsigned short* __restrict__ unit_cell)
 {
     __shared__ unsigned s_warp[33];
     const int cper = (geo.ncells + 1023) / 1024;
@@ -195,7 +197,9 @@ scan_offsets_kernel(ScanGeom geo, unsigned int* __restrict__ cell_begin, unsigne
         cell_begin[c] = run;
         unit_begin[c] = urun;
         run += len[c - c0];
-        urun += (len[c - c0] + geo.piece - 1) / geo.piece;
+        const unsigned np_c = (len[c - c0] + geo.piece - 1) / geo.piece;
+        for (unsigned k = 0; k < np_c; ++k) unit_cell[urun + k] = (unsigned short)c;     // cell of every piece
+        urun += np_c;
     }
     if (threadIdx.x == 0) {
         cell_begin[geo.ncells] = total;
@@ -331,21 +335,15 @@ __device__ __forceinline__ void scan_phase_b(uint32_t slice, int cnt, const doub
 __global__ void __launch_bounds__(32 * kScanWarps)
 scan_main_kernel(const ScanGroup* __restrict__ groups, const ScanSub* __restrict__ subs,
                  const double* __restrict__ sEt, const double* __restrict__ sW,
-                 const unsigned int* __restrict__ cell_begin, const unsigned int* __restrict__ unit_begin, ScanGeom geo,
-                 int nb, int npoints, double* __restrict__ partial)
+                 const unsigned int* __restrict__ cell_begin, const unsigned int* __restrict__ unit_begin,
+                 const unsigned short* __restrict__ unit_cell, ScanGeom geo, int nb, int npoints,
+                 double* __restrict__ partial)
 {
     __shared__ __align__(16) double s_slice[kScanWarps][kSliceEvents][kSliceDoubles];
     const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const unsigned u = blockIdx.x * kScanWarps + warp;
     if (u >= __ldg(unit_begin + geo.ncells)) return;
-    // cell of piece u: the largest c with unit_begin[c] <= u (uniform binary search; empty cells share a value
-    // with their successor and are skipped by taking the largest)
-    int lo = 0, hi = geo.ncells - 1;
-    while (lo < hi) {
-        const int mid = (lo + hi + 1) >> 1;
-        if (__ldg(unit_begin + mid) <= u) lo = mid; else hi = mid - 1;
-    }
-    const int cell = lo;
+    const int cell = (int)__ldg(unit_cell + u);
     const unsigned cb = __ldg(cell_begin + cell), ce = __ldg(cell_begin + cell + 1);
     const unsigned begin = cb + (u - __ldg(unit_begin + cell)) * geo.piece;
     const unsigned end = min(ce, begin + geo.piece);
@@ -440,7 +438,9 @@ struct ChannelKinds {
 // from inside the warp); padding slots carry E = 1, w0 = 0.  Fixed summation order: deterministic.
 constexpr int kFullUnroll = 4;
 
-template <int KIND>
+// STAGED: the events come from the warp's shared-memory copy (E, 1/E, w0); otherwise straight from the sorted arrays
+// in global memory with 1/E taken here -- for one or two points per piece the staging pass costs more than it saves.
+template <int KIND, bool STAGED>
 __device__ __forceinline__ double full_piece_sum(const OscSet& set, const OscTrans& tr, const double* sE,
                                                  const double* sI, const double* sW, int len, unsigned lane)
 {
@@ -454,10 +454,19 @@ __device__ __forceinline__ double full_piece_sum(const OscSet& set, const OscTra
         for (int k = 0; k < kFullUnroll; ++k) {
             const int j = i + 32 * k;
             const bool has = j < len;
-            E[k] = has ? sE[j] : 1.0;
-            I[k] = has ? sI[j] : 1.0;
-            w[k] = has ? sW[j] : 0.0;
+            if (STAGED) {
+                E[k] = has ? sE[j] : 1.0;
+                I[k] = has ? sI[j] : 1.0;
+                w[k] = has ? sW[j] : 0.0;
+            } else {
+                E[k] = has ? __ldg(sE + j) : 1.0;
+                w[k] = has ? __ldg(sW + j) : 0.0;
+            }
             A[k] = tr.sa * E[k];
+        }
+        if (!STAGED) {
+#pragma unroll
+            for (int k = 0; k < kFullUnroll; ++k) I[k] = rcp_pos(E[k]);
         }
 #pragma unroll
         for (int k = 0; k < kFullUnroll; ++k) eig_solve(set, A[k], I[k], e[k]);
@@ -470,37 +479,41 @@ __device__ __forceinline__ double full_piece_sum(const OscSet& set, const OscTra
     return s;
 }
 
+template <bool STAGED>
 __global__ void __launch_bounds__(32 * kScanWarps, 3)
 scan_full_kernel(const double* __restrict__ points, int npoints, int pts_per_slot, const ChannelKinds kinds,
                  const double* __restrict__ sEt, const double* __restrict__ sW,
-                 const unsigned int* __restrict__ cell_begin, const unsigned int* __restrict__ unit_begin, ScanGeom geo,
-                 int nb, double* __restrict__ partial)
+                 const unsigned int* __restrict__ cell_begin, const unsigned int* __restrict__ unit_begin,
+                 const unsigned short* __restrict__ unit_cell, ScanGeom geo, int nb, double* __restrict__ partial)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const unsigned u = blockIdx.x * kScanWarps + warp;
     if (u >= __ldg(unit_begin + geo.ncells)) return;
-    int lo = 0, hi = geo.ncells - 1;                         // cell of piece u, as in scan_main_kernel
-    while (lo < hi) {
-        const int mid = (lo + hi + 1) >> 1;
-        if (__ldg(unit_begin + mid) <= u) lo = mid; else hi = mid - 1;
-    }
-    const int cell = lo;
+    const int cell = (int)__ldg(unit_cell + u);
     const unsigned cb = __ldg(cell_begin + cell), ce = __ldg(cell_begin + cell + 1);
     const unsigned begin = cb + (u - __ldg(unit_begin + cell)) * geo.piece;
     const int len = (int)(min(ce, begin + geo.piece) - begin);
     const int ch = cell / nb;
 
-    double* sE = reinterpret_cast<double*>(smem_raw) + (size_t)warp * 3 * geo.piece;
-    double* sI = sE + geo.piece;
-    double* sWt = sI + geo.piece;
-    for (int i = lane; i < len; i += 32) {
-        const double E = __ldg(sEt + begin + i);
-        sE[i] = E;
-        sI[i] = rcp_pos(E);
-        sWt[i] = __ldg(sW + begin + i);
+    const double* sE = sEt + begin;
+    const double* sI = nullptr;
+    const double* sWt = sW + begin;
+    if (STAGED) {
+        double* tE = reinterpret_cast<double*>(smem_raw) + (size_t)warp * 3 * geo.piece;
+        double* tI = tE + geo.piece;
+        double* tW = tI + geo.piece;
+        for (int i = lane; i < len; i += 32) {
+            const double E = __ldg(sEt + begin + i);
+            tE[i] = E;
+            tI[i] = rcp_pos(E);
+            tW[i] = __ldg(sW + begin + i);
+        }
+        __syncwarp();
+        sE = tE;
+        sI = tI;
+        sWt = tW;
     }
-    __syncwarp();
 
     const int p_begin = blockIdx.y * pts_per_slot, p_end = min(npoints, p_begin + pts_per_slot);
     const int kind = kinds.k[ch];
@@ -525,12 +538,52 @@ scan_full_kernel(const double* __restrict__ points, int npoints, int pts_per_slo
         tr.T2i1 = __ldg(tb + 8);
         tr.pad = 0.0;
         double s;
-        if (kind == 2) s = full_piece_sum<2>(set, tr, sE, sI, sWt, len, lane);
-        else if (kind == 3) s = full_piece_sum<3>(set, tr, sE, sI, sWt, len, lane);
-        else if (kind == 1) s = full_piece_sum<1>(set, tr, sE, sI, sWt, len, lane);
-        else s = full_piece_sum<0>(set, tr, sE, sI, sWt, len, lane);
+        if (kind == 2) s = full_piece_sum<2, STAGED>(set, tr, sE, sI, sWt, len, lane);
+        else if (kind == 3) s = full_piece_sum<3, STAGED>(set, tr, sE, sI, sWt, len, lane);
+        else if (kind == 1) s = full_piece_sum<1, STAGED>(set, tr, sE, sI, sWt, len, lane);
+        else s = full_piece_sum<0, STAGED>(set, tr, sE, sI, sWt, len, lane);
         if (lane == 0) partial[(size_t)u * npoints + p] = s;
     }
+}
+
+// k5 for ONE parameter set (osc_plan_reweight_bin): the parameter block travels as a kernel parameter, as in k2, so
+// the call is two launches and nothing else on the stream (no table upload, no per-call allocation).
+__global__ void __launch_bounds__(32 * kScanWarps, 3)
+scan_full_one_kernel(const __grid_constant__ BinArgs a, const ChannelKinds kinds, const double* __restrict__ sEt,
+                     const double* __restrict__ sW, const unsigned int* __restrict__ cell_begin,
+                     const unsigned int* __restrict__ unit_begin, const unsigned short* __restrict__ unit_cell,
+                     ScanGeom geo, int nb, double* __restrict__ partial)
+{
+    const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const unsigned u = blockIdx.x * kScanWarps + warp;
+    if (u >= __ldg(unit_begin + geo.ncells)) return;
+    const int cell = (int)__ldg(unit_cell + u);
+    const unsigned cb = __ldg(cell_begin + cell), ce = __ldg(cell_begin + cell + 1);
+    const unsigned begin = cb + (u - __ldg(unit_begin + cell)) * geo.piece;
+    const int len = (int)(min(ce, begin + geo.piece) - begin);
+    const int ch = cell / nb;
+    const int kind = kinds.k[ch];
+    // the channel is warp-uniform: copy its transition block out of the parameter space once
+    OscTrans tr;
+    const double* tb = reinterpret_cast<const double*>(&a.ch[0]) + ch * kTransDoubles;
+    tr.sa = tb[0];
+    tr.delta = tb[1];
+    tr.ee = tb[2];
+    tr.Tr0 = tb[3];
+    tr.Ti0 = tb[4];
+    tr.T2r0 = tb[5];
+    tr.T2i0 = tb[6];
+    tr.T2r1 = tb[7];
+    tr.T2i1 = tb[8];
+    tr.pad = 0.0;
+    const double* sE = sEt + begin;
+    const double* sWt = sW + begin;
+    double s;
+    if (kind == 2) s = full_piece_sum<2, false>(a.set, tr, sE, nullptr, sWt, len, lane);
+    else if (kind == 3) s = full_piece_sum<3, false>(a.set, tr, sE, nullptr, sWt, len, lane);
+    else if (kind == 1) s = full_piece_sum<1, false>(a.set, tr, sE, nullptr, sWt, len, lane);
+    else s = full_piece_sum<0, false>(a.set, tr, sE, nullptr, sWt, len, lane);
+    if (lane == 0) partial[u] = s;
 }
 
 // out[p][cell] = sum over the pieces of the cell, in order, of partial[piece][p]; 0 for an empty cell.
@@ -555,6 +608,25 @@ scan_merge_kernel(const double* __restrict__ partial, const unsigned int* __rest
     }
     for (; u < u1; ++u, src += npoints) s += __ldg(src);
     out[(size_t)p * ncells + cell] = s;
+}
+
+
+// The same merge for a handful of points (one warp per (cell, point)): lane l adds the pieces u0 + l, u0 + l + 32, ...
+// of the cell in order, then a fixed xor-tree over the lanes.  A different but equally fixed order of additions.
+__global__ void __launch_bounds__(256)
+scan_merge_few_kernel(const double* __restrict__ partial, const unsigned int* __restrict__ unit_begin, int ncells,
+                      int npoints, double* __restrict__ out)
+{
+    const int cell = blockIdx.x;
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned u0 = unit_begin[cell], u1 = unit_begin[cell + 1];
+    for (int p = threadIdx.x >> 5; p < npoints; p += blockDim.x >> 5) {
+        double s = 0.0;
+        for (unsigned u = u0 + lane; u < u1; u += 32) s += __ldg(partial + (size_t)u * npoints + p);
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+        if (lane == 0) out[(size_t)p * ncells + cell] = s;
+    }
 }
 
 } // namespace oscb

@@ -32,7 +32,7 @@ def declared_symbols():
 
 def test_header_symbols_are_exported(L):
     names = declared_symbols()
-    assert len(names) >= 17
+    assert len(names) >= 22
     for name in names:
         assert hasattr(L, name), f"{name} declared in include/osc.h but not exported"
     assert set(names) == set(binding.EXPORTS)
@@ -123,6 +123,17 @@ def test_host_checkable_faults(L):
     assert L.osc_reweight_bin_scales_host(None, None, None, None, 0, sc, 0, 8, 4, 8) == INVALID
     assert L.osc_reweight_bin_scales_host(None, None, None, None, 0, None, 3, 8, 4, 8) == INVALID
     assert L.osc_reweight_bin_scales_host(None, None, None, None, 3, sc, 3, 8, 4, 8) == INVALID
+    # plans: null output, bad binning, not-a-plan handles
+    out = ctypes.c_void_p()
+    assert L.osc_plan_create(None, None, None, None, 0, 1.0, 8, 4, None, None) == INVALID
+    assert L.osc_plan_create(None, None, None, None, 0, 1.0, 8, 0, None, ctypes.byref(out)) == INVALID
+    assert L.osc_plan_create(None, None, None, None, 5, 1.0, 8, 4, None, ctypes.byref(out)) == INVALID and not out.value
+    junk = (ctypes.c_ulonglong * 8)()
+    assert L.osc_plan_reweight_bin(None, 8, None) == INVALID
+    assert L.osc_plan_reweight_bin(ctypes.addressof(junk), 8, None) == INVALID
+    assert L.osc_plan_reweight_bin_batch(ctypes.addressof(junk), pts, 2, 8, None) == INVALID
+    assert L.osc_plan_destroy(ctypes.addressof(junk)) == INVALID
+    assert L.osc_plan_destroy(None) == OK
     # likelihood: sizes, normalisation, null pointers; no points is a no-op
     assert L.osc_neg2lnl(8, 4, 0, 8, 1.0, 8, None) == INVALID
     assert L.osc_neg2lnl(8, -1, 10, 8, 1.0, 8, None) == INVALID

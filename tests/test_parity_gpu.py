@@ -569,6 +569,63 @@ def test_scales_fall_back_for_large_binnings(osc):
 
 
 # ------------------------------------------------------------------------------------------------
+# plans: events sorted once, many parameter sets afterwards (osc_plan_*)
+# ------------------------------------------------------------------------------------------------
+def test_plan_single_sets_vs_oracle_and_k2(osc):
+    n = 250_000 + 21
+    et, er, w0, ch = wl.events(n, seed=61)
+    et[2] = -3.0; ch[3] = 4; er[4] = 1e9
+    edges = wl.bin_edges()
+    d = [dev(a) for a in (et, er, w0, ch)]
+    de = dev(edges)
+    plan = osc.osc_plan_create(*d, 1.03, de)
+    torch.cuda.synchronize()
+    for t in d:                                   # the plan keeps its own sorted copy: scribble over the inputs
+        t.zero_()
+    d2 = [dev(a) for a in (et, er, w0, ch)]
+    for par in (wl.table1(), wl.table1(delta_cp=2.2, hierarchy=-1), wl.table1(rho_g_cm3=0.0, L_km=1300.0, sin2_th23=0.41)):
+        op = set_params(osc, par)
+        got = host(osc.osc_plan_reweight_bin(plan))
+        again = host(osc.osc_plan_reweight_bin(plan))
+        assert np.array_equal(got, again)
+        assert_hist_close(got, oracle.reweight_bin(op, et, er, w0, ch, 1.03, edges), "plan, single set")
+        np.testing.assert_allclose(got, host(osc.osc_reweight_bin(*d2, 1.03, de)), rtol=1e-12, atol=0.0)
+    osc.osc_plan_destroy(plan)
+    osc.osc_plan_destroy(plan)                    # second destroy of the wrapper is a no-op
+
+
+@pytest.mark.parametrize("n", [0, 1, 33, 1000])
+def test_plan_small_sizes(osc, n):
+    et, er, w0, ch = wl.events(max(n, 1), seed=62)
+    et, er, w0, ch = et[:n], er[:n], w0[:n], ch[:n]
+    edges = wl.bin_edges(7, 4.0)
+    op = set_params(osc, wl.table1())
+    plan = osc.osc_plan_create(dev(et), dev(er), dev(w0), dev(ch), 0.97, dev(edges))
+    assert_hist_close(host(osc.osc_plan_reweight_bin(plan)), oracle.reweight_bin(op, et, er, w0, ch, 0.97, edges),
+                      f"plan n={n}")
+    pts = [wl.table1(sin2_th23=0.4), wl.table1(sin2_th23=0.6, dm2_32=2.5e-3)]
+    got = host(osc.osc_plan_reweight_bin_batch(plan, pts))
+    ref = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 0.97, edges)
+    assert_hist_close(got, ref, f"plan batch n={n}")
+
+
+def test_plan_batch_grid_and_unrelated_points(osc):
+    n = 40_000 + 9
+    et, er, w0, ch = wl.events(n, seed=63)
+    edges = wl.bin_edges()
+    d = [dev(a) for a in (et, er, w0, ch)]
+    plan = osc.osc_plan_create(*d, 1.0, dev(edges))
+    grid = wl.scan_points()[:64]                       # two dm2_32 groups of 32 points: factorised kernel
+    loose = wl.scan_points()[::33][:20]                # unrelated points: one eigen-problem per point
+    for name, pts in (("grid", grid), ("loose", loose)):
+        got = host(osc.osc_plan_reweight_bin_batch(plan, pts))
+        ref = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 1.0, edges)
+        assert_hist_close(got, ref, f"plan batch {name}")
+        direct = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, dev(edges)))
+        np.testing.assert_allclose(got, direct, rtol=1e-12, atol=0.0)
+
+
+# ------------------------------------------------------------------------------------------------
 # NEXT-2: Poisson likelihood ratio of the batched histograms on the device (osc_neg2lnl)
 # ------------------------------------------------------------------------------------------------
 def test_neg2lnl_after_batch(osc):

@@ -447,20 +447,33 @@ __device__ __forceinline__ double full_piece_sum(const OscSet& set, const OscTra
     double acc[kFullUnroll];
 #pragma unroll
     for (int k = 0; k < kFullUnroll; ++k) acc[k] = 0.0;
+    // unstaged: the loads of the next step are issued before the arithmetic of the current one
+    double nE[kFullUnroll], nW[kFullUnroll];
+    if (!STAGED) {
+#pragma unroll
+        for (int k = 0; k < kFullUnroll; ++k) {
+            const int j = (int)lane + 32 * k;
+            nE[k] = j < len ? __ldg(sE + j) : 1.0;
+            nW[k] = j < len ? __ldg(sW + j) : 0.0;
+        }
+    }
     for (int i = lane; i < len; i += 32 * kFullUnroll) {
         double E[kFullUnroll], I[kFullUnroll], w[kFullUnroll], A[kFullUnroll];
         OscEig e[kFullUnroll];
 #pragma unroll
         for (int k = 0; k < kFullUnroll; ++k) {
             const int j = i + 32 * k;
-            const bool has = j < len;
             if (STAGED) {
+                const bool has = j < len;
                 E[k] = has ? sE[j] : 1.0;
                 I[k] = has ? sI[j] : 1.0;
                 w[k] = has ? sW[j] : 0.0;
             } else {
-                E[k] = has ? __ldg(sE + j) : 1.0;
-                w[k] = has ? __ldg(sW + j) : 0.0;
+                E[k] = nE[k];
+                w[k] = nW[k];
+                const int jn = j + 32 * kFullUnroll;
+                nE[k] = jn < len ? __ldg(sE + jn) : 1.0;
+                nW[k] = jn < len ? __ldg(sW + jn) : 0.0;
             }
             A[k] = tr.sa * E[k];
         }

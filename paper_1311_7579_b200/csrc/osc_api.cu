@@ -657,6 +657,19 @@ int sorted_geometry(size_t n, int n_bins, size_t piece, ScanGeom& geo)
     return OSC_OK;
 }
 
+// Kind of the element of S each channel asks for (assemble_kind in osc_core.cuh): 1 (e, e), 2 another diagonal
+// element, 3 off-diagonal.
+ChannelKinds channel_kinds()
+{
+    ChannelKinds kinds;
+    for (int c = 0; c < kChannels; ++c) {
+        int fin, fout, anti;
+        channel_def(c, fin, fout, anti);
+        kinds.k[c] = fin != fout ? 3 : (fin == 0 ? 1 : 2);
+    }
+    return kinds;
+}
+
 // The three sort passes.  se's buffers are assigned by the caller; the temporaries come from a stream-ordered scratch.
 int scan_sort(const SortedEvents& se, const double* E_true, const double* E_reco, const double* w0, const int8_t* channel,
               double energy_scale, const double* bin_edges, cudaStream_t st)
@@ -736,12 +749,7 @@ int scan_run(const SortedEvents& se, const ScanPlan* plan, const std::vector<Bin
                                                            se.unit_cell, geo, se.n_bins, n_points, partial);
         if ((rc = post_launch("batched reweighting on sorted events (k4, factorised)"))) return rc;
     } else {
-        ChannelKinds kinds;
-        for (int c = 0; c < kChannels; ++c) {
-            int fin, fout, anti;
-            channel_def(c, fin, fout, anti);
-            kinds.k[c] = fin != fout ? 3 : (fin == 0 ? 1 : 2);
-        }
+        const ChannelKinds kinds = channel_kinds();
         if (geo.subs_per_slot > 2) {          // a piece is staged in shared memory once and walked by many points
             const size_t smem_ev = sizeof(double) * kScanWarps * 3 * (size_t)geo.piece;  // <= 48 kB at piece = 512
             scan_full_kernel<true><<<grid, 32 * kScanWarps, smem_ev, st>>>(
@@ -1013,12 +1021,7 @@ int osc_plan_reweight_bin(const osc_plan* plan, double* hist_out, void* stream)
     char* scratch = nullptr;
     if ((rc = stream_scratch(kCounterBytes + (size_t)se.geo.max_units * sizeof(double), st, &scratch))) return rc;
     double* partial = reinterpret_cast<double*>(scratch + kCounterBytes);
-    ChannelKinds kinds;
-    for (int c = 0; c < kChannels; ++c) {
-        int fin, fout, anti;
-        channel_def(c, fin, fout, anti);
-        kinds.k[c] = fin != fout ? 3 : (fin == 0 ? 1 : 2);
-    }
+    const ChannelKinds kinds = channel_kinds();
     scan_full_one_kernel<<<(se.geo.max_units + kScanWarps - 1) / kScanWarps, 32 * kScanWarps, 0, st>>>(
         args, kinds, se.sEt, se.sW, se.cell_begin, se.unit_begin, se.unit_cell, se.geo, se.n_bins, partial);
     if ((rc = post_launch("osc_plan_reweight_bin (k5, one parameter set)"))) return rc;

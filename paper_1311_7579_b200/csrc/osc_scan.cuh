@@ -440,28 +440,28 @@ constexpr int kFullUnroll = 4;
 
 // STAGED: the events come from the warp's shared-memory copy (E, 1/E, w0); otherwise straight from the sorted arrays
 // in global memory with 1/E taken here -- for one or two points per piece the staging pass costs more than it saves.
-template <int KIND, bool STAGED>
+template <int KIND, bool STAGED, int UNROLL = kFullUnroll>
 __device__ __forceinline__ double full_piece_sum(const OscSet& set, const OscTrans& tr, const double* sE,
                                                  const double* sI, const double* sW, int len, unsigned lane)
 {
-    double acc[kFullUnroll];
+    double acc[UNROLL];
 #pragma unroll
-    for (int k = 0; k < kFullUnroll; ++k) acc[k] = 0.0;
+    for (int k = 0; k < UNROLL; ++k) acc[k] = 0.0;
     // unstaged: the loads of the next step are issued before the arithmetic of the current one
-    double nE[kFullUnroll], nW[kFullUnroll];
+    double nE[UNROLL], nW[UNROLL];
     if (!STAGED) {
 #pragma unroll
-        for (int k = 0; k < kFullUnroll; ++k) {
+        for (int k = 0; k < UNROLL; ++k) {
             const int j = (int)lane + 32 * k;
             nE[k] = j < len ? __ldg(sE + j) : 1.0;
             nW[k] = j < len ? __ldg(sW + j) : 0.0;
         }
     }
-    for (int i = lane; i < len; i += 32 * kFullUnroll) {
-        double E[kFullUnroll], I[kFullUnroll], w[kFullUnroll], A[kFullUnroll];
-        OscEig e[kFullUnroll];
+    for (int i = lane; i < len; i += 32 * UNROLL) {
+        double E[UNROLL], I[UNROLL], w[UNROLL], A[UNROLL];
+        OscEig e[UNROLL];
 #pragma unroll
-        for (int k = 0; k < kFullUnroll; ++k) {
+        for (int k = 0; k < UNROLL; ++k) {
             const int j = i + 32 * k;
             if (STAGED) {
                 const bool has = j < len;
@@ -471,7 +471,7 @@ __device__ __forceinline__ double full_piece_sum(const OscSet& set, const OscTra
             } else {
                 E[k] = nE[k];
                 w[k] = nW[k];
-                const int jn = j + 32 * kFullUnroll;
+                const int jn = j + 32 * UNROLL;
                 nE[k] = jn < len ? __ldg(sE + jn) : 1.0;
                 nW[k] = jn < len ? __ldg(sW + jn) : 0.0;
             }
@@ -479,14 +479,16 @@ __device__ __forceinline__ double full_piece_sum(const OscSet& set, const OscTra
         }
         if (!STAGED) {
 #pragma unroll
-            for (int k = 0; k < kFullUnroll; ++k) I[k] = rcp_pos(E[k]);
+            for (int k = 0; k < UNROLL; ++k) I[k] = rcp_pos(E[k]);
         }
 #pragma unroll
-        for (int k = 0; k < kFullUnroll; ++k) eig_solve(set, A[k], I[k], e[k]);
+        for (int k = 0; k < UNROLL; ++k) eig_solve(set, A[k], I[k], e[k]);
 #pragma unroll
-        for (int k = 0; k < kFullUnroll; ++k) acc[k] = fma(w[k], assemble_kind<KIND>(e[k], A[k], tr), acc[k]);
+        for (int k = 0; k < UNROLL; ++k) acc[k] = fma(w[k], assemble_kind<KIND>(e[k], A[k], tr), acc[k]);
     }
-    double s = (acc[0] + acc[1]) + (acc[2] + acc[3]);
+    double s = acc[0];
+#pragma unroll
+    for (int k = 1; k < UNROLL; ++k) s += acc[k];
 #pragma unroll
     for (int d = 16; d >= 1; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
     return s;
@@ -559,6 +561,8 @@ scan_full_kernel(const double* __restrict__ points, int npoints, int pts_per_slo
     }
 }
 
+constexpr int kOneUnroll = 4;
+
 // k5 for ONE parameter set (osc_plan_reweight_bin): the parameter block travels as a kernel parameter, as in k2, so
 // the call is two launches and nothing else on the stream (no table upload, no per-call allocation).
 __global__ void __launch_bounds__(32 * kScanWarps, 3)
@@ -592,10 +596,10 @@ scan_full_one_kernel(const __grid_constant__ BinArgs a, const ChannelKinds kinds
     const double* sE = sEt + begin;
     const double* sWt = sW + begin;
     double s;
-    if (kind == 2) s = full_piece_sum<2, false>(a.set, tr, sE, nullptr, sWt, len, lane);
-    else if (kind == 3) s = full_piece_sum<3, false>(a.set, tr, sE, nullptr, sWt, len, lane);
-    else if (kind == 1) s = full_piece_sum<1, false>(a.set, tr, sE, nullptr, sWt, len, lane);
-    else s = full_piece_sum<0, false>(a.set, tr, sE, nullptr, sWt, len, lane);
+    if (kind == 2) s = full_piece_sum<2, false, kOneUnroll>(a.set, tr, sE, nullptr, sWt, len, lane);
+    else if (kind == 3) s = full_piece_sum<3, false, kOneUnroll>(a.set, tr, sE, nullptr, sWt, len, lane);
+    else if (kind == 1) s = full_piece_sum<1, false, kOneUnroll>(a.set, tr, sE, nullptr, sWt, len, lane);
+    else s = full_piece_sum<0, false, kOneUnroll>(a.set, tr, sE, nullptr, sWt, len, lane);
     if (lane == 0) partial[u] = s;
 }
 

@@ -514,6 +514,25 @@ def test_batch_sorted_paths_with_768_bins(osc):
         assert_hist_close(got, ref, f"{path} with 768 bins")
 
 
+@pytest.mark.parametrize("path", ["k4", "k5"])
+def test_batch_sorted_paths_on_corner_parameters(osc, path):
+    """The degenerate and extreme parameter sets of test_corner_parameters through the sorted batched kernels: every
+    corner as its own group (k5), and every corner with four (theta23, delta) variations (k4)."""
+    n = 6_000 + 1
+    et, er, w0, ch = wl.events(n, seed=28)
+    edges = wl.bin_edges()
+    pts = []
+    for c in CORNERS:
+        base = wl.table1(**c)
+        for k in range(4 if path == "k4" else 1):
+            pts.append(dict(base, sin2_th23=base["sin2_th23"] if k == 0 else 0.2 + 0.2 * k,
+                            delta_cp=base["delta_cp"] if k == 0 else -2.5 + 1.7 * k))
+    with batch_path(path):
+        got = host(osc.osc_reweight_bin_batch(pts, dev(et), dev(er), dev(w0), dev(ch), 1.0, dev(edges)))
+    ref = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 1.0, edges)
+    assert_hist_close(got, ref, f"{path} on corner parameters")
+
+
 def test_k4_all_events_dropped(osc):
     n = 500
     et, er, w0, ch = wl.events(n, seed=25)

@@ -84,7 +84,7 @@ class ClockSampler:
         self.proc = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -468,7 +468,8 @@ def main():
     t_wall1 = time.time()
     launches = osc.osc_launch_count() - launches0
     ms = ev0.elapsed_time(ev1)
-    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+    # the clock sampler keeps running through the legs below (the same kernels on the same data, back to back): the
+    # timed region of `value` alone is a few milliseconds, too short for more than a sample or two
     t_ms = torch.tensor([ms], dtype=torch.float64, device=device)
     if world > 1:
         dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
@@ -539,6 +540,9 @@ def main():
                       "events pre-sorted by histogram cell, kernel k5 for one parameter set"}
     for pl in plans:
         osc.osc_plan_destroy(pl)
+    clocks = sampler.stop(t_wall0, time.time()) if sampler else None
+    if clocks is not None:
+        clocks["window"] = "timed region of `value` and the kernel-alone, fused_scales and planned legs that follow it"
 
     # ---- fp64 peak probe in the same run (DFMA-only, register resident) ----------------------------------------
     probe_flops = osc.osc_fp64_peak_probe(1 << 14, 4)

@@ -644,6 +644,43 @@ def test_plan_batch_grid_and_unrelated_points(osc):
         np.testing.assert_allclose(got, direct, rtol=1e-12, atol=0.0)
 
 
+def test_outputs_stay_inside_their_buffers(osc):
+    """Guard bands around every histogram output (the sanitizer is not available on the GPU pool): each call writes its
+    slice of a larger tensor pre-filled with a sentinel, and nothing outside the slice may change."""
+    n = 4_000 + 3
+    et, er, w0, ch = wl.events(n, seed=71)
+    edges = wl.bin_edges(23, 5.0)
+    d = [dev(a) for a in (et, er, w0, ch)]
+    de = dev(edges)
+    osc.osc_set_params(**wl.table1())
+    grid, loose = wl.scan_points()[:40], wl.scan_points()[::33][:12]
+    plan = osc.osc_plan_create(*d, 1.0, de)
+    nh = 4 * 23
+    calls = [
+        (nh, lambda out: osc.osc_reweight_bin(*d, 1.0, de, hist_out=out)),
+        (3 * nh, lambda out: osc.osc_reweight_bin_scales(*d, wl.ENERGY_SCALES, de, hist_out=out)),
+        (40 * nh, lambda out: osc.osc_reweight_bin_batch(grid, *d, 1.0, de, hist_out=out)),
+        (12 * nh, lambda out: osc.osc_reweight_bin_batch(loose, *d, 1.0, de, hist_out=out)),
+        (3 * nh, lambda out: osc.osc_reweight_bin_batch(loose[:3], *d, 1.0, de, hist_out=out)),
+        (nh, lambda out: osc.osc_plan_reweight_bin(plan, hist_out=out)),
+        (40 * nh, lambda out: osc.osc_plan_reweight_bin_batch(plan, grid, hist_out=out)),
+        (12 * nh, lambda out: osc.osc_plan_reweight_bin_batch(plan, loose, hist_out=out)),
+    ]
+    guard = 64
+    for k, (size, call) in enumerate(calls):
+        buf = torch.full((size + 2 * guard,), -7.0, dtype=torch.float64, device="cuda")
+        call(buf[guard:guard + size])
+        torch.cuda.synchronize()
+        b = host(buf)
+        assert np.all(b[:guard] == -7.0) and np.all(b[guard + size:] == -7.0), f"call {k} wrote outside its output"
+        assert np.all(b[guard:guard + size] >= 0.0), f"call {k} left part of its output unwritten"
+    hist = osc.osc_reweight_bin_batch(loose, *d, 1.0, de)
+    buf = torch.full((12 + 2 * guard,), -7.0, dtype=torch.float64, device="cuda")
+    osc.osc_neg2lnl(hist, dev(np.ones(nh)), 1.0, out=buf[guard:guard + 12])
+    b = host(buf)
+    assert np.all(b[:guard] == -7.0) and np.all(b[guard + 12:] == -7.0) and np.all(b[guard:guard + 12] >= 0.0)
+
+
 # ------------------------------------------------------------------------------------------------
 # NEXT-2: Poisson likelihood ratio of the batched histograms on the device (osc_neg2lnl)
 # ------------------------------------------------------------------------------------------------

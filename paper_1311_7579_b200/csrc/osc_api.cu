@@ -205,8 +205,17 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     int sms = 0;
     int rc = sm_count(&sms);
     if (rc) return rc;
-    const int threads = k2_smem_bytes(n_bins, 256, 1) <= kSmemBudget ? 256 : 128;
-    // two sub-histograms per slot halve the collisions inside a warp; taken when at least 3 blocks still fit
+    // One block of 768 threads per SM when its sub-histograms fit (up to about 140 bins), else three blocks of 256,
+    // else six of 128.  Co-resident blocks do not run at the same speed -- the warp schedulers favour the warps
+    // that arrived first: with three blocks of 256 and equal shares of 44 tiles the first block of an SM needed
+    // 85 us, the second 102 us and the third 127 us, and the SM spent the end of the kernel on 8 warps.  The warps of
+    // ONE block are all the same age and finish together (measured: 137 -> 129 us per 1e7 events); a static
+    // re-weighting of the shares does not work, the slot of a block on its SM is not known in advance.
+    int threads = k2_smem_bytes(n_bins, 768, 1) + 1024 <= kSmemBudget ? 768
+                : k2_smem_bytes(n_bins, 256, 1) <= kSmemBudget          ? 256
+                                                                        : 128;
+    if (const char* e = getenv("OSC_TUNE_THREADS")) threads = atoi(e);
+    // 256 threads: two sub-histograms per slot halve the collisions inside a warp; taken when 3 blocks still fit
     const int n_sub = (threads == 256 && 3 * (k2_smem_bytes(n_bins, 256, 2) + 1024) <= kSmemBudget) ? 2 : 1;
     int n_sub_t = n_sub;
     if (const char* e = getenv("OSC_TUNE_NSUB")) n_sub_t = atoi(e);
@@ -214,7 +223,7 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     size_t per_sm = kSmemBudget / (smem + 1024);
     if (const char* e = getenv("OSC_TUNE_BPS")) per_sm = (size_t)atoi(e);
     if (per_sm < 1) per_sm = 1;
-    const size_t max_per_sm = threads == 256 ? 3 : 6;   // __launch_bounds__(THREADS, 768 / THREADS) of k2
+    const size_t max_per_sm = threads >= 512 ? 1 : threads == 256 ? 3 : 6;   // __launch_bounds__(THREADS, 768 / THREADS) of k2
     if (per_sm > max_per_sm && !getenv("OSC_TUNE_BPS")) per_sm = max_per_sm;
     const size_t ntiles = (n + 2 * threads - 1) / (2 * (size_t)threads);
     if (ntiles > 0xFFFFFFFFull) return fail(OSC_ERR_INVALID_ARG, "n = %zu events is more than one call takes (2^32 tiles)", n);
@@ -236,6 +245,11 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     ms.ngroups = ngroups;
 
     const bool vec = aligned(E_true, 16) && aligned(E_reco, 16) && aligned(w0, 16) && aligned(channel, 2);
+    if (threads == 768)
+        return vec ? launch_k2<true, 768>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
+                                          n_bins, n_sub_t, ms, hist_out)
+                   : launch_k2<false, 768>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
+                                           n_bins, n_sub, ms, hist_out);
     if (threads == 256)
         return vec ? launch_k2<true, 256>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
                                           n_bins, n_sub_t, ms, hist_out)

@@ -40,10 +40,10 @@ SCALES = wl.ENERGY_SCALES
 BYTES_PER_EVENT = 25          # E_true + E_reco + w0 (fp64) + channel (int8): SURVEY.md 8(d), DESIGN.md "k2"
 # fp64 operations k2 executes per event (DFMA = 2, DMUL/DADD = 1), counted by ncu
 # (smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum / events): DESIGN.md 5.1, profiles/r1_k2_full_a.md.
-FLOP_PER_EVENT = 199.3        # 75.0 DFMA + 42.0 DMUL + 7.3 DADD per event (profiles/r1_k2_full_b.md)
+FLOP_PER_EVENT = 199.1        # 75.0 DFMA + 42.0 DMUL + 7.1 DADD per event (profiles/r1_launches_d.md)
 # dram__bytes_read.sum + dram__bytes_write.sum of one k2 launch over 1e7 events (same capture); algorithmic: 250.0e6
-NCU_TRAFFIC_BYTES_1E7 = 253.66e6
-NCU_TRAFFIC_SOURCE = "profiles/r1_k2_full_b.md"
+NCU_TRAFFIC_BYTES_1E7 = 253.20e6
+NCU_TRAFFIC_SOURCE = "profiles/r1_launches_d.md"
 FP64_LANES_PER_SM_CLK = 64    # B200 (sm_100): 4 sub-partitions x 16 fp64 lanes; DESIGN.md "fp64 roofline"
 
 

@@ -214,7 +214,7 @@ const char *osc_last_error(void);
 /* Number of kernel launches this library has enqueued since it was loaded (for bench.py's gpu_launches). */
 unsigned long long osc_launch_count(void);
 
-/* Library version string, e.g. "osc_b200 0.1 (sm_100a)". */
+/* Library version string, e.g. "osc_b200 0.2 (sm_100a)". */
 const char *osc_version(void);
 
 /* The library works on the calling thread's current CUDA device.  These two wrap cudaSetDevice /

@@ -1193,7 +1193,7 @@ const char* osc_last_error(void) { return t_err; }
 
 unsigned long long osc_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
-const char* osc_version(void) { return "osc_b200 0.1 (sm_100a)"; }
+const char* osc_version(void) { return "osc_b200 0.2 (sm_100a)"; }
 
 int osc_set_device(int device)
 {

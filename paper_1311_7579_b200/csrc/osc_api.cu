@@ -205,13 +205,17 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     int sms = 0;
     int rc = sm_count(&sms);
     if (rc) return rc;
-    // One block of 768 threads per SM when its sub-histograms fit (up to about 140 bins), else three blocks of 256,
-    // else six of 128.  Co-resident blocks do not run at the same speed -- the warp schedulers favour the warps
-    // that arrived first: with three blocks of 256 and equal shares of 44 tiles the first block of an SM needed
-    // 85 us, the second 102 us and the third 127 us, and the SM spent the end of the kernel on 8 warps.  The warps of
-    // ONE block are all the same age and finish together (measured: 137 -> 129 us per 1e7 events); a static
-    // re-weighting of the shares does not work, the slot of a block on its SM is not known in advance.
+    // One block of 768 threads per SM when its sub-histograms fit (up to about 140 bins), else one block of 512 (up to
+    // about 210 bins; 118 registers, 5 % fewer instructions, and four warps per scheduler still fill the issue slots:
+    // 138-140 us per 1e7 events against 148-151 us for three blocks of 256), else blocks of 256, else of 128.  Warp
+    // counts that are not a multiple of four per scheduler lose (576, 640, 704 threads: 145, 135, 138 us against 129).
+    // Co-resident blocks do not run at the same speed -- the warp schedulers favour the warps that arrived first:
+    // with three blocks of 256 and equal shares of 44 tiles the first block of an SM needed 85 us, the second 102 us
+    // and the third 127 us, and the SM spent the end of the kernel on 8 warps.  The warps of ONE block are all the
+    // same age and finish together (measured: 137 -> 129 us per 1e7 events); a static re-weighting of the shares
+    // does not work, the slot of a block on its SM is not known in advance.
     int threads = k2_smem_bytes(n_bins, 768, 1) + 1024 <= kSmemBudget ? 768
+                : k2_smem_bytes(n_bins, 512, 1) + 1024 <= kSmemBudget ? 512
                 : k2_smem_bytes(n_bins, 256, 1) <= kSmemBudget          ? 256
                                                                         : 128;
     if (const char* e = getenv("OSC_TUNE_THREADS")) threads = atoi(e);
@@ -249,6 +253,11 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
         return vec ? launch_k2<true, 768>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
                                           n_bins, n_sub_t, ms, hist_out)
                    : launch_k2<false, 768>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
+                                           n_bins, n_sub, ms, hist_out);
+if (threads == 512)
+        return vec ? launch_k2<true, 512>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
+                                          n_bins, n_sub_t, ms, hist_out)
+                   : launch_k2<false, 512>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
                                            n_bins, n_sub, ms, hist_out);
     if (threads == 256)
         return vec ? launch_k2<true, 256>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,

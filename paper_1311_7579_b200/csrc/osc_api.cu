@@ -80,12 +80,12 @@ int check_flavour(int f, const char* what)
 // Blocks per SM the persistent kernels are sized for (register budget: see DESIGN.md "Kernels").
 constexpr int kBlocksPerSM = 4;
 
-int grid_for(size_t work_items, int* grid)
+int grid_for(size_t work_items, int* grid, int blocks_per_sm = kBlocksPerSM)
 {
     int sms = 0;
     int rc = sm_count(&sms);
     if (rc) return rc;
-    size_t g = (size_t)sms * kBlocksPerSM;
+    size_t g = (size_t)sms * blocks_per_sm;
     if (work_items < g) g = work_items;
     if (g < 1) g = 1;
     *grid = (int)g;
@@ -389,21 +389,29 @@ int osc_prob(const double* E_true, size_t n, int flavour_in, int flavour_out, in
     a.set = h.set;
     a.tr = make_trans(h, flavour_in, flavour_out, antinu);
     const size_t npairs = (n + 1) / 2;
+    // one block of kBlockProb threads per SM once every SM gets two full iterations of it; below that, blocks of
+    // kBlock threads spread the events over more SMs (configs[0]: 1e5 events)
+    int sms = 0;
+    if ((rc = sm_count(&sms))) return rc;
+    const bool big = npairs >= (size_t)2 * sms * kBlockProb;
     int grid = 1;
-    if ((rc = grid_for((npairs + kBlock - 1) / kBlock, &grid))) return rc;
+    if ((rc = big ? grid_for((npairs + kBlockProb - 1) / kBlockProb, &grid, 1)
+                  : grid_for((npairs + kBlock - 1) / kBlock, &grid)))
+        return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     // the element of S that is asked for is known here: 1 (e, e), 2 another diagonal element, 3 off-diagonal
     const int kind = flavour_in != flavour_out ? 3 : (flavour_in == 0 ? 1 : 2);
-#define OSC_K1(VEC)                                                                       \
+#define OSC_K1(VEC, T)                                                                    \
     switch (kind) {                                                                       \
-    case 1: prob_kernel<VEC, 1><<<grid, kBlock, 0, st>>>(a, E_true, n, P_out); break;     \
-    case 2: prob_kernel<VEC, 2><<<grid, kBlock, 0, st>>>(a, E_true, n, P_out); break;     \
-    default: prob_kernel<VEC, 3><<<grid, kBlock, 0, st>>>(a, E_true, n, P_out); break;    \
+    case 1: prob_kernel<VEC, 1, T><<<grid, T, 0, st>>>(a, E_true, n, P_out); break;       \
+    case 2: prob_kernel<VEC, 2, T><<<grid, T, 0, st>>>(a, E_true, n, P_out); break;       \
+    default: prob_kernel<VEC, 3, T><<<grid, T, 0, st>>>(a, E_true, n, P_out); break;      \
     }
-    if (aligned(E_true, 16) && aligned(P_out, 16)) {
-        OSC_K1(true)
+    const bool vec = aligned(E_true, 16) && aligned(P_out, 16);
+    if (big) {
+        if (vec) { OSC_K1(true, kBlockProb) } else { OSC_K1(false, kBlockProb) }
     } else {
-        OSC_K1(false)
+        if (vec) { OSC_K1(true, kBlock) } else { OSC_K1(false, kBlock) }
     }
 #undef OSC_K1
     return post_launch("osc_prob");

@@ -19,7 +19,9 @@
 
 namespace oscb {
 
-constexpr int kBlock = 256;          // threads per block of k1 / k1b (8 warps)
+constexpr int kBlock = 256;          // threads per block of k1b and the small kernels (8 warps)
+constexpr int kBlockProb = 768;      // k1 above ~5e5 events: ONE block of 24 warps per SM (as k2; 88.7 us against 95.0 us
+                                     // per 1e7 events for four blocks of 256, whose warps finish at different times)
 
 // Streaming loads/stores: every event byte is touched once (evict-first, no L1 allocation).
 __device__ __forceinline__ double ld_stream(const double* p) { return __ldcs(p); }
@@ -46,18 +48,18 @@ __device__ __forceinline__ double qnan() { return __longlong_as_double(0x7FF8000
 // k1: P_out[j] = P(alpha -> beta)(E_true[j]).  VEC: pointers 16-byte aligned -> 128-bit accesses.
 // KIND: which element of S is asked for (assemble_kind): the launch knows it, so the assembly is specialised.
 // ------------------------------------------------------------------------------------------------
-template <bool VEC, int KIND>
-__global__ void __launch_bounds__(kBlock)
+template <bool VEC, int KIND, int THREADS>
+__global__ void __launch_bounds__(THREADS, THREADS >= 512 ? 1 : 4)
 prob_kernel(const __grid_constant__ ProbArgs a, const double* __restrict__ E_true, size_t n,
             double* __restrict__ P_out)
 {
-    // VEC: slot i holds events (2i, 2i+1); otherwise tile i / kBlock holds events j0 and j0 + kBlock.
+    // VEC: slot i holds events (2i, 2i+1); otherwise tile i / THREADS holds events j0 and j0 + THREADS.
     // The energies of the thread's next slot are loaded before the arithmetic of the current one.
-    const size_t nslots = VEC ? (n + 1) / 2 : ((n + 2 * kBlock - 1) / (2 * kBlock)) * kBlock;
-    const size_t stride = (size_t)gridDim.x * kBlock;
+    const size_t nslots = VEC ? (n + 1) / 2 : ((n + 2 * THREADS - 1) / (2 * THREADS)) * THREADS;
+    const size_t stride = (size_t)gridDim.x * THREADS;
     auto load = [&](size_t i, double& E0, double& E1) {
-        const size_t j0 = VEC ? 2 * i : (i / kBlock) * (2 * kBlock) + (i % kBlock);
-        const size_t j1 = VEC ? j0 + 1 : j0 + kBlock;
+        const size_t j0 = VEC ? 2 * i : (i / THREADS) * (2 * THREADS) + (i % THREADS);
+        const size_t j1 = VEC ? j0 + 1 : j0 + THREADS;
         if (VEC && j1 < n) {
             const double2 v = ld_stream2(E_true + j0);
             E0 = v.x;
@@ -67,12 +69,12 @@ prob_kernel(const __grid_constant__ ProbArgs a, const double* __restrict__ E_tru
             E1 = (j1 < n) ? ld_stream(E_true + j1) : 1.0;
         }
     };
-    size_t i = (size_t)blockIdx.x * kBlock + threadIdx.x;
+    size_t i = (size_t)blockIdx.x * THREADS + threadIdx.x;
     double N0 = 1.0, N1 = 1.0;
     if (i < nslots) load(i, N0, N1);
     while (i < nslots) {
-        const size_t j0 = VEC ? 2 * i : (i / kBlock) * (2 * kBlock) + (i % kBlock);
-        const size_t j1 = VEC ? j0 + 1 : j0 + kBlock;
+        const size_t j0 = VEC ? 2 * i : (i / THREADS) * (2 * THREADS) + (i % THREADS);
+        const size_t j1 = VEC ? j0 + 1 : j0 + THREADS;
         const bool has1 = j1 < n;
         const double E0 = N0, E1 = N1;
         i += stride;

@@ -214,6 +214,25 @@ def test_ragged_sizes(osc, n):
         assert_prob_close(o[1:1 + 9 * n].reshape(9, n), oracle.prob_all(op, Es, 0), f"ragged all n={n}")
 
 
+def test_ragged_sizes_wide_blocks(osc):
+    """osc_prob above ~4.5e5 events runs as one block of 768 threads per SM: the three assemblies (e->e, another
+    diagonal element, off-diagonal), 128-bit and scalar path, a ragged tail, and nothing written outside P_out."""
+    n = 2 * 148 * 768 * 2 + 768 * 2 * 3 + 5
+    op = set_params(osc, wl.table1(delta_cp=-0.4))
+    E = wl.e_true(n + 1, seed=4242)
+    E[[11, n // 2, n - 1]] = [np.nan, 0.0, -2.0]
+    d = dev(E)
+    for off in (0, 1):
+        Es = E[off:off + n]
+        o0 = 2 - off
+        for fin, fout, anti in ((0, 0, 0), (1, 1, 1), (1, 0, 0)):
+            out = torch.full((n + 4,), -7.0, dtype=torch.float64, device="cuda")
+            osc.osc_prob(d[off:off + n], fin, fout, anti, P_out=out[o0:o0 + n])
+            o = host(out)
+            assert np.all(o[:o0] == -7.0) and np.all(o[o0 + n:] == -7.0), "wrote outside P_out"
+            assert_prob_close(o[o0:o0 + n], oracle.prob(op, Es, fin, fout, anti), f"wide blocks {fin}->{fout} off={off}")
+
+
 def test_n_zero(osc):
     set_params(osc, wl.table1())
     e = torch.empty(0, dtype=torch.float64, device="cuda")

@@ -207,7 +207,8 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     if (rc) return rc;
     // One block of 768 threads per SM when its sub-histograms fit (up to about 140 bins), else one block of 512 (up to
     // about 210 bins; 118 registers, 5 % fewer instructions, and four warps per scheduler still fill the issue slots:
-    // 138-140 us per 1e7 events against 148-151 us for three blocks of 256), else blocks of 256, else of 128.  Warp
+    // 138-140 us per 1e7 events against 148-151 us for three blocks of 256), else one block of 384 (up to about 280
+    // bins: 165 us against 205-211 us for the one block of 256 that fits), else blocks of 256, else of 128.  Warp
     // counts that are not a multiple of four per scheduler lose (576, 640, 704 threads: 145, 135, 138 us against 129).
     // Co-resident blocks do not run at the same speed -- the warp schedulers favour the warps that arrived first:
     // with three blocks of 256 and equal shares of 44 tiles the first block of an SM needed 85 us, the second 102 us
@@ -216,6 +217,7 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     // does not work, the slot of a block on its SM is not known in advance.
     int threads = k2_smem_bytes(n_bins, 768, 1) + 1024 <= kSmemBudget ? 768
                 : k2_smem_bytes(n_bins, 512, 1) + 1024 <= kSmemBudget ? 512
+                : k2_smem_bytes(n_bins, 384, 1) + 1024 <= kSmemBudget ? 384
                 : k2_smem_bytes(n_bins, 256, 1) <= kSmemBudget          ? 256
                                                                         : 128;
     if (const char* e = getenv("OSC_TUNE_THREADS")) threads = atoi(e);
@@ -227,7 +229,7 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     size_t per_sm = kSmemBudget / (smem + 1024);
     if (const char* e = getenv("OSC_TUNE_BPS")) per_sm = (size_t)atoi(e);
     if (per_sm < 1) per_sm = 1;
-    const size_t max_per_sm = threads >= 512 ? 1 : threads == 256 ? 3 : 6;   // __launch_bounds__(THREADS, 768 / THREADS) of k2
+    const size_t max_per_sm = threads >= 384 ? 1 : threads == 256 ? 3 : 6;   // __launch_bounds__(THREADS, 768 / THREADS) of k2
     if (per_sm > max_per_sm && !getenv("OSC_TUNE_BPS")) per_sm = max_per_sm;
     const size_t ntiles = (n + 2 * threads - 1) / (2 * (size_t)threads);
     if (ntiles > 0xFFFFFFFFull) return fail(OSC_ERR_INVALID_ARG, "n = %zu events is more than one call takes (2^32 tiles)", n);
@@ -254,7 +256,12 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
                                           n_bins, n_sub_t, ms, hist_out)
                    : launch_k2<false, 768>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
                                            n_bins, n_sub, ms, hist_out);
-if (threads == 512)
+    if (threads == 384)
+        return vec ? launch_k2<true, 384>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
+                                          n_bins, n_sub_t, ms, hist_out)
+                   : launch_k2<false, 384>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
+                                           n_bins, n_sub, ms, hist_out);
+    if (threads == 512)
         return vec ? launch_k2<true, 512>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
                                           n_bins, n_sub_t, ms, hist_out)
                    : launch_k2<false, 512>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,

@@ -331,7 +331,7 @@ __device__ __forceinline__ void k2_loop(const BinArgs& a, const double* __restri
 #define OSC_K2_TPS 768
 #endif
 template <bool VEC, int THREADS>
-__global__ void __launch_bounds__(THREADS, OSC_K2_TPS / THREADS)
+__global__ void __launch_bounds__(THREADS, THREADS >= 384 ? 1 : OSC_K2_TPS / THREADS)
 reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict__ E_true,
                     const double* __restrict__ E_reco, const double* __restrict__ w0,
                     const int8_t* __restrict__ channel, size_t n, double energy_scale,

@@ -314,7 +314,8 @@ def test_dropped_and_bad_events_are_skipped(osc):
 
 @pytest.mark.parametrize("nb,kind", [(1, "uniform"), (2, "uniform"), (3, "log"), (7, "random"), (50, "random"),
                                      (64, "uniform"), (140, "uniform"), (141, "random"), (200, "log"),
-                                     (210, "uniform"), (211, "random"), (768, "uniform")])
+                                     (210, "uniform"), (215, "random"), (250, "uniform"), (290, "log"),
+                                     (768, "uniform")])
 def test_bin_layouts(osc, nb, kind):
     n = 30_007
     et, er, w0, ch = wl.events(n, seed=9)

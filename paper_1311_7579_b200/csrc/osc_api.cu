@@ -220,7 +220,11 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
                 : k2_smem_bytes(n_bins, 384, 1) + 1024 <= kSmemBudget ? 384
                 : k2_smem_bytes(n_bins, 256, 1) <= kSmemBudget          ? 256
                                                                         : 128;
-    if (const char* e = getenv("OSC_TUNE_THREADS")) threads = atoi(e);
+    if (const char* e = getenv("OSC_TUNE_THREADS")) {
+        threads = atoi(e);
+        if (threads != 768 && threads != 512 && threads != 384 && threads != 256 && threads != 128)
+            return fail(OSC_ERR_INVALID_ARG, "OSC_TUNE_THREADS = %s: k2 is built for 128, 256, 384, 512 and 768 threads", e);
+    }
     // 256 threads: two sub-histograms per slot halve the collisions inside a warp; taken when 3 blocks still fit
     const int n_sub = (threads == 256 && 3 * (k2_smem_bytes(n_bins, 256, 2) + 1024) <= kSmemBudget) ? 2 : 1;
     int n_sub_t = n_sub;

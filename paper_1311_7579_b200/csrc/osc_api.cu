@@ -105,10 +105,10 @@ constexpr size_t kSmemBudget = 220 * 1024;
 
 size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-size_t k2_smem_bytes(int nb, int threads, int n_sub)
+size_t k2_smem_bytes(int nb, int threads, int n_sub, int slots = kSlots)
 {
     return sizeof(double) * kBinArgsDoubles + bin_table_bytes(nb) +
-           sizeof(double) * (size_t)(threads / 32) * kSlots * n_sub * kChannels * (size_t)nb;
+           sizeof(double) * (size_t)(threads / 32) * slots * n_sub * kChannels * (size_t)nb;
 }
 
 int check_bin_args(const double* E_true, const double* E_reco, const double* w0, const int8_t* channel, size_t n,
@@ -179,16 +179,17 @@ int stream_scratch(size_t bytes, cudaStream_t st, char** out)
     return OSC_OK;
 }
 
-template <bool VEC, int THREADS>
+template <bool VEC, int THREADS, int SLOTS = kSlots>
 int launch_k2(int grid, size_t smem, cudaStream_t st, const BinArgs& args, const double* E_true, const double* E_reco,
               const double* w0, const int8_t* channel, size_t n, double energy_scale, const double* bin_edges,
               int n_bins, int n_sub, const MergeScratch& ms, double* hist_out)
 {
     if (smem > 48 * 1024)
-        CUDA_TRY(cudaFuncSetAttribute(reweight_bin_kernel<VEC, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)smem));
-    reweight_bin_kernel<VEC, THREADS><<<grid, THREADS, smem, st>>>(args, E_true, E_reco, w0, channel, n, energy_scale,
-                                                                  bin_edges, n_bins, n_sub, ms, hist_out);
+        CUDA_TRY(cudaFuncSetAttribute(reweight_bin_kernel<VEC, THREADS, SLOTS>,
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    reweight_bin_kernel<VEC, THREADS, SLOTS><<<grid, THREADS, smem, st>>>(args, E_true, E_reco, w0, channel, n,
+                                                                         energy_scale, bin_edges, n_bins, n_sub, ms,
+                                                                         hist_out);
     return post_launch("osc_reweight_bin");
 }
 
@@ -205,31 +206,47 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     int sms = 0;
     int rc = sm_count(&sms);
     if (rc) return rc;
-    // One block of 768 threads per SM when its sub-histograms fit (up to about 140 bins), else one block of 512 (up to
-    // about 210 bins; 118 registers, 5 % fewer instructions, and four warps per scheduler still fill the issue slots:
-    // 138-140 us per 1e7 events against 148-151 us for three blocks of 256), else one block of 384 (up to about 280
-    // bins: 165 us against 205-211 us for the one block of 256 that fits), else blocks of 256, else of 128.  Warp
-    // counts that are not a multiple of four per scheduler lose (576, 640, 704 threads: 145, 135, 138 us against 129).
-    // Co-resident blocks do not run at the same speed -- the warp schedulers favour the warps that arrived first:
-    // with three blocks of 256 and equal shares of 44 tiles the first block of an SM needed 85 us, the second 102 us
-    // and the third 127 us, and the SM spent the end of the kernel on 8 warps.  The warps of ONE block are all the
-    // same age and finish together (measured: 137 -> 129 us per 1e7 events); a static re-weighting of the shares
-    // does not work, the slot of a block on its SM is not known in advance.
-    int threads = k2_smem_bytes(n_bins, 768, 1) + 1024 <= kSmemBudget ? 768
-                : k2_smem_bytes(n_bins, 512, 1) + 1024 <= kSmemBudget ? 512
-                : k2_smem_bytes(n_bins, 384, 1) + 1024 <= kSmemBudget ? 384
-                : k2_smem_bytes(n_bins, 256, 1) <= kSmemBudget          ? 256
-                                                                        : 128;
+    // ONE block per SM, as many warps as the sub-histograms leave room for (1e7 events, B200):
+    //   up to ~140 bins   768 threads, a sub-histogram per (warp, event of the lane)   129-138 us
+    //   up to ~213 bins   512 threads, same layout (118 registers, 5 % fewer instructions)   138-140 us
+    //   up to ~425 bins   512 threads, ONE sub-histogram per warp (SLOTS = 1, lane_hist_single)   139-155 us
+    //   up to ~570 bins   384 threads, one sub-histogram per warp   170-174 us
+    //   up to 768 bins    256 threads, one sub-histogram per warp   245-251 us
+    // Warp counts that are not a multiple of four per scheduler lose (576, 640, 704 threads: 145, 135, 138 us against
+    // 129).  Why one block: co-resident blocks do not run at the same speed -- the warp schedulers favour the warps
+    // that arrived first: with three blocks of 256 and equal shares of 44 tiles the first block of an SM needed
+    // 85 us, the second 102 us and the third 127 us, and the SM spent the end of the kernel on 8 warps.  The warps of
+    // ONE block are all the same age and finish together (measured: 137 -> 129 us per 1e7 events); a static
+    // re-weighting of the shares does not work, the slot of a block on its SM is not known in advance.  (Several
+    // blocks of 256 or 128 threads with two-slot sub-histograms remain reachable through OSC_TUNE_THREADS /
+    // OSC_TUNE_SLOTS for measurements: 147-230 us and 150-420 us over the same range of binnings.)
+    int threads = 256, slots = 1;
+    if (k2_smem_bytes(n_bins, 768, 1) + 1024 <= kSmemBudget) {
+        threads = 768;
+        slots = kSlots;
+    } else if (k2_smem_bytes(n_bins, 512, 1) + 1024 <= kSmemBudget) {
+        threads = 512;
+        slots = kSlots;
+    } else if (k2_smem_bytes(n_bins, 512, 1, 1) + 1024 <= kSmemBudget) {
+        threads = 512;
+    } else if (k2_smem_bytes(n_bins, 384, 1, 1) + 1024 <= kSmemBudget) {
+        threads = 384;
+    }
+    if (const char* e = getenv("OSC_TUNE_SLOTS")) slots = atoi(e) == 1 ? 1 : kSlots;
     if (const char* e = getenv("OSC_TUNE_THREADS")) {
         threads = atoi(e);
         if (threads != 768 && threads != 512 && threads != 384 && threads != 256 && threads != 128)
             return fail(OSC_ERR_INVALID_ARG, "OSC_TUNE_THREADS = %s: k2 is built for 128, 256, 384, 512 and 768 threads", e);
+        if (threads == 384) slots = 1;
     }
     // 256 threads: two sub-histograms per slot halve the collisions inside a warp; taken when 3 blocks still fit
-    const int n_sub = (threads == 256 && 3 * (k2_smem_bytes(n_bins, 256, 2) + 1024) <= kSmemBudget) ? 2 : 1;
+    const int n_sub = (slots == kSlots && threads == 256 && 3 * (k2_smem_bytes(n_bins, 256, 2) + 1024) <= kSmemBudget) ? 2 : 1;
     int n_sub_t = n_sub;
-    if (const char* e = getenv("OSC_TUNE_NSUB")) n_sub_t = atoi(e);
-    const size_t smem = k2_smem_bytes(n_bins, threads, n_sub_t);
+    if (const char* e = getenv("OSC_TUNE_NSUB")) n_sub_t = slots == kSlots ? atoi(e) : 1;
+    const size_t smem = k2_smem_bytes(n_bins, threads, n_sub_t, slots);
+    if (smem + 1024 > (size_t)227 * 1024)
+        return fail(OSC_ERR_INVALID_ARG, "%d bins with %d threads and %d slot(s) need %zu bytes of shared memory", n_bins,
+                    threads, slots, smem);
     size_t per_sm = kSmemBudget / (smem + 1024);
     if (const char* e = getenv("OSC_TUNE_BPS")) per_sm = (size_t)atoi(e);
     if (per_sm < 1) per_sm = 1;
@@ -255,15 +272,19 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     ms.ngroups = ngroups;
 
     const bool vec = aligned(E_true, 16) && aligned(E_reco, 16) && aligned(w0, 16) && aligned(channel, 2);
+#define OSC_K2_SINGLE(T)                                                                                               \
+    if (slots == 1 && threads == T)                                                                                    \
+        return vec ? launch_k2<true, T, 1>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale,         \
+                                           bin_edges, n_bins, 1, ms, hist_out)                                         \
+                   : launch_k2<false, T, 1>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale,        \
+                                            bin_edges, n_bins, 1, ms, hist_out);
+    OSC_K2_SINGLE(512) OSC_K2_SINGLE(384) OSC_K2_SINGLE(256)
+#undef OSC_K2_SINGLE
+    if (slots == 1) return fail(OSC_ERR_INVALID_ARG, "single-slot k2 is built for 256, 384 and 512 threads");
     if (threads == 768)
         return vec ? launch_k2<true, 768>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
                                           n_bins, n_sub_t, ms, hist_out)
                    : launch_k2<false, 768>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
-                                           n_bins, n_sub, ms, hist_out);
-    if (threads == 384)
-        return vec ? launch_k2<true, 384>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
-                                          n_bins, n_sub_t, ms, hist_out)
-                   : launch_k2<false, 384>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
                                            n_bins, n_sub, ms, hist_out);
     if (threads == 512)
         return vec ? launch_k2<true, 512>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,

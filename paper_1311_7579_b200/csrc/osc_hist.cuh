@@ -109,6 +109,45 @@ __device__ __forceinline__ void warp_hist_commit(const HistPlan& p, double w0, d
     }
 }
 
+// One sub-histogram per warp for both events of a lane (binnings whose two-slot layout leaves room for too few warps):
+// slot 0 is committed completely before slot 1 reads anything, so the order of the additions to one word is
+// slot 0 in lane order, then slot 1 in lane order.  Only slot 0 can be pre-read.
+__device__ __forceinline__ LaneHist lane_hist_single(const double* hist, int nh, unsigned warp)
+{
+    LaneHist lh;
+    lh.h0 = smem_u32(hist) + 8u * (warp * (unsigned)nh);
+    lh.h1 = lh.h0;
+    return lh;
+}
+
+__device__ __forceinline__ void warp_hist_rank_single(HistPlan& p, unsigned lt_mask, int& rmax1)
+{
+    const unsigned FULL = 0xffffffffu;
+    p.r0 = p.a0 != 0xFFFFFFFFu ? __popc(p.m0 & lt_mask) : -1;
+    p.r1 = p.a1 != 0xFFFFFFFFu ? __popc(p.m1 & lt_mask) : -1;
+    p.rmax = __reduce_max_sync(FULL, p.r0);
+    rmax1 = __reduce_max_sync(FULL, p.r1);
+    p.v0 = 0.0;
+    p.v1 = 0.0;
+    if (p.r0 == 0) p.v0 = lds_f64_volatile(p.a0);
+}
+
+__device__ __forceinline__ void warp_hist_commit_single(const HistPlan& p, int rmax1, double w0, double w1)
+{
+    if (p.r0 == 0) sts_f64_volatile(p.a0, p.v0 + w0);
+    __syncwarp();
+#pragma unroll 1
+    for (int ph = 1; ph <= p.rmax; ++ph) {
+        if (p.r0 == ph) sts_f64_volatile(p.a0, lds_f64_volatile(p.a0) + w0);
+        __syncwarp();
+    }
+#pragma unroll 1
+    for (int ph = 0; ph <= rmax1; ++ph) {
+        if (p.r1 == ph) sts_f64_volatile(p.a1, lds_f64_volatile(p.a1) + w1);
+        __syncwarp();
+    }
+}
+
 __device__ __forceinline__ void warp_hist_add2(const LaneHist& lh, int cell0, double w0, int cell1, double w1,
                                                unsigned lt_mask)
 {

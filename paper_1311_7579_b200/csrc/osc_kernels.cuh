@@ -288,7 +288,7 @@ __device__ __forceinline__ EventPair load_pair(const double* __restrict__ E_true
 }
 
 // Event loop of k2 (STEPS as in find_bin): software-pipelined by hand, see the kernel's comment.
-template <bool VEC, int THREADS, int STEPS>
+template <bool VEC, int THREADS, int STEPS, int SLOTS>
 __device__ __forceinline__ void k2_loop(const BinArgs& a, const double* __restrict__ E_true,
                                         const double* __restrict__ E_reco, const double* __restrict__ w0,
                                         const int8_t* __restrict__ channel, size_t n, double energy_scale,
@@ -313,16 +313,19 @@ __device__ __forceinline__ void k2_loop(const BinArgs& a, const double* __restri
         OscEig e0, e1;
         eig_solve(a.set, A0, rcp_pos(Es0), e0);             // a2b-a2d
         eig_solve(a.set, A1, rcp_pos(Es1), e1);
-        warp_hist_rank(plan, lt_mask);
+        int rmax1 = 0;
+        if (SLOTS == 2) warp_hist_rank(plan, lt_mask);
+        else warp_hist_rank_single(plan, lt_mask, rmax1);
         const double P0 = assemble(e0, A0, tr0);            // a2e-a2f
         const double P1 = assemble(e1, A1, tr1);
-        warp_hist_commit(plan, __dmul_rn(wp0, P0), __dmul_rn(wp1, P1));   // a3a, a3c
+        if (SLOTS == 2) warp_hist_commit(plan, __dmul_rn(wp0, P0), __dmul_rn(wp1, P1));   // a3a, a3c
+        else warp_hist_commit_single(plan, rmax1, __dmul_rn(wp0, P0), __dmul_rn(wp1, P1));
     }
 }
 
 // ------------------------------------------------------------------------------------------------
 // k2: fused reweight + histogram, one parameter set.
-// Shared memory per block:  param block | bin table | hist[warps][kSlots][n_sub][4 * nb]
+// Shared memory per block:  param block | bin table | hist[warps][SLOTS][n_sub][4 * nb]
 // The loop is software-pipelined by hand: the loads of the block's next tile are issued before the arithmetic
 // of the current one (the kernel is bound by instruction issue around the fp64 pipe, so a warp that sits on a
 // global load is an issue slot lost), and the histogram ranking (MATCH + first read) precedes the closed form.
@@ -330,7 +333,8 @@ __device__ __forceinline__ void k2_loop(const BinArgs& a, const double* __restri
 #ifndef OSC_K2_TPS
 #define OSC_K2_TPS 768
 #endif
-template <bool VEC, int THREADS>
+// SLOTS = 1: one sub-histogram per warp instead of one per (warp, event of the lane), see lane_hist_single.
+template <bool VEC, int THREADS, int SLOTS = kSlots>
 __global__ void __launch_bounds__(THREADS, THREADS >= 384 ? 1 : OSC_K2_TPS / THREADS)
 reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict__ E_true,
                     const double* __restrict__ E_reco, const double* __restrict__ w0,
@@ -348,7 +352,7 @@ reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict_
 
     const unsigned lane = threadIdx.x & 31u;
     const unsigned warp = threadIdx.x >> 5;
-    const int n_hist = WARPS * kSlots * n_sub;
+    const int n_hist = WARPS * SLOTS * n_sub;
 
     // tiles are counted in 32 bits (the host rejects n >= 2^32 tiles); pinned so that the loop does not recompute it
     const unsigned ntiles = pin_u32((unsigned)((n + 2 * THREADS - 1) / (2 * THREADS)));
@@ -362,15 +366,15 @@ reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict_
     bt.ekey = pin_u32(bt.ekey);
     bt.lut = pin_u32(bt.lut);
     const uint32_t pb = pin_u32(smem_u32(pbuf));
-    LaneHist lh = lane_hist(hist, nh, n_sub, warp, lane);
+    LaneHist lh = SLOTS == 2 ? lane_hist(hist, nh, n_sub, warp, lane) : lane_hist_single(hist, nh, warp);
     lh.h0 = pin_u32(lh.h0);
-    lh.h1 = pin_u32(lh.h1);
+    lh.h1 = SLOTS == 2 ? pin_u32(lh.h1) : lh.h0;
     const unsigned lt_mask = pin_u32((1u << lane) - 1u);
 
     if (bt.steps <= 1u)
-        k2_loop<VEC, THREADS, 1>(a, E_true, E_reco, w0, channel, n, energy_scale, bt, pb, lh, lt_mask, ntiles, t, cur);
+        k2_loop<VEC, THREADS, 1, SLOTS>(a, E_true, E_reco, w0, channel, n, energy_scale, bt, pb, lh, lt_mask, ntiles, t, cur);
     else
-        k2_loop<VEC, THREADS, 0>(a, E_true, E_reco, w0, channel, n, energy_scale, bt, pb, lh, lt_mask, ntiles, t, cur);
+        k2_loop<VEC, THREADS, 0, SLOTS>(a, E_true, E_reco, w0, channel, n, energy_scale, bt, pb, lh, lt_mask, ntiles, t, cur);
     block_merge(hist, n_hist, nh, ms, hist_out, &s_ticket);
 }
 

@@ -312,9 +312,29 @@ def test_dropped_and_bad_events_are_skipped(osc):
     assert_hist_close(got, oracle.reweight_bin(op, et, er, w0, ch, 1.0, edges), "bad events")
 
 
+@pytest.mark.parametrize("threads", [256, 384, 512])
+@pytest.mark.parametrize("nb", [1, 7, 50])
+def test_one_sub_histogram_per_warp_under_collisions(osc, monkeypatch, nb, threads):
+    """The layout of large binnings (one sub-histogram per warp for both events of a lane), forced onto few bins so that
+    most lanes of a warp, and both events of a lane, hit the same word: every weight must still arrive exactly once."""
+    n = 60_013
+    et, er, w0, ch = wl.events(n, seed=31 + nb)
+    er[:n // 3] = 0.7                                   # one third of all events in one bin
+    edges = wl.bin_edges(nb, 5.0)
+    op = set_params(osc, wl.table1())
+    ref = oracle.reweight_bin(op, et, er, w0, ch, 1.0, edges)
+    monkeypatch.setenv("OSC_TUNE_SLOTS", "1")
+    monkeypatch.setenv("OSC_TUNE_THREADS", str(threads))
+    for off in (0, 1):                                  # 128-bit and scalar loads
+        got = host(osc.osc_reweight_bin(dev(et)[off:], dev(er)[off:], dev(w0)[off:], dev(ch)[off:], 1.0, dev(edges)))
+        want = ref if off == 0 else oracle.reweight_bin(op, et[1:], er[1:], w0[1:], ch[1:], 1.0, edges)
+        assert_hist_close(got, want, f"single slot, {nb} bins, {threads} threads, off={off}")
+
+
 @pytest.mark.parametrize("nb,kind", [(1, "uniform"), (2, "uniform"), (3, "log"), (7, "random"), (50, "random"),
                                      (64, "uniform"), (140, "uniform"), (141, "random"), (200, "log"),
                                      (210, "uniform"), (215, "random"), (250, "uniform"), (290, "log"),
+                                     (425, "uniform"), (430, "random"), (570, "uniform"), (575, "log"),
                                      (768, "uniform")])
 def test_bin_layouts(osc, nb, kind):
     n = 30_007

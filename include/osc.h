@@ -103,7 +103,11 @@ int osc_prob_all(const double *E_true, size_t n, int antinu, double *P_out, void
  *   bin_edges           DEVICE [n_bins + 1] fp64, strictly increasing (not checked: device data)
  *   hist_out            DEVICE [OSC_N_CHANNELS][n_bins] fp64 row-major, OVERWRITTEN (zeroed when n == 0)
  * No per-event weight array is written to memory.  The result is bit-reproducible from run to run for
- * fixed inputs (fixed event -> thread map, fixed-order merges, no floating-point atomics). */
+ * fixed inputs (fixed event -> thread map, fixed-order merges, no floating-point atomics).
+ * The launch shape follows n_bins (one block per SM of 768, 512, 384 or 256 threads).  The
+ * environment variables OSC_TUNE_THREADS (128 | 256 | 384 | 512 | 768), OSC_TUNE_SLOTS (1 | 2), OSC_TUNE_NSUB and
+ * OSC_TUNE_BPS, read at every call, override it for measurements and tests; a combination that does not fit in
+ * shared memory returns OSC_ERR_INVALID_ARG or OSC_ERR_CUDA, never a wrong histogram. */
 int osc_reweight_bin(const double *E_true, const double *E_reco, const double *w0, const int8_t *channel,
                      size_t n, double energy_scale, const double *bin_edges, int n_bins, double *hist_out,
                      void *stream);

@@ -242,7 +242,11 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     // 256 threads: two sub-histograms per slot halve the collisions inside a warp; taken when 3 blocks still fit
     const int n_sub = (slots == kSlots && threads == 256 && 3 * (k2_smem_bytes(n_bins, 256, 2) + 1024) <= kSmemBudget) ? 2 : 1;
     int n_sub_t = n_sub;
-    if (const char* e = getenv("OSC_TUNE_NSUB")) n_sub_t = slots == kSlots ? atoi(e) : 1;
+    if (const char* e = getenv("OSC_TUNE_NSUB")) {
+        n_sub_t = slots == kSlots ? atoi(e) : 1;
+        if (n_sub_t != 1 && n_sub_t != 2 && n_sub_t != 4)
+            return fail(OSC_ERR_INVALID_ARG, "OSC_TUNE_NSUB = %s: 1, 2 or 4 sub-histograms per slot", e);
+    }
     const size_t smem = k2_smem_bytes(n_bins, threads, n_sub_t, slots);
     if (smem + 1024 > (size_t)227 * 1024)
         return fail(OSC_ERR_INVALID_ARG, "%d bins with %d threads and %d slot(s) need %zu bytes of shared memory", n_bins,
@@ -285,21 +289,21 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
         return vec ? launch_k2<true, 768>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
                                           n_bins, n_sub_t, ms, hist_out)
                    : launch_k2<false, 768>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
-                                           n_bins, n_sub, ms, hist_out);
+                                           n_bins, n_sub_t, ms, hist_out);
     if (threads == 512)
         return vec ? launch_k2<true, 512>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
                                           n_bins, n_sub_t, ms, hist_out)
                    : launch_k2<false, 512>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
-                                           n_bins, n_sub, ms, hist_out);
+                                           n_bins, n_sub_t, ms, hist_out);
     if (threads == 256)
         return vec ? launch_k2<true, 256>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
                                           n_bins, n_sub_t, ms, hist_out)
                    : launch_k2<false, 256>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
-                                           n_bins, n_sub, ms, hist_out);
+                                           n_bins, n_sub_t, ms, hist_out);
     return vec ? launch_k2<true, 128>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
                                       n_bins, n_sub_t, ms, hist_out)
                : launch_k2<false, 128>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
-                                       n_bins, n_sub, ms, hist_out);
+                                       n_bins, n_sub_t, ms, hist_out);
 }
 
 template <bool VEC, int NS>

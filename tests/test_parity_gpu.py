@@ -329,6 +329,8 @@ def test_one_sub_histogram_per_warp_under_collisions(osc, monkeypatch, nb, threa
         got = host(osc.osc_reweight_bin(dev(et)[off:], dev(er)[off:], dev(w0)[off:], dev(ch)[off:], 1.0, dev(edges)))
         want = ref if off == 0 else oracle.reweight_bin(op, et[1:], er[1:], w0[1:], ch[1:], 1.0, edges)
         assert_hist_close(got, want, f"single slot, {nb} bins, {threads} threads, off={off}")
+        again = host(osc.osc_reweight_bin(dev(et)[off:], dev(er)[off:], dev(w0)[off:], dev(ch)[off:], 1.0, dev(edges)))
+        assert np.array_equal(got, again), "not bit-reproducible"
 
 
 @pytest.mark.parametrize("nb,kind", [(1, "uniform"), (2, "uniform"), (3, "log"), (7, "random"), (50, "random"),

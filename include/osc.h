@@ -104,10 +104,8 @@ int osc_prob_all(const double *E_true, size_t n, int antinu, double *P_out, void
  *   hist_out            DEVICE [OSC_N_CHANNELS][n_bins] fp64 row-major, OVERWRITTEN (zeroed when n == 0)
  * No per-event weight array is written to memory.  The result is bit-reproducible from run to run for
  * fixed inputs (fixed event -> thread map, fixed-order merges, no floating-point atomics).
- * The launch shape follows n_bins (one block per SM of 768, 512, 384 or 256 threads).  The
- * environment variables OSC_TUNE_THREADS (128 | 256 | 384 | 512 | 768), OSC_TUNE_SLOTS (1 | 2), OSC_TUNE_NSUB and
- * OSC_TUNE_BPS, read at every call, override it for measurements and tests; a combination that does not fit in
- * shared memory returns OSC_ERR_INVALID_ARG or OSC_ERR_CUDA, never a wrong histogram. */
+ * The launch shape follows n_bins (one block per SM of 768, 512, 384 or 256 threads);
+ * osc_set_k2_tuning overrides it for measurements and tests.  No environment variable is read. */
 int osc_reweight_bin(const double *E_true, const double *E_reco, const double *w0, const int8_t *channel,
                      size_t n, double energy_scale, const double *bin_edges, int n_bins, double *hist_out,
                      void *stream);
@@ -139,8 +137,7 @@ int osc_reweight_bin_scales(const double *E_true, const double *E_reco, const do
  *     2e6 events), on the events sorted by histogram cell, with the weights of a cell summed in registers
  *     (kernel k5); below that the sort does not pay and every point gets its own pass of
  *     osc_reweight_bin's kernel (k2).  Binnings up to the library's limit of 768 bins are taken by all paths.
- * The environment variable OSC_BATCH_PATH = k2 | k4 | k5, read at every call, forces one path (tests use
- * it to check the paths on the same inputs); any other value, or none, leaves the choice to the library. */
+ * osc_set_batch_path forces one path (tests use it to check the paths on the same inputs). */
 int osc_reweight_bin_batch(const osc_params *points, int n_points, const double *E_true,
                            const double *E_reco, const double *w0, const int8_t *channel, size_t n,
                            double energy_scale, const double *bin_edges, int n_bins, double *hist_out,
@@ -211,6 +208,18 @@ int osc_reweight_bin_host(const double *E_true_host, const double *E_reco_host, 
 int osc_reweight_bin_scales_host(const double *E_true_host, const double *E_reco_host, const double *w0_host,
                                  const int8_t *channel_host, size_t n, const double *energy_scales, int n_scales,
                                  const double *bin_edges_host, int n_bins, double *hist_out_host);
+
+/* Measurement and test overrides (process-wide, thread-safe; they affect calls enqueued afterwards).
+ *   osc_set_batch_path  path = "auto" (default: the library chooses, see osc_reweight_bin_batch), "k2", "k4" or "k5":
+ *                       the code path of osc_reweight_bin_batch / osc_plan_reweight_bin_batch ("k2" does not apply to plans).
+ *   osc_set_k2_tuning   launch shape of osc_reweight_bin's kernel; 0 leaves a field to the library.
+ *                       threads in {128, 256, 384, 512, 768}, slots in {1, 2} (sub-histograms per warp: one, or one per
+ *                       event of the lane), n_sub in {1, 2, 4} (sub-histograms per slot), blocks_per_sm <= 16.
+ *                       A combination that does not fit in shared memory makes the call it would shape return
+ *                       OSC_ERR_INVALID_ARG or OSC_ERR_CUDA, never a wrong histogram.
+ * Both return OSC_ERR_INVALID_ARG (state unchanged) for any other value. */
+int osc_set_batch_path(const char *path);
+int osc_set_k2_tuning(int threads, int slots, int n_sub, int blocks_per_sm);
 
 /* Message of the calling thread's most recent error ("" if none).  Never NULL. */
 const char *osc_last_error(void);

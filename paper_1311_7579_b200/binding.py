@@ -9,6 +9,7 @@ from __future__ import annotations
 
 import ctypes
 import os
+import threading
 from typing import Mapping, Optional, Sequence
 
 import numpy as np
@@ -26,7 +27,8 @@ PARAM_FIELDS = ("sin2_th12", "sin2_th23", "sin2_th13", "dm2_32", "dm2_21", "delt
 EXPORTS = ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_scales", "osc_reweight_bin_batch",
            "osc_plan_create", "osc_plan_reweight_bin", "osc_plan_reweight_bin_batch", "osc_plan_destroy",
            "osc_neg2lnl", "osc_bin_centre_compare", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_reweight_bin_scales_host", "osc_last_error", "osc_launch_count",
-           "osc_version", "osc_set_device", "osc_get_device", "osc_fp64_peak_probe")
+           "osc_version", "osc_set_device", "osc_get_device", "osc_fp64_peak_probe", "osc_set_batch_path",
+           "osc_set_k2_tuning")
 
 
 class OscError(RuntimeError):
@@ -72,12 +74,14 @@ def lib() -> ctypes.CDLL:
     L.osc_set_device.argtypes = [i]
     L.osc_get_device.argtypes = [ctypes.POINTER(i)]
     L.osc_fp64_peak_probe.argtypes = [i, i, ctypes.POINTER(d), vp]
+    L.osc_set_batch_path.argtypes = [ctypes.c_char_p]
+    L.osc_set_k2_tuning.argtypes = [i, i, i, i]
     for name in ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_scales",
                  "osc_reweight_bin_batch",
                  "osc_plan_create", "osc_plan_reweight_bin", "osc_plan_reweight_bin_batch", "osc_plan_destroy",
                  "osc_neg2lnl", "osc_bin_centre_compare", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_reweight_bin_scales_host", "osc_set_device",
                  "osc_get_device",
-                 "osc_fp64_peak_probe"):
+                 "osc_fp64_peak_probe", "osc_set_batch_path", "osc_set_k2_tuning"):
         getattr(L, name).restype = i
     L.osc_last_error.restype = ctypes.c_char_p
     L.osc_version.restype = ctypes.c_char_p
@@ -111,17 +115,16 @@ def _dev(t, dtype, what: str) -> int:
     return t.data_ptr()
 
 
-_cur_dev = None
+_tls = threading.local()       # the current CUDA device is a per-thread property, and so is this cache of it
 
 
 def _sync_device(index: Optional[int]) -> None:
     """Align the library's (statically linked) CUDA runtime with the device of the tensors."""
-    global _cur_dev
     if index is None:
         index = 0
-    if _cur_dev != index:
+    if getattr(_tls, "dev", None) != index:
         _check(lib().osc_set_device(int(index)))
-        _cur_dev = index
+        _tls.dev = index
 
 
 def _host(a: np.ndarray, dtype, what: str) -> int:
@@ -154,6 +157,8 @@ def osc_prob(E_true, flavour_in: int, flavour_out: int, antinu: int, P_out=None,
     n = E_true.numel()
     if P_out is None:
         P_out = torch.empty_like(E_true)
+    if P_out.numel() != n:
+        raise ValueError("P_out must hold n values")
     _check(lib().osc_prob(_dev(E_true, torch.float64, "E_true"), n, flavour_in, flavour_out, int(antinu),
                           _dev(P_out, torch.float64, "P_out"), _stream(stream)))
     return P_out
@@ -183,12 +188,19 @@ def _event_ptrs(E_true, E_reco, w0, channel):
             _dev(w0, torch.float64, "w0") if w0 is not None else None, _dev(channel, torch.int8, "channel"))
 
 
+def _n_bins(bin_edges) -> int:
+    nb = (bin_edges.numel() if hasattr(bin_edges, "numel") else bin_edges.size) - 1
+    if nb < 1:
+        raise ValueError("bin_edges must hold at least two edges")
+    return nb
+
+
 def osc_reweight_bin(E_true, E_reco, w0, channel, energy_scale: float, bin_edges, hist_out=None, stream=None):
     """[N_CHANNELS, n_bins] histogram tensor (overwritten)."""
     import torch
 
+    nb = _n_bins(bin_edges)
     n, pt, pr, pw, pc = _event_ptrs(E_true, E_reco, w0, channel)
-    nb = bin_edges.numel() - 1
     if hist_out is None:
         hist_out = torch.empty((N_CHANNELS, nb), dtype=torch.float64, device=E_true.device)
     if hist_out.numel() != N_CHANNELS * nb:
@@ -203,8 +215,8 @@ def osc_reweight_bin_scales(E_true, E_reco, w0, channel, energy_scales: Sequence
     """[n_scales, N_CHANNELS, n_bins] histograms, one slice per energy-scale value, in one pass over the events."""
     import torch
 
+    nb = _n_bins(bin_edges)
     n, pt, pr, pw, pc = _event_ptrs(E_true, E_reco, w0, channel)
-    nb = bin_edges.numel() - 1
     ns = len(energy_scales)
     arr = (ctypes.c_double * max(ns, 1))(*[float(v) for v in energy_scales])
     if hist_out is None:
@@ -227,8 +239,8 @@ def osc_reweight_bin_batch(points: Sequence, E_true, E_reco, w0, channel, energy
     """[n_points, N_CHANNELS, n_bins] histograms, one slice per parameter set, in one call."""
     import torch
 
+    nb = _n_bins(bin_edges)
     n, pt, pr, pw, pc = _event_ptrs(E_true, E_reco, w0, channel)
-    nb = bin_edges.numel() - 1
     npts = len(points)
     arr = points if isinstance(points, ctypes.Array) else pack_params(points)
     if hist_out is None:
@@ -258,8 +270,8 @@ class OscPlan:
 def osc_plan_create(E_true, E_reco, w0, channel, energy_scale: float, bin_edges, stream=None) -> OscPlan:
     import torch
 
+    nb = _n_bins(bin_edges)
     n, pt, pr, pw, pc = _event_ptrs(E_true, E_reco, w0, channel)
-    nb = bin_edges.numel() - 1
     out = ctypes.c_void_p()
     _check(lib().osc_plan_create(pt, pr, pw, pc, n, float(energy_scale), _dev(bin_edges, torch.float64, "bin_edges"), nb,
                                  _stream(stream), ctypes.byref(out)))
@@ -321,7 +333,7 @@ def osc_bin_centre_compare(E_true, w0, channel, bin_edges, stream=None):
     import torch
 
     n, pt, _, pw, pc = _event_ptrs(E_true, E_true, w0, channel)
-    nb = bin_edges.numel() - 1
+    nb = _n_bins(bin_edges)
     he = torch.empty((N_CHANNELS, nb), dtype=torch.float64, device=E_true.device)
     hc = torch.empty_like(he)
     _check(lib().osc_bin_centre_compare(pt, pw, pc, n, _dev(bin_edges, torch.float64, "bin_edges"), nb,
@@ -333,8 +345,10 @@ def osc_bin_centre_compare(E_true, w0, channel, bin_edges, stream=None):
 def osc_bin_index(E_true, E_reco, channel, energy_scale: float, bin_edges, bin_out=None, stream=None):
     import torch
 
+    nb = _n_bins(bin_edges)
+    if bin_out is not None and bin_out.numel() != E_true.numel():
+        raise ValueError("bin_out must hold n values")
     n, pt, pr, _, pc = _event_ptrs(E_true, E_reco, None, channel)
-    nb = bin_edges.numel() - 1
     if bin_out is None:
         bin_out = torch.empty(n, dtype=torch.int32, device=E_true.device)
     _check(lib().osc_bin_index(pt, pr, pc, n, float(energy_scale), _dev(bin_edges, torch.float64, "bin_edges"), nb,
@@ -347,6 +361,8 @@ def osc_prob_host(E_true: np.ndarray, flavour_in: int, flavour_out: int, antinu:
     """Host buffers in and out (the flow of the paper's Listing 1): H2D, kernel, D2H, synchronise."""
     if P_out is None:
         P_out = np.empty_like(E_true)
+    if P_out.size != E_true.size:
+        raise ValueError("P_out must hold n values")
     _check(lib().osc_prob_host(_host(E_true, np.float64, "E_true"), E_true.size, flavour_in, flavour_out,
                                int(antinu), _host(P_out, np.float64, "P_out")))
     return P_out
@@ -355,14 +371,33 @@ def osc_prob_host(E_true: np.ndarray, flavour_in: int, flavour_out: int, antinu:
 def osc_reweight_bin_host(E_true: np.ndarray, E_reco: np.ndarray, w0: np.ndarray, channel: np.ndarray,
                           energy_scale: float, bin_edges: np.ndarray,
                           hist_out: Optional[np.ndarray] = None) -> np.ndarray:
-    nb = bin_edges.size - 1
+    nb = _n_bins(bin_edges)
     if hist_out is None:
         hist_out = np.empty((N_CHANNELS, nb), dtype=np.float64)
+    _check_host_events(E_true, E_reco, w0, channel)
+    if hist_out.size != N_CHANNELS * nb:
+        raise ValueError("hist_out must hold N_CHANNELS * n_bins values")
     _check(lib().osc_reweight_bin_host(_host(E_true, np.float64, "E_true"), _host(E_reco, np.float64, "E_reco"),
                                        _host(w0, np.float64, "w0"), _host(channel, np.int8, "channel"), E_true.size,
                                        float(energy_scale), _host(bin_edges, np.float64, "bin_edges"), nb,
                                        _host(hist_out, np.float64, "hist_out")))
     return hist_out
+
+
+def _check_host_events(E_true, E_reco, w0, channel) -> None:
+    n = E_true.size
+    if E_reco.size != n or w0.size != n or channel.size != n:
+        raise ValueError("host event arrays differ in length")
+
+
+def osc_set_batch_path(path: str) -> None:
+    """"auto" | "k2" | "k4" | "k5": code path of the batched calls (measurements and tests)."""
+    _check(lib().osc_set_batch_path(path.encode()))
+
+
+def osc_set_k2_tuning(threads: int = 0, slots: int = 0, n_sub: int = 0, blocks_per_sm: int = 0) -> None:
+    """Launch shape of osc_reweight_bin's kernel; 0 leaves a field to the library (measurements and tests)."""
+    _check(lib().osc_set_k2_tuning(int(threads), int(slots), int(n_sub), int(blocks_per_sm)))
 
 
 def osc_last_error() -> str:
@@ -378,9 +413,8 @@ def osc_version() -> str:
 
 
 def osc_set_device(device: int) -> None:
-    global _cur_dev
     _check(lib().osc_set_device(int(device)))
-    _cur_dev = int(device)
+    _tls.dev = int(device)
 
 
 def osc_get_device() -> int:
@@ -400,11 +434,14 @@ def osc_reweight_bin_scales_host(E_true: np.ndarray, E_reco: np.ndarray, w0: np.
                                  energy_scales: Sequence[float], bin_edges: np.ndarray,
                                  hist_out: Optional[np.ndarray] = None) -> np.ndarray:
     """Host buffers in and out, several energy scales, one trip of the events over PCIe."""
-    nb = bin_edges.size - 1
+    nb = _n_bins(bin_edges)
     ns = len(energy_scales)
     if hist_out is None:
         hist_out = np.empty((ns, N_CHANNELS, nb), dtype=np.float64)
     arr = (ctypes.c_double * max(ns, 1))(*[float(v) for v in energy_scales])
+    _check_host_events(E_true, E_reco, w0, channel)
+    if hist_out.size != ns * N_CHANNELS * nb:
+        raise ValueError("hist_out must hold n_scales * N_CHANNELS * n_bins values")
     _check(lib().osc_reweight_bin_scales_host(_host(E_true, np.float64, "E_true"), _host(E_reco, np.float64, "E_reco"),
                                               _host(w0, np.float64, "w0"), _host(channel, np.int8, "channel"),
                                               E_true.size, arr, ns, _host(bin_edges, np.float64, "bin_edges"), nb,

@@ -10,6 +10,7 @@
 #include <array>
 #include <complex>
 #include <map>
+#include <memory>
 #include <mutex>
 #include <new>
 #include <utility>
@@ -30,6 +31,11 @@ std::mutex g_mu;
 HostSet g_state;
 bool g_configured = false;
 std::atomic<unsigned long long> g_launches{0};
+
+// Measurement / test overrides (osc_set_batch_path, osc_set_k2_tuning); 0 = the library chooses.  Never read from
+// the environment: a stray variable must not change launch shapes in a fitter that calls the library 1e6 times.
+std::atomic<int> g_batch_path{0};                       // 0 auto, 2 k2, 4 k4, 5 k5
+std::atomic<int> g_tune_threads{0}, g_tune_slots{0}, g_tune_nsub{0}, g_tune_bps{0};
 
 int fail(int code, const char* fmt, ...)
 {
@@ -150,16 +156,32 @@ constexpr size_t kCounterBytes = 4096;
 struct StreamScratch {
     char* buf = nullptr;
     size_t cap = 0;
+    std::mutex mu;            // held from the hand-out of the buffer until the launch that uses it is enqueued
 };
 std::mutex g_scratch_mu;
-std::map<std::pair<int, cudaStream_t>, StreamScratch> g_scratch;
+std::map<std::pair<int, cudaStream_t>, std::unique_ptr<StreamScratch>> g_scratch;
 
-int stream_scratch(size_t bytes, cudaStream_t st, char** out)
+// The buffer of (current device, stream) with at least `bytes` bytes.  The lease keeps the entry locked: a second host
+// thread that enqueues on the same stream waits until the first one has launched, so a buffer that is about to be
+// replaced (grown) is never handed to a launch that has not been enqueued yet.
+struct ScratchLease {
+    std::unique_lock<std::mutex> lk;
+    char* p = nullptr;
+};
+
+int stream_scratch(size_t bytes, cudaStream_t st, ScratchLease& lease)
 {
     int dev = 0;
     CUDA_TRY(cudaGetDevice(&dev));
-    std::lock_guard<std::mutex> lk(g_scratch_mu);
-    StreamScratch& s = g_scratch[std::make_pair(dev, st)];
+    StreamScratch* sp = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(g_scratch_mu);
+        std::unique_ptr<StreamScratch>& e = g_scratch[std::make_pair(dev, st)];
+        if (!e) e.reset(new StreamScratch);
+        sp = e.get();
+    }
+    lease.lk = std::unique_lock<std::mutex>(sp->mu);
+    StreamScratch& s = *sp;
     if (s.cap < bytes) {
         if (s.buf) CUDA_TRY(cudaFreeAsync(s.buf, st));
         s.buf = nullptr;
@@ -175,7 +197,7 @@ int stream_scratch(size_t bytes, cudaStream_t st, char** out)
         s.buf = p;
         s.cap = cap;
     }
-    *out = s.buf;
+    lease.p = s.buf;
     return OSC_OK;
 }
 
@@ -218,8 +240,8 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     // 85 us, the second 102 us and the third 127 us, and the SM spent the end of the kernel on 8 warps.  The warps of
     // ONE block are all the same age and finish together (measured: 137 -> 129 us per 1e7 events); a static
     // re-weighting of the shares does not work, the slot of a block on its SM is not known in advance.  (Several
-    // blocks of 256 or 128 threads with two-slot sub-histograms remain reachable through OSC_TUNE_THREADS /
-    // OSC_TUNE_SLOTS for measurements: 147-230 us and 150-420 us over the same range of binnings.)
+    // blocks of 256 or 128 threads with two-slot sub-histograms remain reachable through
+    // osc_set_k2_tuning for measurements: 147-230 us and 150-420 us over the same range of binnings.)
     int threads = 256, slots = 1;
     if (k2_smem_bytes(n_bins, 768, 1) + 1024 <= kSmemBudget) {
         threads = 768;
@@ -232,30 +254,26 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     } else if (k2_smem_bytes(n_bins, 384, 1, 1) + 1024 <= kSmemBudget) {
         threads = 384;
     }
-    if (const char* e = getenv("OSC_TUNE_SLOTS")) slots = atoi(e) == 1 ? 1 : kSlots;
-    if (const char* e = getenv("OSC_TUNE_THREADS")) {
-        threads = atoi(e);
-        if (threads != 768 && threads != 512 && threads != 384 && threads != 256 && threads != 128)
-            return fail(OSC_ERR_INVALID_ARG, "OSC_TUNE_THREADS = %s: k2 is built for 128, 256, 384, 512 and 768 threads", e);
+    const int t_threads = g_tune_threads.load(), t_slots = g_tune_slots.load(), t_nsub = g_tune_nsub.load();
+    const int t_bps = g_tune_bps.load();
+    if (t_slots) slots = t_slots == 1 ? 1 : kSlots;
+    if (t_threads) {
+        threads = t_threads;
         if (threads == 384) slots = 1;
     }
     // 256 threads: two sub-histograms per slot halve the collisions inside a warp; taken when 3 blocks still fit
     const int n_sub = (slots == kSlots && threads == 256 && 3 * (k2_smem_bytes(n_bins, 256, 2) + 1024) <= kSmemBudget) ? 2 : 1;
     int n_sub_t = n_sub;
-    if (const char* e = getenv("OSC_TUNE_NSUB")) {
-        n_sub_t = slots == kSlots ? atoi(e) : 1;
-        if (n_sub_t != 1 && n_sub_t != 2 && n_sub_t != 4)
-            return fail(OSC_ERR_INVALID_ARG, "OSC_TUNE_NSUB = %s: 1, 2 or 4 sub-histograms per slot", e);
-    }
+    if (t_nsub) n_sub_t = slots == kSlots ? t_nsub : 1;
     const size_t smem = k2_smem_bytes(n_bins, threads, n_sub_t, slots);
     if (smem + 1024 > (size_t)227 * 1024)
         return fail(OSC_ERR_INVALID_ARG, "%d bins with %d threads and %d slot(s) need %zu bytes of shared memory", n_bins,
                     threads, slots, smem);
     size_t per_sm = kSmemBudget / (smem + 1024);
-    if (const char* e = getenv("OSC_TUNE_BPS")) per_sm = (size_t)atoi(e);
+    if (t_bps) per_sm = (size_t)t_bps;
     if (per_sm < 1) per_sm = 1;
     const size_t max_per_sm = threads >= 384 ? 1 : threads == 256 ? 3 : 6;   // __launch_bounds__(THREADS, 768 / THREADS) of k2
-    if (per_sm > max_per_sm && !getenv("OSC_TUNE_BPS")) per_sm = max_per_sm;
+    if (per_sm > max_per_sm && !t_bps) per_sm = max_per_sm;
     const size_t ntiles = (n + 2 * threads - 1) / (2 * (size_t)threads);
     if (ntiles > 0xFFFFFFFFull) return fail(OSC_ERR_INVALID_ARG, "n = %zu events is more than one call takes (2^32 tiles)", n);
     size_t g = (size_t)sms * per_sm;
@@ -267,8 +285,9 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
         return fail(OSC_ERR_CUDA, "merge ticket area too small for %d groups", ngroups);
     const size_t bytes_partial = (size_t)grid * nh * sizeof(double);
     const size_t bytes_gpartial = (size_t)ngroups * nh * sizeof(double);
-    char* scratch = nullptr;
-    if ((rc = stream_scratch(kCounterBytes + bytes_partial + bytes_gpartial, st, &scratch))) return rc;
+    ScratchLease lease;
+    if ((rc = stream_scratch(kCounterBytes + bytes_partial + bytes_gpartial, st, lease))) return rc;
+    char* scratch = lease.p;
     MergeScratch ms;
     ms.counters = reinterpret_cast<unsigned int*>(scratch);
     ms.partial = reinterpret_cast<double*>(scratch + kCounterBytes);
@@ -341,8 +360,9 @@ int launch_reweight_scales(const BinArgs& args, const double* E_true, const doub
     const int ngroups = (grid + kGroup - 1) / kGroup;
     const size_t bytes_partial = (size_t)grid * nht * sizeof(double);
     const size_t bytes_gpartial = (size_t)ngroups * nht * sizeof(double);
-    char* scratch = nullptr;
-    if ((rc = stream_scratch(kCounterBytes + bytes_partial + bytes_gpartial, st, &scratch))) return rc;
+    ScratchLease lease;
+    if ((rc = stream_scratch(kCounterBytes + bytes_partial + bytes_gpartial, st, lease))) return rc;
+    char* scratch = lease.p;
     MergeScratch ms;
     ms.counters = reinterpret_cast<unsigned int*>(scratch);
     ms.partial = reinterpret_cast<double*>(scratch + kCounterBytes);
@@ -383,7 +403,16 @@ struct HostPath {
         return OSC_OK;
     }
 };
-HostPath g_host;
+HostPath g_hosts[64];          // one per device: a stream and a cudaMalloc'd buffer belong to the device they were made on
+
+int host_path(HostPath** out)
+{
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return fail(OSC_ERR_CUDA, "device index %d out of range", dev);
+    *out = &g_hosts[dev];
+    return OSC_OK;
+}
 
 } // namespace
 
@@ -504,9 +533,11 @@ struct PinnedRing {
     int next = 0;
     std::mutex mu;
 
-    int acquire(size_t bytes, Slot** out)
+    // `lk` stays locked until the caller has filled the slot, enqueued the copy that reads it and called fence():
+    // a concurrent caller cannot be handed a slot that is still being filled.
+    int acquire(size_t bytes, Slot** out, std::unique_lock<std::mutex>& lk)
     {
-        std::lock_guard<std::mutex> lk(mu);
+        lk = std::unique_lock<std::mutex>(mu);
         Slot& s = slot[next];
         next = (next + 1) % kSlots;
         if (s.in_flight) {
@@ -800,7 +831,8 @@ int scan_run(const SortedEvents& se, const ScanPlan* plan, const std::vector<Bin
     PinnedRing* ring = nullptr;
     if ((rc = ring_for_device(&ring))) return rc;
     PinnedRing::Slot* slot = nullptr;
-    if ((rc = ring->acquire(b_groups + b_subs, &slot))) return rc;
+    std::unique_lock<std::mutex> ring_lock;
+    if ((rc = ring->acquire(b_groups + b_subs, &slot, ring_lock))) return rc;
     if (plan) {
         std::memcpy(slot->host, plan->groups.data(), plan->groups.size() * sizeof(ScanGroup));
         std::memcpy(static_cast<char*>(slot->host) + b_groups, plan->subs.data(), plan->subs.size() * sizeof(ScanSub));
@@ -809,6 +841,7 @@ int scan_run(const SortedEvents& se, const ScanPlan* plan, const std::vector<Bin
     }
     CUDA_TRY(cudaMemcpyAsync(d_groups, slot->host, b_groups + b_subs, cudaMemcpyHostToDevice, st));
     if ((rc = ring->fence(slot, st))) return rc;
+    ring_lock.unlock();
 
     const dim3 grid((geo.max_units + kScanWarps - 1) / kScanWarps, (unsigned)slots);
     if (plan) {
@@ -933,14 +966,14 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
     }
     // Points that differ only in theta23 and delta_cp share the eigen-problem: when the list has enough of that
     // structure (a scan grid), the factorised path k4 does the eigen-solve once per group (osc_scan.cuh).
-    // OSC_BATCH_PATH = k2 | k4 | k5 overrides the choice (tests exercise all paths on the same inputs).
+    // osc_set_batch_path overrides the choice (tests exercise all paths on the same inputs).
+    const int forced = g_batch_path.load();
     {
         ScanPlan plan;
         build_scan_plan(points, n_points, plan);
         bool use_scan = (size_t)n_points >= 8 * plan.subs.size();
-        const char* e = getenv("OSC_BATCH_PATH");
-        if (e && !std::strcmp(e, "k4")) use_scan = true;
-        if (e && (!std::strcmp(e, "k2") || !std::strcmp(e, "k5"))) use_scan = false;
+        if (forced == 4) use_scan = true;
+        if (forced == 2 || forced == 5) use_scan = false;
         if (use_scan)
             return launch_batch_scan(&plan, nullptr, n_points, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
                                      n_bins, hist_out, st);
@@ -957,10 +990,8 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
     // on a B200, k5 is ahead from 4 points on at 1e6 events and from 10 points on at 1e7.  Below that every point gets
     // its own k2 pass.
     bool use_full = n_points >= (n <= 2000000 ? 4 : 10);
-    if (const char* e = getenv("OSC_BATCH_PATH")) {
-        if (!std::strcmp(e, "k5")) use_full = true;
-        if (!std::strcmp(e, "k2")) use_full = false;
-    }
+    if (forced == 5) use_full = true;
+    if (forced == 2) use_full = false;
     if (use_full)
         return launch_batch_scan(nullptr, &blocks, n_points, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
                                  n_bins, hist_out, st);
@@ -1056,10 +1087,9 @@ int osc_plan_reweight_bin_batch(const osc_plan* plan, const osc_params* points, 
     ScanPlan sp;
     build_scan_plan(points, n_points, sp);
     bool use_scan = (size_t)n_points >= 8 * sp.subs.size();
-    if (const char* e = getenv("OSC_BATCH_PATH")) {
-        if (!std::strcmp(e, "k4")) use_scan = true;
-        if (!std::strcmp(e, "k5")) use_scan = false;
-    }
+    const int forced = g_batch_path.load();
+    if (forced == 4) use_scan = true;
+    if (forced == 5) use_scan = false;
     if (use_scan) return scan_run(pl->se, &sp, nullptr, n_points, hist_out, st);
     std::vector<BinArgs> blocks((size_t)n_points);
     for (int p = 0; p < n_points; ++p) {
@@ -1085,8 +1115,9 @@ int osc_plan_reweight_bin(const osc_plan* plan, double* hist_out, void* stream)
     // launches and nothing else on the stream
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const SortedEvents& se = pl->se;
-    char* scratch = nullptr;
-    if ((rc = stream_scratch(kCounterBytes + (size_t)se.geo.max_units * sizeof(double), st, &scratch))) return rc;
+    ScratchLease lease;
+    if ((rc = stream_scratch(kCounterBytes + (size_t)se.geo.max_units * sizeof(double), st, lease))) return rc;
+    char* scratch = lease.p;
     double* partial = reinterpret_cast<double*>(scratch + kCounterBytes);
     const ChannelKinds kinds = channel_kinds();
     scan_full_one_kernel<<<(se.geo.max_units + kScanWarps - 1) / kScanWarps, 32 * kScanWarps, 0, st>>>(
@@ -1112,6 +1143,15 @@ int osc_bin_centre_compare(const double* E_true, const double* w0, const int8_t*
     make_bin_args(h, args);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const int nh = kChannels * n_bins;
+    // launch shape of the unit histogram, fixed before anything is enqueued: a sub-histogram per (warp, event of the
+    // lane) while that fits, one per warp above (768 bins: 8 warps x 4 x 768 x 8 B = 196 kB)
+    const size_t sub2 = sizeof(double) * (kBlock / 32) * kSlots * (size_t)nh;
+    const bool two_slots = bin_table_bytes(n_bins) + sub2 + 1024 <= kSmemBudget;
+    const size_t sub1 = two_slots ? sub2 : sub2 / kSlots;
+    const int n_sub = two_slots && bin_table_bytes(n_bins) + 2 * sub1 <= 100 * 1024 ? 2 : 1;
+    const size_t smem = bin_table_bytes(n_bins) + n_sub * sub1;
+    if (smem + 1024 > (size_t)227 * 1024)
+        return fail(OSC_ERR_INVALID_ARG, "n_bins = %d needs more shared memory than one SM has", n_bins);
     // event by event: the fused kernel with the true energy in the role of the binned energy
     if ((rc = launch_reweight(args, E_true, E_true, w0, channel, n, 1.0, bin_edges, n_bins, hist_event_out, st))) return rc;
     // bin centre: unoscillated content of every true-energy bin, times the probability at the centre
@@ -1120,26 +1160,28 @@ int osc_bin_centre_compare(const double* E_true, const double* w0, const int8_t*
     } else {
         int sms = 0;
         if ((rc = sm_count(&sms))) return rc;
-        const size_t sub1 = sizeof(double) * (kBlock / 32) * kSlots * (size_t)nh;
-        const int n_sub = bin_table_bytes(n_bins) + 2 * sub1 <= 100 * 1024 ? 2 : 1;
-        const size_t smem = bin_table_bytes(n_bins) + n_sub * sub1;
-        if (smem > kSmemBudget) return fail(OSC_ERR_INVALID_ARG, "n_bins = %d needs more shared memory than one SM has", n_bins);
         const size_t ntiles = (n + 2 * kBlock - 1) / (2 * (size_t)kBlock);
         size_t g = (size_t)sms * (smem <= 100 * 1024 ? 2 : 1);
         if (ntiles < g) g = ntiles;
         const int grid = (int)g;
         const int ngroups = (grid + kGroup - 1) / kGroup;
         const size_t bytes_partial = (size_t)grid * nh * sizeof(double), bytes_gpartial = (size_t)ngroups * nh * sizeof(double);
-        char* scratch = nullptr;
-        if ((rc = stream_scratch(kCounterBytes + bytes_partial + bytes_gpartial, st, &scratch))) return rc;
+        ScratchLease lease;
+        if ((rc = stream_scratch(kCounterBytes + bytes_partial + bytes_gpartial, st, lease))) return rc;
+        char* scratch = lease.p;
         MergeScratch ms;
         ms.counters = reinterpret_cast<unsigned int*>(scratch);
         ms.partial = reinterpret_cast<double*>(scratch + kCounterBytes);
         ms.gpartial = reinterpret_cast<double*>(scratch + kCounterBytes + bytes_partial);
         ms.ngroups = ngroups;
-        if (smem > 48 * 1024)
-            CUDA_TRY(cudaFuncSetAttribute(unit_hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        unit_hist_kernel<<<grid, kBlock, smem, st>>>(E_true, w0, channel, n, bin_edges, n_bins, n_sub, ms, hist_centre_out);
+        if (two_slots) {
+            if (smem > 48 * 1024)
+                CUDA_TRY(cudaFuncSetAttribute(unit_hist_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            unit_hist_kernel<2><<<grid, kBlock, smem, st>>>(E_true, w0, channel, n, bin_edges, n_bins, n_sub, ms, hist_centre_out);
+        } else {
+            CUDA_TRY(cudaFuncSetAttribute(unit_hist_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            unit_hist_kernel<1><<<grid, kBlock, smem, st>>>(E_true, w0, channel, n, bin_edges, n_bins, 1, ms, hist_centre_out);
+        }
         if ((rc = post_launch("osc_bin_centre_compare (unit histogram)"))) return rc;
     }
     centre_weight_kernel<<<(nh + 255) / 256, 256, 0, st>>>(args, bin_edges, n_bins, hist_centre_out);
@@ -1179,10 +1221,13 @@ int osc_prob_host(const double* E_true_host, size_t n, int flavour_in, int flavo
                   double* P_out_host)
 {
     if (n > 0 && (!E_true_host || !P_out_host)) return fail(OSC_ERR_INVALID_ARG, "null host array with n > 0");
+    HostPath* hp = nullptr;
+    int rc = host_path(&hp);
+    if (rc) return rc;
+    HostPath& g_host = *hp;
     std::lock_guard<std::mutex> lk(g_host.mu);
     const size_t bytes = round_up(n * sizeof(double), 256);
-    int rc = g_host.ensure(2 * bytes + 256);
-    if (rc) return rc;
+    if ((rc = g_host.ensure(2 * bytes + 256))) return rc;
     double* dE = reinterpret_cast<double*>(g_host.buf);
     double* dP = reinterpret_cast<double*>(g_host.buf + bytes);
     if (n) CUDA_TRY(cudaMemcpyAsync(dE, E_true_host, n * sizeof(double), cudaMemcpyHostToDevice, g_host.stream));
@@ -1204,14 +1249,17 @@ int osc_reweight_bin_scales_host(const double* E_true_host, const double* E_reco
         return fail(OSC_ERR_INVALID_ARG, "null energy_scales, bin_edges or hist_out");
     if (n > 0 && (!E_true_host || !E_reco_host || !w0_host || !channel_host))
         return fail(OSC_ERR_INVALID_ARG, "null host array with n > 0");
+    HostPath* hp = nullptr;
+    int rc = host_path(&hp);
+    if (rc) return rc;
+    HostPath& g_host = *hp;
     std::lock_guard<std::mutex> lk(g_host.mu);
     const size_t nh = (size_t)kChannels * n_bins;
     const size_t b8 = round_up(n * sizeof(double), 256);
     const size_t b1 = round_up(n, 256);
     const size_t be = round_up((size_t)(n_bins + 1) * sizeof(double), 256);
     const size_t bh = round_up((size_t)n_scales * nh * sizeof(double), 256);
-    int rc = g_host.ensure(3 * b8 + b1 + be + bh + 256);
-    if (rc) return rc;
+    if ((rc = g_host.ensure(3 * b8 + b1 + be + bh + 256))) return rc;
     char* p = g_host.buf;
     double* dEt = reinterpret_cast<double*>(p);
     double* dEr = reinterpret_cast<double*>(p + b8);
@@ -1240,6 +1288,34 @@ int osc_reweight_bin_host(const double* E_true_host, const double* E_reco_host, 
 {
     return osc_reweight_bin_scales_host(E_true_host, E_reco_host, w0_host, channel_host, n, &energy_scale, 1,
                                         bin_edges_host, n_bins, hist_out_host);
+}
+
+int osc_set_batch_path(const char* path)
+{
+    if (!path) return fail(OSC_ERR_INVALID_ARG, "null path");
+    int v = -1;
+    if (!std::strcmp(path, "auto")) v = 0;
+    if (!std::strcmp(path, "k2")) v = 2;
+    if (!std::strcmp(path, "k4")) v = 4;
+    if (!std::strcmp(path, "k5")) v = 5;
+    if (v < 0) return fail(OSC_ERR_INVALID_ARG, "osc_set_batch_path: \"%s\" is not auto, k2, k4 or k5", path);
+    g_batch_path.store(v);
+    return OSC_OK;
+}
+
+int osc_set_k2_tuning(int threads, int slots, int n_sub, int blocks_per_sm)
+{
+    if (threads != 0 && threads != 768 && threads != 512 && threads != 384 && threads != 256 && threads != 128)
+        return fail(OSC_ERR_INVALID_ARG, "osc_set_k2_tuning: k2 is built for 128, 256, 384, 512 and 768 threads, not %d", threads);
+    if (slots < 0 || slots > 2) return fail(OSC_ERR_INVALID_ARG, "osc_set_k2_tuning: slots = %d is not 0, 1 or 2", slots);
+    if (n_sub != 0 && n_sub != 1 && n_sub != 2 && n_sub != 4)
+        return fail(OSC_ERR_INVALID_ARG, "osc_set_k2_tuning: n_sub = %d is not 0, 1, 2 or 4", n_sub);
+    if (blocks_per_sm < 0 || blocks_per_sm > 16) return fail(OSC_ERR_INVALID_ARG, "osc_set_k2_tuning: blocks_per_sm = %d", blocks_per_sm);
+    g_tune_threads.store(threads);
+    g_tune_slots.store(slots);
+    g_tune_nsub.store(n_sub);
+    g_tune_bps.store(blocks_per_sm);
+    return OSC_OK;
 }
 
 const char* osc_last_error(void) { return t_err; }

@@ -155,6 +155,17 @@ __device__ __forceinline__ void warp_hist_add2(const LaneHist& lh, int cell0, do
     warp_hist_commit(p, w0, w1);
 }
 
+// The same for the one-sub-histogram-per-warp layout (lane_hist_single).
+__device__ __forceinline__ void warp_hist_add2_single(const LaneHist& lh, int cell0, double w0, int cell1, double w1,
+                                                      unsigned lt_mask)
+{
+    HistPlan p;
+    warp_hist_match(p, lh, cell0, cell1);
+    int rmax1;
+    warp_hist_rank_single(p, lt_mask, rmax1);
+    warp_hist_commit_single(p, rmax1, w0, w1);
+}
+
 // Scratch of one call: counters[ngroups + 1] | partial[grid][nh] | gpartial[ngroups][nh].  It lives in a
 // buffer the library keeps per (device, stream); calls on one stream are ordered, so they can share it.
 // The counters are zero when a kernel starts and the blocks that consume them set them back to zero.

@@ -481,6 +481,8 @@ reweight_bin_scales_kernel(const __grid_constant__ BinArgs a, const __grid_const
 // unit_hist_kernel fills hist[channel][bin] += w0 over true-energy bins (the machinery of k2 without the closed
 // form); centre_weight_kernel multiplies each cell by P_channel(centre of the bin).
 // ------------------------------------------------------------------------------------------------
+// SLOTS = 2: a sub-histogram per (warp, event of the lane) as in k2; SLOTS = 1: one per warp (binnings above ~420 bins).
+template <int SLOTS>
 __global__ void __launch_bounds__(kBlock)
 unit_hist_kernel(const double* __restrict__ E_true, const double* __restrict__ w0, const int8_t* __restrict__ channel,
                  size_t n, const double* __restrict__ edges, int nb, int n_sub, MergeScratch ms,
@@ -493,11 +495,11 @@ unit_hist_kernel(const double* __restrict__ E_true, const double* __restrict__ w
     __shared__ unsigned int s_ticket;
     const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const unsigned lt_mask = (1u << lane) - 1u;
-    const int n_hist = WARPS * kSlots * n_sub;
+    const int n_hist = WARPS * SLOTS * n_sub;
     for (int i = threadIdx.x; i < n_hist * nh; i += kBlock) hist[i] = 0.0;
     build_bin_table(smem_raw, edges, nb);
     const BinView bt = bin_view(smem_raw);
-    const LaneHist lh = lane_hist(hist, nh, n_sub, warp, lane);
+    const LaneHist lh = SLOTS == 2 ? lane_hist(hist, nh, n_sub, warp, lane) : lane_hist_single(hist, nh, warp);
     const size_t ntiles = (n + 2 * kBlock - 1) / (2 * kBlock);
     for (size_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
         const size_t j0 = t * (2 * kBlock) + threadIdx.x, j1 = j0 + kBlock;
@@ -518,7 +520,8 @@ unit_hist_kernel(const double* __restrict__ E_true, const double* __restrict__ w
                 }
             }
         }
-        warp_hist_add2(lh, cell[0], w[0], cell[1], w[1], lt_mask);
+        if (SLOTS == 2) warp_hist_add2(lh, cell[0], w[0], cell[1], w[1], lt_mask);
+        else warp_hist_add2_single(lh, cell[0], w[0], cell[1], w[1], lt_mask);
     }
     block_merge(hist, n_hist, nh, ms, hist_out, &s_ticket);
 }

@@ -154,3 +154,44 @@ def test_missing_library_fails_loudly(monkeypatch, tmp_path):
     monkeypatch.setattr(binding, "_lib", None)
     with pytest.raises(binding.OscError):
         binding.lib()
+
+
+def test_binding_checks_sizes_before_handing_out_pointers():
+    """Caller-supplied outputs and secondary inputs are size-checked in the binding: a short array must raise, not
+    become an out-of-bounds write behind a raw pointer."""
+    import numpy as np
+    import torch
+
+    e = torch.zeros(8, dtype=torch.float64)
+    with pytest.raises(ValueError):
+        binding.osc_prob(e, 1, 1, 0, P_out=torch.zeros(7, dtype=torch.float64))
+    with pytest.raises(ValueError):
+        binding.osc_prob_all(e, 0, P_out=torch.zeros(8 * 9 - 1, dtype=torch.float64))
+    with pytest.raises(ValueError):
+        binding.osc_bin_index(e, e, torch.zeros(8, dtype=torch.int8), 1.0, torch.zeros(3, dtype=torch.float64),
+                              bin_out=torch.zeros(7, dtype=torch.int32))
+    with pytest.raises(ValueError):
+        binding.osc_reweight_bin(e, e, e, torch.zeros(8, dtype=torch.int8), 1.0, torch.zeros(1, dtype=torch.float64))
+    h = np.zeros(8)
+    ch = np.zeros(8, dtype=np.int8)
+    edges = np.array([0.0, 1.0, 2.0])
+    with pytest.raises(ValueError):
+        binding.osc_prob_host(h, 1, 1, 0, P_out=np.zeros(7))
+    with pytest.raises(ValueError):
+        binding.osc_reweight_bin_host(h, h[:7], h, ch, 1.0, edges)
+    with pytest.raises(ValueError):
+        binding.osc_reweight_bin_host(h, h, h, ch, 1.0, edges, hist_out=np.zeros(7))
+    with pytest.raises(ValueError):
+        binding.osc_reweight_bin_scales_host(h, h, h, ch[:5], (1.0, 1.1), edges)
+    with pytest.raises(ValueError):
+        binding.osc_reweight_bin_scales_host(h, h, h, ch, (1.0, 1.1), edges, hist_out=np.zeros(8))
+
+
+def test_setters_validate():
+    L = binding.lib()
+    assert L.osc_set_batch_path(b"k7") == INVALID and b"k7" in L.osc_last_error()
+    assert L.osc_set_batch_path(b"k5") == OK and L.osc_set_batch_path(b"auto") == OK
+    assert L.osc_set_k2_tuning(700, 0, 0, 0) == INVALID
+    assert L.osc_set_k2_tuning(0, 3, 0, 0) == INVALID
+    assert L.osc_set_k2_tuning(0, 0, 3, 0) == INVALID
+    assert L.osc_set_k2_tuning(512, 1, 0, 0) == OK and L.osc_set_k2_tuning(0, 0, 0, 0) == OK

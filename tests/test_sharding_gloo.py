@@ -94,7 +94,7 @@ def _scan_worker(rank: int, world: int, port: int, n: int, out_dir: str):
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
-        pts = wl.scan_points()[:80]                  # 2.5 groups of 32: the ranks own 64 and 16 points
+        pts = wl.scan_points()[:80]                  # 32 dm2_32 groups of 2 or 3 points each, strided through the list
         et, er, w0, ch = wl.events(n, seed=3)
         edges = wl.bin_edges()
 
@@ -123,4 +123,34 @@ def test_world2_scan_sharded_by_points(tmp_path):
     h1 = np.load(tmp_path / "scan_1.npy")
     assert h0.shape == (80, 4, 50)
     assert np.array_equal(h0, h1) and np.array_equal(h0, ref)    # no arithmetic across ranks: bit-identical
-    assert sharding.shard_bounds(80, 0, 2, align=32) == (0, 64) and sharding.shard_bounds(80, 1, 2, align=32) == (64, 80)
+
+
+@pytest.mark.parametrize("world", [1, 2, 3, 4, 8])
+def test_scan_partition_keeps_groups_whole(world):
+    """configs[3] (p = 32 i_th23 + j_dm2: the 32 points of a dm2_32 group are strided by 32): every rank gets whole
+    groups -- at least 32 points of each group it touches -- the ranks partition the list, and the loads are balanced."""
+    pts = wl.scan_points()
+    owned = sharding.scan_partition(pts, world)
+    assert sorted(i for o in owned for i in o) == list(range(1024))
+    for o in owned:
+        per_group = {}
+        for i in o:
+            per_group.setdefault(pts[i]["dm2_32"], 0)
+            per_group[pts[i]["dm2_32"]] += 1
+        assert all(c == 32 for c in per_group.values()), per_group
+        assert o == sorted(o)
+    sizes = [len(o) for o in owned]
+    assert max(sizes) - min(sizes) <= 32
+    assert owned == sharding.scan_partition(pts, world)          # deterministic
+
+
+def test_scan_partition_few_groups_and_loose_points():
+    one_group = [wl.table1(sin2_th23=0.3 + 0.001 * k, delta_cp=0.01 * k) for k in range(200)]
+    owned = sharding.scan_partition(one_group, 4)                 # one group, four ranks: cut at multiples of 32
+    assert sorted(i for o in owned for i in o) == list(range(200))
+    assert all(len(o) > 0 for o in owned)
+    assert sum(1 for o in owned if len(o) % 32 != 0) <= 1         # only the remainder piece is ragged
+    loose = [wl.table1(dm2_32=2.0e-3 + 1e-5 * k) for k in range(10)]   # ten unrelated points
+    owned = sharding.scan_partition(loose, 4)
+    assert sorted(len(o) for o in owned) == [2, 2, 3, 3]
+    assert sharding.scan_partition([], 2) == [[], []]

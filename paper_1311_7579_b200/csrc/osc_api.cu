@@ -153,6 +153,9 @@ struct Scratch {
 // ordered, so consecutive calls can share the buffer; it is allocated, zeroed and (when it has to grow)
 // freed in stream order.
 constexpr size_t kCounterBytes = 4096;
+constexpr size_t kTableCacheBytes = 12 * 1024;          // >= bin_table_bytes(kMaxBins): image of the last bin table (osc_bins.cuh)
+constexpr size_t kScratchHead = kCounterBytes + kTableCacheBytes;   // zeroed at allocation; the per-call areas follow
+static_assert(bin_table_bytes(768) <= kTableCacheBytes, "bin-table cache too small for the largest binning");
 struct StreamScratch {
     char* buf = nullptr;
     size_t cap = 0;
@@ -189,7 +192,7 @@ int stream_scratch(size_t bytes, cudaStream_t st, ScratchLease& lease)
         const size_t cap = round_up(bytes + bytes / 2, 1 << 16);
         char* p = nullptr;
         CUDA_TRY(cudaMallocAsync((void**)&p, cap, st));
-        cudaError_t e = cudaMemsetAsync(p, 0, kCounterBytes, st);
+        cudaError_t e = cudaMemsetAsync(p, 0, kScratchHead, st);
         if (e != cudaSuccess) {
             cudaFreeAsync(p, st);
             return fail(OSC_ERR_CUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e));
@@ -201,17 +204,47 @@ int stream_scratch(size_t bytes, cudaStream_t st, ScratchLease& lease)
     return OSC_OK;
 }
 
+// The per-call areas of a stream scratch: ticket counter and bin-table cache in the zeroed head, block partials behind.
+struct CallScratch {
+    MergeScratch ms;
+    unsigned char* table_cache;
+};
+
+CallScratch call_scratch(char* scratch)
+{
+    CallScratch c;
+    c.ms.counters = reinterpret_cast<unsigned int*>(scratch);
+    c.ms.partial = reinterpret_cast<double*>(scratch + kScratchHead);
+    c.table_cache = reinterpret_cast<unsigned char*>(scratch + kCounterBytes);
+    return c;
+}
+
 template <bool VEC, int THREADS, int SLOTS = kSlots>
 int launch_k2(int grid, size_t smem, cudaStream_t st, const BinArgs& args, const double* E_true, const double* E_reco,
               const double* w0, const int8_t* channel, size_t n, double energy_scale, const double* bin_edges,
-              int n_bins, int n_sub, const MergeScratch& ms, double* hist_out)
+              int n_bins, int n_sub, const CallScratch& cs, double* hist_out)
 {
-    if (smem > 48 * 1024)
+    // the attribute is set once per instantiation and size (the call costs a microsecond of host time otherwise)
+    static std::atomic<size_t> configured{0};
+    if (smem > 48 * 1024 && configured.load(std::memory_order_relaxed) < smem) {
         CUDA_TRY(cudaFuncSetAttribute(reweight_bin_kernel<VEC, THREADS, SLOTS>,
                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    reweight_bin_kernel<VEC, THREADS, SLOTS><<<grid, THREADS, smem, st>>>(args, E_true, E_reco, w0, channel, n,
-                                                                         energy_scale, bin_edges, n_bins, n_sub, ms,
-                                                                         hist_out);
+        configured.store(smem, std::memory_order_relaxed);
+    }
+    // programmatic dependent launch: the set-up of this launch may overlap the tail of the kernel before it on the
+    // stream; the kernel waits (griddepcontrol.wait) before it touches global memory (osc_kernels.cuh, pdl_wait)
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    CUDA_TRY(cudaLaunchKernelEx(&cfg, reweight_bin_kernel<VEC, THREADS, SLOTS>, args, E_true, E_reco, w0, channel, n,
+                                energy_scale, bin_edges, n_bins, n_sub, cs.ms, cs.table_cache, hist_out));
     return post_launch("osc_reweight_bin");
 }
 
@@ -280,19 +313,9 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     if (ntiles < g) g = ntiles;
     const int grid = (int)g;
 
-    const int ngroups = (grid + kGroup - 1) / kGroup;
-    if ((size_t)(ngroups + 1) * sizeof(unsigned int) > kCounterBytes)
-        return fail(OSC_ERR_CUDA, "merge ticket area too small for %d groups", ngroups);
-    const size_t bytes_partial = (size_t)grid * nh * sizeof(double);
-    const size_t bytes_gpartial = (size_t)ngroups * nh * sizeof(double);
     ScratchLease lease;
-    if ((rc = stream_scratch(kCounterBytes + bytes_partial + bytes_gpartial, st, lease))) return rc;
-    char* scratch = lease.p;
-    MergeScratch ms;
-    ms.counters = reinterpret_cast<unsigned int*>(scratch);
-    ms.partial = reinterpret_cast<double*>(scratch + kCounterBytes);
-    ms.gpartial = reinterpret_cast<double*>(scratch + kCounterBytes + bytes_partial);
-    ms.ngroups = ngroups;
+    if ((rc = stream_scratch(kScratchHead + (size_t)grid * nh * sizeof(double), st, lease))) return rc;
+    const CallScratch ms = call_scratch(lease.p);
 
     const bool vec = aligned(E_true, 16) && aligned(E_reco, 16) && aligned(w0, 16) && aligned(channel, 2);
 #define OSC_K2_SINGLE(T)                                                                                               \
@@ -328,12 +351,26 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
 template <bool VEC, int NS>
 int launch_k2s(int grid, size_t smem, cudaStream_t st, const BinArgs& args, const ScaleArgs& sc, const double* E_true,
                const double* E_reco, const double* w0, const int8_t* channel, size_t n, const double* bin_edges,
-               int n_bins, int n_sub, const MergeScratch& ms, double* hist_out)
+               int n_bins, int n_sub, const CallScratch& cs, double* hist_out)
 {
-    CUDA_TRY(cudaFuncSetAttribute(reweight_bin_scales_kernel<VEC, 256, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)smem));
-    reweight_bin_scales_kernel<VEC, 256, NS><<<grid, 256, smem, st>>>(args, sc, E_true, E_reco, w0, channel, n, bin_edges,
-                                                                      n_bins, n_sub, ms, hist_out);
+    static std::atomic<size_t> configured{0};
+    if (configured.load(std::memory_order_relaxed) < smem) {
+        CUDA_TRY(cudaFuncSetAttribute(reweight_bin_scales_kernel<VEC, 256, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)smem));
+        configured.store(smem, std::memory_order_relaxed);
+    }
+    cudaLaunchConfig_t cfg = {};                      // programmatic dependent launch, as launch_k2
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(256);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    CUDA_TRY(cudaLaunchKernelEx(&cfg, reweight_bin_scales_kernel<VEC, 256, NS>, args, sc, E_true, E_reco, w0, channel, n,
+                                bin_edges, n_bins, n_sub, cs.ms, cs.table_cache, hist_out));
     return post_launch("osc_reweight_bin_scales");
 }
 
@@ -357,24 +394,16 @@ int launch_reweight_scales(const BinArgs& args, const double* E_true, const doub
     size_t g = (size_t)sms * 2;
     if (ntiles < g) g = ntiles;
     const int grid = (int)g;
-    const int ngroups = (grid + kGroup - 1) / kGroup;
-    const size_t bytes_partial = (size_t)grid * nht * sizeof(double);
-    const size_t bytes_gpartial = (size_t)ngroups * nht * sizeof(double);
     ScratchLease lease;
-    if ((rc = stream_scratch(kCounterBytes + bytes_partial + bytes_gpartial, st, lease))) return rc;
-    char* scratch = lease.p;
-    MergeScratch ms;
-    ms.counters = reinterpret_cast<unsigned int*>(scratch);
-    ms.partial = reinterpret_cast<double*>(scratch + kCounterBytes);
-    ms.gpartial = reinterpret_cast<double*>(scratch + kCounterBytes + bytes_partial);
-    ms.ngroups = ngroups;
+    if ((rc = stream_scratch(kScratchHead + (size_t)grid * nht * sizeof(double), st, lease))) return rc;
+    const CallScratch ms = call_scratch(lease.p);
     ScaleArgs sc;
     for (int k = 0; k < kMaxScales; ++k) sc.s[k] = k < n_scales ? scales[k] : 1.0;
     const bool vec = aligned(E_true, 16) && aligned(E_reco, 16) && aligned(w0, 16) && aligned(channel, 2);
 #define OSC_K2S(NS)                                                                                                  \
-    return vec ? launch_k2s<true, NS>(grid, smem, st, args, sc, E_true, E_reco, w0, channel, n, bin_edges, n_bins,    \
+    return vec ? launch_k2s<true, NS>(grid, smem, st, args, sc, E_true, E_reco, w0, channel, n, bin_edges, n_bins, \
                                       n_sub, ms, hist_out)                                                           \
-               : launch_k2s<false, NS>(grid, smem, st, args, sc, E_true, E_reco, w0, channel, n, bin_edges, n_bins,   \
+               : launch_k2s<false, NS>(grid, smem, st, args, sc, E_true, E_reco, w0, channel, n, bin_edges, n_bins, \
                                        n_sub, ms, hist_out)
     switch (n_scales) {
     case 2: OSC_K2S(2);
@@ -1116,9 +1145,8 @@ int osc_plan_reweight_bin(const osc_plan* plan, double* hist_out, void* stream)
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const SortedEvents& se = pl->se;
     ScratchLease lease;
-    if ((rc = stream_scratch(kCounterBytes + (size_t)se.geo.max_units * sizeof(double), st, lease))) return rc;
-    char* scratch = lease.p;
-    double* partial = reinterpret_cast<double*>(scratch + kCounterBytes);
+    if ((rc = stream_scratch(kScratchHead + (size_t)se.geo.max_units * sizeof(double), st, lease))) return rc;
+    double* partial = reinterpret_cast<double*>(lease.p + kScratchHead);
     const ChannelKinds kinds = channel_kinds();
     scan_full_one_kernel<<<(se.geo.max_units + kScanWarps - 1) / kScanWarps, 32 * kScanWarps, 0, st>>>(
         args, kinds, se.sEt, se.sW, se.cell_begin, se.unit_begin, se.unit_cell, se.geo, se.n_bins, partial);
@@ -1164,16 +1192,9 @@ int osc_bin_centre_compare(const double* E_true, const double* w0, const int8_t*
         size_t g = (size_t)sms * (smem <= 100 * 1024 ? 2 : 1);
         if (ntiles < g) g = ntiles;
         const int grid = (int)g;
-        const int ngroups = (grid + kGroup - 1) / kGroup;
-        const size_t bytes_partial = (size_t)grid * nh * sizeof(double), bytes_gpartial = (size_t)ngroups * nh * sizeof(double);
         ScratchLease lease;
-        if ((rc = stream_scratch(kCounterBytes + bytes_partial + bytes_gpartial, st, lease))) return rc;
-        char* scratch = lease.p;
-        MergeScratch ms;
-        ms.counters = reinterpret_cast<unsigned int*>(scratch);
-        ms.partial = reinterpret_cast<double*>(scratch + kCounterBytes);
-        ms.gpartial = reinterpret_cast<double*>(scratch + kCounterBytes + bytes_partial);
-        ms.ngroups = ngroups;
+        if ((rc = stream_scratch(kScratchHead + (size_t)grid * nh * sizeof(double), st, lease))) return rc;
+        const MergeScratch ms = call_scratch(lease.p).ms;
         if (two_slots) {
             if (smem > 48 * 1024)
                 CUDA_TRY(cudaFuncSetAttribute(unit_hist_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

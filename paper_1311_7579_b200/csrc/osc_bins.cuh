@@ -38,12 +38,12 @@ struct BinHead {
 };
 
 // Byte layout of the table in shared memory (all parts 16-byte aligned).
-__host__ __device__ inline size_t bin_keys_offset() { return sizeof(BinHead); }
-__host__ __device__ inline size_t bin_lut_offset(int nb)
+__host__ __device__ constexpr size_t bin_keys_offset() { return sizeof(BinHead); }
+__host__ __device__ constexpr size_t bin_lut_offset(int nb)
 {
     return (sizeof(BinHead) + sizeof(unsigned long long) * (size_t)(nb + 1 + kKeySentinels) + 15) / 16 * 16;
 }
-__host__ __device__ inline size_t bin_table_bytes(int nb)
+__host__ __device__ constexpr size_t bin_table_bytes(int nb)
 {
     return bin_lut_offset(nb) + sizeof(unsigned short) * (size_t)kLutCells;
 }
@@ -186,6 +186,41 @@ __device__ __forceinline__ void build_bin_table(unsigned char* smem_table, const
     steps = __reduce_max_sync(0xffffffffu, steps);
     if ((threadIdx.x & 31) == 0) atomicMax(&head->steps, steps);
     __syncthreads();
+}
+
+// The table of a call in shared memory, taken from a cache in global memory when that cache was built from the same
+// edges.  `cache` is an image of a table (bin_table_bytes(nb) bytes, 16-byte aligned; all zero when nothing has been
+// cached yet) that the library keeps per (device, stream): calls on a stream are ordered, the last block of a kernel
+// that had to build the table writes it back (store_bin_table), and a fitter that rebuilds its PDF a million times with
+// the same binning pays one L2 read and one comparison of the edge keys per block instead of the build.  The cache is
+// validated against the caller's edges in every block -- same number of bins and bit-identical keys of all edges, which
+// determine the rest of the table -- so a stale image is never used.  `fresh` is shared-memory scratch for nb + 1 keys
+// (the caller's still unused histogram area).  Called by all threads of the block; ends with a barrier; returns
+// (block-uniform) whether the cache was valid.
+__device__ __forceinline__ bool load_or_build_bin_table(unsigned char* smem_table, long long* fresh,
+                                                        const unsigned char* __restrict__ cache,
+                                                        const double* __restrict__ edges, int nb)
+{
+    for (int i = threadIdx.x; i <= nb; i += blockDim.x) fresh[i] = edge_key(__ldg(edges + i));
+    const int bytes = (int)bin_table_bytes(nb);
+    for (int o = (int)threadIdx.x * 16; o < bytes; o += (int)blockDim.x * 16)
+        *reinterpret_cast<int4*>(smem_table + o) = __ldcg(reinterpret_cast<const int4*>(cache + o));
+    __syncthreads();
+    const BinHead* h = reinterpret_cast<const BinHead*>(smem_table);
+    const long long* key = reinterpret_cast<const long long*>(smem_table + bin_keys_offset());
+    int ok = h->nb == (unsigned int)nb;
+    if (ok)
+        for (int i = threadIdx.x; i <= nb; i += blockDim.x) ok &= key[i] == fresh[i];
+    ok = __syncthreads_and(ok);
+    if (!ok) build_bin_table(smem_table, edges, nb);
+    return ok != 0;
+}
+
+__device__ __forceinline__ void store_bin_table(const unsigned char* smem_table, unsigned char* __restrict__ cache, int nb)
+{
+    const int bytes = (int)bin_table_bytes(nb);
+    for (int o = (int)threadIdx.x * 16; o < bytes; o += (int)blockDim.x * 16)
+        *reinterpret_cast<int4*>(cache + o) = *reinterpret_cast<const int4*>(smem_table + o);
 }
 
 } // namespace oscb

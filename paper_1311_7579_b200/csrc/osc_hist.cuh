@@ -166,71 +166,132 @@ __device__ __forceinline__ void warp_hist_add2_single(const LaneHist& lh, int ce
     warp_hist_commit_single(p, rmax1, w0, w1);
 }
 
-// Scratch of one call: counters[ngroups + 1] | partial[grid][nh] | gpartial[ngroups][nh].  It lives in a
-// buffer the library keeps per (device, stream); calls on one stream are ordered, so they can share it.
-// The counters are zero when a kernel starts and the blocks that consume them set them back to zero.
+// Scratch of one call: counters[1] | partial[grid][nh].  It lives in a buffer the library keeps per (device, stream);
+// calls on one stream are ordered, so they can share it.  The ticket counter is zero when a kernel starts and the block
+// that consumes it sets it back to zero.
 struct MergeScratch {
     double* partial;
-    double* gpartial;
     unsigned int* counters;
-    int ngroups;
 };
 
-constexpr int kGroup = 16; // blocks per first-level merge group
-
-// src[0] + src[stride] + ... (count terms, added in that order), read through L2.  The loads of eight terms are
-// issued together before they are added: the merge is a chain of dependent L2 round trips otherwise, and it sits
-// on the critical path of every call (the last block does it alone).
+// src[0] + src[stride] + ... (count terms, added in that order), read through L2.  The loads of sixteen terms are
+// issued together before they are added: the merge is a chain of dependent L2 round trips otherwise, and it sits on
+// the critical path of every call (the last block does it alone).
 __device__ __forceinline__ double ordered_sum_cg(const double* src, int count, int stride)
 {
     double s = 0.0;
     int b = 0;
-    for (; b + 8 <= count; b += 8) {
+    for (; b + 16 <= count; b += 16) {
+        double v[16];
+#pragma unroll
+        for (int k = 0; k < 16; ++k) v[k] = __ldcg(src + (size_t)(b + k) * stride);
+#pragma unroll
+        for (int k = 0; k < 16; ++k) s += v[k];
+    }
+    if (b + 8 <= count) {
         double v[8];
 #pragma unroll
         for (int k = 0; k < 8; ++k) v[k] = __ldcg(src + (size_t)(b + k) * stride);
 #pragma unroll
         for (int k = 0; k < 8; ++k) s += v[k];
+        b += 8;
     }
     for (; b < count; ++b) s += __ldcg(src + (size_t)b * stride);
     return s;
 }
 
-// hist: [n_sub][nh] sub-histograms of this block in shared memory (n_sub = warps * kSlots).
-// Writes the block's sum to ms.partial, then the last block of each group sums the group and the last
-// group sums the groups into out[nh].  Must be called by all threads of the block.
-__device__ __forceinline__ void block_merge(const double* hist, int n_sub, int nh, const MergeScratch& ms,
+// The same for two adjacent cells at once (src 16-byte aligned, stride2 in units of double2), twelve terms per batch:
+// with up to kMergeSegs threads per pair of cells the 148 block partials of a call arrive in two round trips.
+constexpr int kMergeBatch = 12;
+__device__ __forceinline__ double2 ordered_sum2_cg(const double2* src, int count, int stride2)
+{
+    double2 s = make_double2(0.0, 0.0);
+    for (int b = 0; b < count; b += kMergeBatch) {
+        double2 v[kMergeBatch];
+#pragma unroll
+        for (int k = 0; k < kMergeBatch; ++k)
+            v[k] = b + k < count ? __ldcg(src + (size_t)(b + k) * stride2) : make_double2(0.0, 0.0);
+#pragma unroll
+        for (int k = 0; k < kMergeBatch; ++k) {
+            if (b + k < count) {           // (a padding term would turn a -0.0 sum into +0.0; sums here are >= 0 anyway)
+                s.x += v[k].x;
+                s.y += v[k].y;
+            }
+        }
+    }
+    return s;
+}
+
+constexpr int kMergeSegs = 8; // at most this many threads share the partials of one pair of cells in the final merge
+
+// hist: [n_sub][nh] sub-histograms of this block in shared memory (n_sub >= kMergeSegs, nh even, hist 16-byte aligned;
+// the memory is reused as scratch by the last block).  Every block writes its sum to ms.partial; the block that arrives
+// last (ticket) adds the partials of all blocks in block order into out[nh].  One level: the critical path after the
+// slowest block is one fence, one atomic and the loads of the partials, which up to kMergeSegs threads per pair of cells
+// issue all at once.  Every sum has a fixed order (given the launch shape), so the result is a deterministic function
+// of the inputs.  Ordering: the barrier orders the block's stores before thread 0's release-acquire atomic, which is
+// cumulative (the pattern of a grid-wide barrier).  Must be called by all threads of the block; returns true in the last block (all
+// threads), false elsewhere.
+__device__ __forceinline__ bool block_merge(double* hist, int n_sub, int nh, const MergeScratch& ms,
                                             double* __restrict__ out, unsigned int* s_ticket)
 {
     __syncthreads();
     double* my_partial = ms.partial + (size_t)blockIdx.x * nh;
     for (int i = threadIdx.x; i < nh; i += blockDim.x) {
-        double s = hist[i];
-        for (int w = 1; w < n_sub; ++w) s += hist[(size_t)w * nh + i];
-        my_partial[i] = s;
+        // four interleaved chains, combined at the end: a quarter of the dependent additions of a single chain
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+        int w = 0;
+        for (; w + 4 <= n_sub; w += 4) {
+            s0 += hist[(size_t)w * nh + i];
+            s1 += hist[(size_t)(w + 1) * nh + i];
+            s2 += hist[(size_t)(w + 2) * nh + i];
+            s3 += hist[(size_t)(w + 3) * nh + i];
+        }
+        for (; w < n_sub; ++w) s0 += hist[(size_t)w * nh + i];
+        __stcg(my_partial + i, (s0 + s1) + (s2 + s3));
     }
-    __threadfence();
     __syncthreads();
+    if (threadIdx.x == 0) {
+        // release: the block's partial (ordered before this by the barrier) is visible to whoever sees the ticket;
+        // acquire: the last block's loads below see every other block's partial
+        unsigned ticket;
+        asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(ticket) : "l"(ms.counters) : "memory");
+        if (ticket == gridDim.x - 1u) ms.counters[0] = 0u;  // last block: nobody else reads it again
+        *s_ticket = ticket;
+    }
+    __syncthreads();
+    if (*s_ticket != gridDim.x - 1u) return false;
 
-    const int group = blockIdx.x / kGroup;
-    const int gfirst = group * kGroup;
-    const int gsize = min(kGroup, (int)gridDim.x - gfirst);
-    if (threadIdx.x == 0) *s_ticket = atomicAdd(ms.counters + group, 1u);
+    const int grid = (int)gridDim.x;
+    const int npair = nh / 2;
+    int nseg = (int)blockDim.x / npair;
+    nseg = nseg < 1 ? 1 : (nseg > kMergeSegs ? kMergeSegs : nseg);
+    const double2* part2 = reinterpret_cast<const double2*>(ms.partial);
+    double2* out2 = reinterpret_cast<double2*>(out);
+    if (nseg == 1 || (reinterpret_cast<size_t>(out) & 15)) {
+        for (int i = threadIdx.x; i < nh; i += blockDim.x) out[i] = ordered_sum_cg(ms.partial + i, grid, nh);
+        return true;
+    }
+    // a pair of cells is shared by nseg threads, each adds a contiguous range of blocks; the ranges are then added in order
+    const int per = (grid + nseg - 1) / nseg;
+    const int t = (int)threadIdx.x;
+    double2* seg_sum = reinterpret_cast<double2*>(hist);
+    if (t < nseg * npair) {
+        const int seg = t / npair, i = t - seg * npair;
+        const int b0 = seg * per, b1 = min(grid, b0 + per);
+        seg_sum[t] = b1 > b0 ? ordered_sum2_cg(part2 + (size_t)b0 * npair + i, b1 - b0, npair) : make_double2(0.0, 0.0);
+    }
     __syncthreads();
-    if (*s_ticket != (unsigned)(gsize - 1)) return;
-    if (threadIdx.x == 0) ms.counters[group] = 0u;          // last of the group: nobody else reads it again
-    __threadfence();
-    for (int i = threadIdx.x; i < nh; i += blockDim.x)
-        ms.gpartial[(size_t)group * nh + i] = ordered_sum_cg(ms.partial + (size_t)gfirst * nh + i, gsize, nh);
-    __threadfence();
-    __syncthreads();
-
-    if (threadIdx.x == 0) *s_ticket = atomicAdd(ms.counters + ms.ngroups, 1u);
-    __syncthreads();
-    if (*s_ticket != (unsigned)(ms.ngroups - 1)) return;
-    if (threadIdx.x == 0) ms.counters[ms.ngroups] = 0u;
-    __threadfence();
-    for (int i = threadIdx.x; i < nh; i += blockDim.x) out[i] = ordered_sum_cg(ms.gpartial + i, ms.ngroups, nh);
+    if (t < npair) {
+        double2 s = seg_sum[t];
+        for (int k = 1; k < nseg; ++k) {
+            const double2 v = seg_sum[k * npair + t];
+            s.x += v.x;
+            s.y += v.y;
+        }
+        out2[t] = s;
+    }
+    return true;
 }
 
 } // namespace oscb

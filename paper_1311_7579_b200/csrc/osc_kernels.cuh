@@ -44,6 +44,31 @@ __device__ __forceinline__ double ld_stream_pinned(const double* p)
 
 __device__ __forceinline__ double qnan() { return __longlong_as_double(0x7FF8000000000000LL); }
 
+// Lanes of the warp below this one (%lanemask_lt): one special-register read where the compiler would otherwise
+// rebuild (1 << lane) - 1 from the thread index in every iteration.
+__device__ __forceinline__ unsigned lanemask_lt()
+{
+    unsigned m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+
+// Programmatic dependent launch (PTX griddepcontrol): the fused kernels are launched with the programmatic-stream-
+// serialization attribute, so a launch may be set up -- blocks scheduled, shared memory initialised -- while the kernel
+// before it on the stream is still draining; pdl_wait() returns once that kernel has completed and its memory is
+// visible, and nothing before it may touch global memory.  Without the attribute, or after a kernel that never
+// triggers, both are no-ops and the launch is ordered as usual.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// p[0 .. count) = 0.0 with 16-byte stores (p 16-byte aligned); called by all threads of the block.
+__device__ __forceinline__ void zero_shared(double* p, int count)
+{
+    double2* q = reinterpret_cast<double2*>(p);
+    for (int i = threadIdx.x; i < count / 2; i += blockDim.x) q[i] = make_double2(0.0, 0.0);
+    if (threadIdx.x == 0 && (count & 1)) p[count - 1] = 0.0;
+}
+
 // ------------------------------------------------------------------------------------------------
 // k1: P_out[j] = P(alpha -> beta)(E_true[j]).  VEC: pointers 16-byte aligned -> 128-bit accesses.
 // KIND: which element of S is asked for (assemble_kind): the launch knows it, so the assembly is specialised.
@@ -340,7 +365,7 @@ reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict_
                     const double* __restrict__ E_reco, const double* __restrict__ w0,
                     const int8_t* __restrict__ channel, size_t n, double energy_scale,
                     const double* __restrict__ edges, int nb, int n_sub, MergeScratch ms,
-                    double* __restrict__ hist_out)
+                    unsigned char* __restrict__ table_cache, double* __restrict__ hist_out)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int WARPS = THREADS / 32;
@@ -349,19 +374,29 @@ reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict_
     unsigned char* tab = smem_raw + sizeof(double) * kBinArgsDoubles;
     double* hist = reinterpret_cast<double*>(tab + bin_table_bytes(nb));
     __shared__ unsigned int s_ticket;
+    __shared__ int s_cached;
 
     const unsigned lane = threadIdx.x & 31u;
     const unsigned warp = threadIdx.x >> 5;
     const int n_hist = WARPS * SLOTS * n_sub;
 
-    // tiles are counted in 32 bits (the host rejects n >= 2^32 tiles); pinned so that the loop does not recompute it
+    // tiles are counted in 32 bits (the host rejects n >= 2^32 tiles).  Measured: handing ntiles over as a kernel
+    // parameter removes the eleven uniform instructions with which the compiler re-derives it from n in every iteration
+    // of the event loop -- and makes the loop 6 % SLOWER (1200 instead of 1132 us per 1e8 events: a different schedule
+    // with more MIO-queue and short-scoreboard stalls), so it stays computed here
     const unsigned ntiles = pin_u32((unsigned)((n + 2 * THREADS - 1) / (2 * THREADS)));
+    // before pdl_wait(): only kernel parameters and shared memory (the previous kernel on the stream may still run)
+    pdl_launch_dependents();
+    if (threadIdx.x < kBinArgsDoubles) pbuf[threadIdx.x] = reinterpret_cast<const double*>(&a)[threadIdx.x];
+    const int keep = (nb + 2) & ~1;                           // the first nb + 1 words stage the edge keys below
+    zero_shared(hist + keep, n_hist * nh - keep);
+    pdl_wait();
     const unsigned t = blockIdx.x;
     EventPair cur = load_pair<VEC, THREADS>(E_true, E_reco, w0, channel, n, t);   // grid <= ntiles
-
-    if (threadIdx.x < kBinArgsDoubles) pbuf[threadIdx.x] = reinterpret_cast<const double*>(&a)[threadIdx.x];
-    for (int i = threadIdx.x; i < n_hist * nh; i += THREADS) hist[i] = 0.0;
-    build_bin_table(tab, edges, nb);
+    const bool cached = load_or_build_bin_table(tab, reinterpret_cast<long long*>(hist), table_cache, edges, nb);
+    if (threadIdx.x == 0) s_cached = cached;
+    for (int i = threadIdx.x; i < keep; i += THREADS) hist[i] = 0.0;
+    __syncthreads();
     BinView bt = bin_view(tab);
     bt.ekey = pin_u32(bt.ekey);
     bt.lut = pin_u32(bt.lut);
@@ -369,13 +404,14 @@ reweight_bin_kernel(const __grid_constant__ BinArgs a, const double* __restrict_
     LaneHist lh = SLOTS == 2 ? lane_hist(hist, nh, n_sub, warp, lane) : lane_hist_single(hist, nh, warp);
     lh.h0 = pin_u32(lh.h0);
     lh.h1 = SLOTS == 2 ? pin_u32(lh.h1) : lh.h0;
-    const unsigned lt_mask = pin_u32((1u << lane) - 1u);
+    const unsigned lt_mask = lanemask_lt();
 
     if (bt.steps <= 1u)
         k2_loop<VEC, THREADS, 1, SLOTS>(a, E_true, E_reco, w0, channel, n, energy_scale, bt, pb, lh, lt_mask, ntiles, t, cur);
     else
         k2_loop<VEC, THREADS, 0, SLOTS>(a, E_true, E_reco, w0, channel, n, energy_scale, bt, pb, lh, lt_mask, ntiles, t, cur);
-    block_merge(hist, n_hist, nh, ms, hist_out, &s_ticket);
+    const bool last = block_merge(hist, n_hist, nh, ms, hist_out, &s_ticket);
+    if (last && !s_cached) store_bin_table(tab, table_cache, nb);      // every other block is past its read of the cache
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -439,7 +475,7 @@ reweight_bin_scales_kernel(const __grid_constant__ BinArgs a, const __grid_const
                            const double* __restrict__ E_true, const double* __restrict__ E_reco,
                            const double* __restrict__ w0, const int8_t* __restrict__ channel, size_t n,
                            const double* __restrict__ edges, int nb, int n_sub, MergeScratch ms,
-                           double* __restrict__ hist_out)
+                           unsigned char* __restrict__ table_cache, double* __restrict__ hist_out)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int WARPS = THREADS / 32;
@@ -448,17 +484,24 @@ reweight_bin_scales_kernel(const __grid_constant__ BinArgs a, const __grid_const
     unsigned char* tab = smem_raw + sizeof(double) * kBinArgsDoubles;
     double* hist = reinterpret_cast<double*>(tab + bin_table_bytes(nb));
     __shared__ unsigned int s_ticket;
+    __shared__ int s_cached;
 
     const unsigned lane = threadIdx.x & 31u;
     const unsigned warp = threadIdx.x >> 5;
     const int n_hist = WARPS * kSlots * n_sub;
     const unsigned ntiles = pin_u32((unsigned)((n + 2 * THREADS - 1) / (2 * THREADS)));
+    // before pdl_wait(): only kernel parameters and shared memory (the previous kernel on the stream may still run)
+    pdl_launch_dependents();
+    if (threadIdx.x < kBinArgsDoubles) pbuf[threadIdx.x] = reinterpret_cast<const double*>(&a)[threadIdx.x];
+    const int keep = (nb + 2) & ~1;                           // the first nb + 1 words stage the edge keys below
+    zero_shared(hist + keep, n_hist * nht - keep);
+    pdl_wait();
     const unsigned t = blockIdx.x;
     EventPair cur = load_pair<VEC, THREADS>(E_true, E_reco, w0, channel, n, t);   // grid <= ntiles
-
-    if (threadIdx.x < kBinArgsDoubles) pbuf[threadIdx.x] = reinterpret_cast<const double*>(&a)[threadIdx.x];
-    for (int i = threadIdx.x; i < n_hist * nht; i += THREADS) hist[i] = 0.0;
-    build_bin_table(tab, edges, nb);
+    const bool cached = load_or_build_bin_table(tab, reinterpret_cast<long long*>(hist), table_cache, edges, nb);
+    if (threadIdx.x == 0) s_cached = cached;
+    for (int i = threadIdx.x; i < keep; i += THREADS) hist[i] = 0.0;
+    __syncthreads();
     BinView bt = bin_view(tab);
     bt.ekey = pin_u32(bt.ekey);
     bt.lut = pin_u32(bt.lut);
@@ -466,13 +509,14 @@ reweight_bin_scales_kernel(const __grid_constant__ BinArgs a, const __grid_const
     LaneHist lh = lane_hist(hist, nht, n_sub, warp, lane);
     lh.h0 = pin_u32(lh.h0);
     lh.h1 = pin_u32(lh.h1);
-    const unsigned lt_mask = pin_u32((1u << lane) - 1u);
+    const unsigned lt_mask = lanemask_lt();
 
     if (bt.steps <= 1u)
         k2s_loop<VEC, THREADS, NS, 1>(a, E_true, E_reco, w0, channel, n, sc, bt, pb, lh, lt_mask, ntiles, t, cur);
     else
         k2s_loop<VEC, THREADS, NS, 0>(a, E_true, E_reco, w0, channel, n, sc, bt, pb, lh, lt_mask, ntiles, t, cur);
-    block_merge(hist, n_hist, nht, ms, hist_out, &s_ticket);
+    const bool last = block_merge(hist, n_hist, nht, ms, hist_out, &s_ticket);
+    if (last && !s_cached) store_bin_table(tab, table_cache, nb);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -524,9 +524,26 @@ int osc_prob_all(const double* E_true, size_t n, int antinu, double* P_out, void
     a.set = h.set;
     for (int beta = 0; beta < 2; ++beta)
         for (int alpha = 0; alpha < 2; ++alpha) a.tr[2 * beta + alpha] = make_trans(h, alpha, beta, antinu);
+    // launch shape as osc_prob: one block of kBlockProbAll threads per SM once every SM gets two full iterations of it,
+    // blocks of kBlock threads below that; 128-bit accesses when E_true and every row of P_out are 16-byte aligned
+    const size_t npairs = (n + 1) / 2;
+    int sms = 0;
+    if ((rc = sm_count(&sms))) return rc;
+    constexpr int kT = kBlockProbAll;
+    const bool big = npairs >= (size_t)2 * sms * kT;
     int grid = 1;
-    if ((rc = grid_for((n + 2 * kBlock - 1) / (2 * kBlock), &grid))) return rc;
-    prob_all_kernel<<<grid, kBlock, 0, static_cast<cudaStream_t>(stream)>>>(a, E_true, n, P_out);
+    if ((rc = big ? grid_for((npairs + kT - 1) / kT, &grid, 1)
+                  : grid_for((npairs + kBlock - 1) / kBlock, &grid)))
+        return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const bool vec = aligned(E_true, 16) && aligned(P_out, 16) && n % 2 == 0;
+    if (big) {
+        if (vec) prob_all_kernel<true, kT><<<grid, kT, 0, st>>>(a, E_true, n, P_out);
+        else prob_all_kernel<false, kT><<<grid, kT, 0, st>>>(a, E_true, n, P_out);
+    } else {
+        if (vec) prob_all_kernel<true, kBlock><<<grid, kBlock, 0, st>>>(a, E_true, n, P_out);
+        else prob_all_kernel<false, kBlock><<<grid, kBlock, 0, st>>>(a, E_true, n, P_out);
+    }
     return post_launch("osc_prob_all");
 }
 

@@ -20,6 +20,9 @@
 namespace oscb {
 
 constexpr int kBlock = 256;          // threads per block of k1b and the small kernels (8 warps)
+constexpr int kBlockProbAll = 640;   // k1b above ~4e5 events: one block of 20 warps per SM, 96 registers per thread (us per call of
+                                     // 1e7 events: 384 threads 230, 512 150.7, 640 148.8, 768 154.4, 896 156.5, 1024 160.0;
+                                     // two blocks of 512: 158.1, four of 256: 163.4)
 constexpr int kBlockProb = 768;      // k1 above ~5e5 events: ONE block of 24 warps per SM (as k2; 88.7 us against 95.0 us
                                      // per 1e7 events for four blocks of 256, whose warps finish at different times)
 
@@ -123,8 +126,21 @@ prob_kernel(const __grid_constant__ ProbArgs a, const double* __restrict__ E_tru
 // the remaining five probabilities are the unitarity complements.  Row 3*beta + alpha of P_out.
 // ------------------------------------------------------------------------------------------------
 // max(x, 0) that lets NaN through (fmax would turn it into 0): the complements below are differences of numbers near
-// 1 and may come out as -1e-17.
-__device__ __forceinline__ double clamp0_keep_nan(double x) { return x < 0.0 ? 0.0 : x; }
+// 1 and may come out as -1e-17.  On the integer pipe: a negative number that is not NaN has its upper word in
+// [0x80000000, 0xFFF00000) (the complements are never -inf), and is replaced by +0.0 with two selects.
+__device__ __forceinline__ double clamp0_keep_nan(double x)
+{
+    const unsigned hi = (unsigned)__double2hiint(x);
+    const bool neg = hi - 0x80000000u < 0x7FF00000u;
+    return __hiloint2double(neg ? 0 : (int)hi, neg ? 0 : __double2loint(x));
+}
+
+__device__ __forceinline__ double2 ld_stream2_pinned(const double* p)
+{
+    double2 v;
+    asm volatile("ld.global.cs.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p) : "memory");
+    return v;
+}
 
 // A11: an unusable energy is replaced by NaN, which then propagates through the closed form into all nine outputs
 // (two selects instead of nine).
@@ -155,49 +171,59 @@ __device__ __forceinline__ void prob_nine(const ProbAllArgs& a, double E, double
     P[8] = p22;
 }
 
-__global__ void __launch_bounds__(kBlock)
+// VEC (E_true and every row of P_out 16-byte aligned, i.e. n even): slot i holds the adjacent events (2i, 2i + 1), one
+// 128-bit load and nine 128-bit streaming stores per slot; otherwise tile i / THREADS holds events j0 and j0 + THREADS
+// with scalar accesses.  The energies of the thread's next slot are loaded (pinned, see ld_stream_pinned) before the
+// arithmetic of the current one.  THREADS = kBlockProbAll: one block per SM, as k1 and k2 (the warps of co-resident blocks
+// finish at different times); 256: four blocks per SM for sizes that would leave SMs idle otherwise.
+template <bool VEC, int THREADS>
+__global__ void __launch_bounds__(THREADS, THREADS >= 512 ? 1 : 4)
 prob_all_kernel(const __grid_constant__ ProbAllArgs a, const double* __restrict__ E_true, size_t n,
                 double* __restrict__ P_out)
 {
-    // the energies are loaded two tiles ahead (ncu: 3.3 long-scoreboard stalls per issue without look-ahead, 1.9 with;
-    // ptxas still sinks the loads to the bottom of the body, so the rest of that stall is the store queue: with the
-    // stores removed the kernel takes 135 us per 1e7 events, with them 167 us)
-    const size_t ntiles = (n + 2 * kBlock - 1) / (2 * kBlock);
-    auto load = [&](size_t tile, double& E0, double& E1) {
-        E0 = 1.0;
-        E1 = 1.0;
-        if (tile < ntiles) {
-            const size_t j0 = tile * (2 * kBlock) + threadIdx.x, j1 = j0 + kBlock;
-            if (j0 < n) E0 = ld_stream_pinned(E_true + j0);
-            if (j1 < n) E1 = ld_stream_pinned(E_true + j1);
+    const size_t nslots = VEC ? (n + 1) / 2 : ((n + 2 * THREADS - 1) / (2 * THREADS)) * THREADS;
+    const size_t stride = (size_t)gridDim.x * THREADS;
+    auto load = [&](size_t i, double& E0, double& E1) {
+        const size_t j0 = VEC ? 2 * i : (i / THREADS) * (2 * THREADS) + (i % THREADS);
+        const size_t j1 = VEC ? j0 + 1 : j0 + THREADS;
+        if (VEC) {                                           // n is even: both events of a slot exist
+            const double2 v = ld_stream2_pinned(E_true + j0);
+            E0 = v.x;
+            E1 = v.y;
+        } else {
+            E0 = (j0 < n) ? ld_stream_pinned(E_true + j0) : 1.0;
+            E1 = (j1 < n) ? ld_stream_pinned(E_true + j1) : 1.0;
         }
     };
-    size_t t = blockIdx.x;
-    double N0, N1, M0, M1;
-    load(t, N0, N1);
-    load(t + gridDim.x, M0, M1);
-    while (t < ntiles) {
-        const size_t j0 = t * (2 * kBlock) + threadIdx.x;
-        const size_t j1 = j0 + kBlock;
-        const bool in0 = j0 < n, in1 = j1 < n;
+    size_t i = (size_t)blockIdx.x * THREADS + threadIdx.x;
+    double N0 = 1.0, N1 = 1.0;
+    if (i < nslots) load(i, N0, N1);
+    while (i < nslots) {
+        const size_t j0 = VEC ? 2 * i : (i / THREADS) * (2 * THREADS) + (i % THREADS);
+        const size_t j1 = VEC ? j0 + 1 : j0 + THREADS;
         const double E0 = N0, E1 = N1;
-        N0 = M0;
-        N1 = M1;
-        load(t + 2 * (size_t)gridDim.x, M0, M1);
-        t += gridDim.x;
+        i += stride;
+        if (i < nslots) load(i, N0, N1);
         double P0[9], P1[9];
         prob_nine(a, E0, P0);
         prob_nine(a, E1, P1);
-        // one running pointer per event, advanced by the row stride: nine row bases would not fit the uniform
-        // registers next to the constants of the closed form (ptxas spilled them and refilled them every iteration)
-        double* q0 = P_out + j0;
-        double* q1 = P_out + j1;
+        // one running pointer, advanced by the row stride: nine row bases would not fit the uniform registers next to
+        // the constants of the closed form
+        double* q = P_out + j0;
+        if (VEC) {
 #pragma unroll
-        for (int k = 0; k < 9; ++k) {
-            if (in0) st_stream(q0, P0[k]);
-            if (in1) st_stream(q1, P1[k]);
-            q0 += n;
-            q1 += n;
+            for (int k = 0; k < 9; ++k) {
+                st_stream2(q, P0[k], P1[k]);
+                q += n;
+            }
+        } else {
+            const bool in0 = j0 < n, in1 = j1 < n;
+#pragma unroll
+            for (int k = 0; k < 9; ++k) {
+                if (in0) st_stream(q, P0[k]);
+                if (in1) st_stream(q + THREADS, P1[k]);
+                q += n;
+            }
         }
     }
 }

@@ -133,7 +133,7 @@ int osc_reweight_bin_scales(const double *E_true, const double *E_reco, const do
  *     at least 8 points per such group on average (a scan grid: "only theta23 and dm2_32
  *     float"), the events are sorted by histogram cell once and the eigen-solve is done once per (event,
  *     group); a point then costs 4 to 6 fused multiply-adds per event (kernel k4, csrc/osc_scan.cuh);
- *   - otherwise every (event, point) pair gets the full closed form: from 4 points on (10 for more than
+ *   - otherwise every (event, point) pair gets the full closed form: from 4 points on (6 for more than
  *     2e6 events), on the events sorted by histogram cell, with the weights of a cell summed in registers
  *     (kernel k5); below that the sort does not pay and every point gets its own pass of
  *     osc_reweight_bin's kernel (k2).  Binnings up to the library's limit of 768 bins are taken by all paths.

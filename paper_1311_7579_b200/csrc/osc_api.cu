@@ -36,6 +36,10 @@ std::atomic<unsigned long long> g_launches{0};
 // the environment: a stray variable must not change launch shapes in a fitter that calls the library 1e6 times.
 std::atomic<int> g_batch_path{0};                       // 0 auto, 2 k2, 4 k4, 5 k5
 std::atomic<int> g_tune_threads{0}, g_tune_slots{0}, g_tune_nsub{0}, g_tune_bps{0};
+#ifndef OSC_SORT_CHUNK
+#define OSC_SORT_CHUNK 2048
+#endif
+std::atomic<size_t> g_sort_chunk{OSC_SORT_CHUNK};                 // events per block-local sort chunk (multiple of 512)
 
 int fail(int code, const char* fmt, ...)
 {
@@ -795,6 +799,18 @@ int sorted_geometry(size_t n, int n_bins, size_t piece, ScanGeom& geo)
     // long enough to keep the [ncells][nranges] count table below 64 MB
     const size_t max_ranges = std::min<size_t>(16384, (64u << 20) / (sizeof(unsigned int) * (size_t)geo.ncells));
     geo.range = round_up(std::max<size_t>(256, (n + max_ranges - 1) / max_ranges), 32);
+    if (geo.ncells <= kSortMaxCells) {
+        // block-local sort (sort_count_kernel / sort_scatter_kernel): a block sorts a chunk of `range` events in shared
+        // memory; chunks short enough to give every SM a few blocks, long enough for runs of whole sectors per cell
+        int sms = 0;
+        int rc = sm_count(&sms);
+        if (rc) return rc;
+        // chunk = 512 * STEPS events with STEPS in {2, 4, 8} (sort_scatter_kernel<STEPS>)
+        size_t chunk = g_sort_chunk.load();
+        while (chunk > 1024 && n / chunk < (size_t)sms * 4) chunk /= 2;
+        while (chunk < 4096 && (n + chunk - 1) / chunk > max_ranges) chunk *= 2;
+        geo.range = chunk;
+    }
     geo.nranges = (unsigned)((n + geo.range - 1) / geo.range);
     geo.piece = (unsigned)piece;
     geo.max_units = (unsigned)(n / piece + (size_t)geo.ncells + 1);
@@ -828,6 +844,29 @@ int scan_sort(const SortedEvents& se, const double* E_true, const double* E_reco
     unsigned int* count = reinterpret_cast<unsigned int*>(tmp.p + b_cellid);
     int sms = 0;
     if ((rc = sm_count(&sms))) return rc;
+    if (geo.ncells <= kSortMaxCells) {
+        // block-local sort: cell ids and per-(cell, chunk) counts, offsets, then the scatter through shared memory
+        const size_t smem_c = bin_table_bytes(se.n_bins) + sizeof(unsigned int) * (size_t)geo.ncells;
+        const size_t smem_s = round_up(((size_t)(kSortWarps + 2) * geo.ncells + 1) * sizeof(unsigned int), 16) +
+                              geo.range * (sizeof(double2) + sizeof(unsigned short));
+        if (smem_s + 1024 > (size_t)227 * 1024) return fail(OSC_ERR_INVALID_ARG, "internal: sort chunk of %zu events does not fit shared memory", geo.range);
+        const unsigned per_sm = (unsigned)std::max<size_t>(1, std::min<size_t>(4, kSmemBudget / (smem_s + 1024)));
+        const int steps = (int)(geo.range / (32 * kSortWarps));
+        auto scatter = steps == 2 ? sort_scatter_kernel<2> : steps == 4 ? sort_scatter_kernel<4> : sort_scatter_kernel<8>;
+        if (steps != 2 && steps != 4 && steps != 8)
+            return fail(OSC_ERR_INVALID_ARG, "internal: sort chunk of %zu events is not 1024, 2048 or 4096", geo.range);
+        if (smem_s > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_s));
+        sort_count_kernel<<<std::min<unsigned>(geo.nranges, (unsigned)sms * 4u), kSortThreads, smem_c, st>>>(
+            E_true, E_reco, channel, se.n, energy_scale, bin_edges, se.n_bins, geo, cellid, count);
+        if ((rc = post_launch("sort of the events: count"))) return rc;
+        scan_offsets_cell_kernel<<<geo.ncells, 1024, 0, st>>>(count, geo, se.cell_begin);
+        if ((rc = post_launch("sort of the events: offsets per cell"))) return rc;
+        scan_offsets_kernel<<<1, 1024, 0, st>>>(geo, se.cell_begin, se.unit_begin, se.unit_cell);
+        if ((rc = post_launch("sort of the events: offsets"))) return rc;
+        scatter<<<std::min<unsigned>(geo.nranges, (unsigned)sms * per_sm), kSortThreads, smem_s, st>>>(
+            E_true, w0, cellid, se.n, geo, count, se.cell_begin, se.sEt, se.sW);
+        return post_launch("sort of the events: scatter");
+    }
     // blocks per SM of the two event-ordered passes (measured at 1e7 events): the count pass is latency-bound and wants
     // all the warps an SM holds, the scatter pass is bound by its write pattern and gets slower with more of them
     const unsigned range_blocks = (geo.nranges + kScanWarps - 1) / kScanWarps;
@@ -1031,11 +1070,11 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
         precompute(points[p], h);
         make_bin_args(h, blocks[(size_t)p]);
     }
-    // Point lists without scan structure.  The sort of the events costs about 45 ps per event and then a point costs
-    // 9 ps per event in k5 against 14 ps (plus 20 us per launch) for a pass of the fused single-set kernel k2: measured
-    // on a B200, k5 is ahead from 4 points on at 1e6 events and from 10 points on at 1e7.  Below that every point gets
-    // its own k2 pass.
-    bool use_full = n_points >= (n <= 2000000 ? 4 : 10);
+    // Point lists without scan structure.  The sort of the events costs about 20 ps per event (44 us at 1e6 events, 201 us at
+    // 1e7) and then a point costs 9 ps per event in k5 against 12.4 ps (23 us per 1e6 events) for a pass of the fused
+    // single-set kernel k2: k5 is ahead from 4 points on at 1e6 events and from 6 points on at 1e7.  Below that every
+    // point gets its own k2 pass.
+    bool use_full = n_points >= (n <= 2000000 ? 4 : 6);
     if (forced == 5) use_full = true;
     if (forced == 2) use_full = false;
     if (use_full)

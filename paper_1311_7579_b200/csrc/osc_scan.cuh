@@ -181,6 +181,7 @@ scan_offsets_kernel(ScanGeom geo, unsigned int* __restrict__ cell_begin, unsigne
                     unsigned short* __restrict__ unit_cell)
 {
     __shared__ unsigned s_warp[33];
+    __shared__ unsigned s_ub[4 * 768 + 1];
     const int cper = (geo.ncells + 1023) / 1024;
     const int c0 = min(geo.ncells, (int)threadIdx.x * cper), c1 = min(geo.ncells, c0 + cper);
     unsigned len[3] = {0u, 0u, 0u};
@@ -197,13 +198,20 @@ scan_offsets_kernel(ScanGeom geo, unsigned int* __restrict__ cell_begin, unsigne
         cell_begin[c] = run;
         unit_begin[c] = urun;
         run += len[c - c0];
-        const unsigned np_c = (len[c - c0] + geo.piece - 1) / geo.piece;
-        for (unsigned k = 0; k < np_c; ++k) unit_cell[urun + k] = (unsigned short)c;     // cell of every piece
-        urun += np_c;
+        urun += (len[c - c0] + geo.piece - 1) / geo.piece;
     }
     if (threadIdx.x == 0) {
         cell_begin[geo.ncells] = total;
         unit_begin[geo.ncells] = utotal;
+    }
+    // cell of every piece: a warp per cell, lanes over its pieces (a populated cell has thousands of pieces; one thread
+    // per cell took 24 us at 1e7 events)
+    __syncthreads();
+    for (int c = threadIdx.x; c <= geo.ncells; c += 1024) s_ub[c] = unit_begin[c];
+    __syncthreads();
+    for (int c = threadIdx.x >> 5; c < geo.ncells; c += 32) {
+        const unsigned u0 = s_ub[c], u1 = s_ub[c + 1];
+        for (unsigned u = u0 + (threadIdx.x & 31u); u < u1; u += 32) unit_cell[u] = (unsigned short)c;
     }
 }
 
@@ -239,6 +247,171 @@ scan_scatter_kernel(const double* __restrict__ E_true, const double* __restrict_
             }
             __syncwarp();
         }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Block-local sort (binnings of up to kSortMaxCells cells): the same stable sort by cell, with a block-wide chunk
+// of geo.range events as the unit instead of a warp range.  The per-warp-range scatter above writes 8-byte words to
+// ~200 destinations per warp (one sector per lane: 277 us per 1e7 events); here a block first sorts its chunk by cell
+// in shared memory and then writes it out in sorted order, so that the events of a (chunk, cell) pair -- 4096 events
+// over 200 cells: ~20 on average, hundreds in the populated cells -- leave as runs of whole sectors.
+// The order inside a cell is chunk-major and, inside a chunk, the order of the caller's arrays: the sorted arrays are
+// the ones the per-warp-range sort produces.
+// ------------------------------------------------------------------------------------------------
+constexpr int kSortThreads = 512;
+constexpr int kSortWarps = kSortThreads / 32;
+constexpr int kSortMaxCells = 1024;
+
+// Pass 1: cell of every event, and count[cell][chunk].  Shared memory: bin table | cnt[ncells] (u32).
+__global__ void __launch_bounds__(kSortThreads)
+sort_count_kernel(const double* __restrict__ E_true, const double* __restrict__ E_reco,
+                  const int8_t* __restrict__ channel, size_t n, double energy_scale,
+                  const double* __restrict__ edges, int nb, ScanGeom geo, unsigned short* __restrict__ cellid,
+                  unsigned int* __restrict__ count)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    unsigned int* cnt = reinterpret_cast<unsigned int*>(smem_raw + bin_table_bytes(nb));
+    for (int c = threadIdx.x; c < geo.ncells; c += kSortThreads) cnt[c] = 0u;
+    build_bin_table(smem_raw, edges, nb);                        // ends with a barrier
+    const BinView bt = bin_view(smem_raw);
+    for (unsigned r = blockIdx.x; r < geo.nranges; r += gridDim.x) {
+        const size_t begin = (size_t)r * geo.range, end = min(n, begin + geo.range);
+        for (size_t j = begin + threadIdx.x; j < end; j += kSortThreads) {
+            const double x = scaled_energy(energy_scale, E_reco[j]);
+            const int bin = find_bin<0>(bt, x);
+            const unsigned ch = (unsigned)(unsigned char)channel[j];
+            unsigned cell = kNoCell;
+            if (energy_ok(E_true[j]) && ch < (unsigned)kChannels && bin >= 0) cell = ch * (unsigned)nb + (unsigned)bin;
+            cellid[j] = (unsigned short)cell;
+            if (cell != kNoCell) atomicAdd(cnt + cell, 1u);      // integer counts: the order does not matter
+        }
+        __syncthreads();
+        for (int c = threadIdx.x; c < geo.ncells; c += kSortThreads) {
+            count[(size_t)c * geo.nranges + r] = cnt[c];
+            cnt[c] = 0u;
+        }
+        __syncthreads();
+    }
+}
+
+// Pass 3: stable scatter of (E_true, w0) through a chunk sorted in shared memory.  A chunk is 32 * kSortWarps * STEPS
+// events; a warp owns STEPS consecutive groups of 32 events and keeps their cells, match masks and payload in
+// registers between the counting and the placing phase, so every global load of the chunk is issued up front.
+// Shared memory: wcnt[kSortWarps][ncells] | cbase[ncells + 1] | gbase[ncells] (u32) | buf[range] (double2) | bcell[range] (u16)
+template <int STEPS>
+__global__ void __launch_bounds__(kSortThreads)
+sort_scatter_kernel(const double* __restrict__ E_true, const double* __restrict__ w0,
+                    const unsigned short* __restrict__ cellid, size_t n, ScanGeom geo,
+                    const unsigned int* __restrict__ offsets, const unsigned int* __restrict__ cell_begin,
+                    double* __restrict__ sEt, double* __restrict__ sW)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ unsigned s_warp[33];
+    const int nc = geo.ncells;
+    unsigned int* wcnt_all = reinterpret_cast<unsigned int*>(smem_raw);
+    unsigned int* cbase = wcnt_all + (size_t)kSortWarps * nc;
+    unsigned int* gbase = cbase + nc + 1;
+    double2* buf = reinterpret_cast<double2*>(smem_raw + (((size_t)(kSortWarps + 2) * nc + 1) * 4 + 15) / 16 * 16);
+    unsigned short* bcell = reinterpret_cast<unsigned short*>(buf + geo.range);
+    const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    unsigned int* wcnt = wcnt_all + (size_t)warp * nc;
+    constexpr unsigned per = 32u * STEPS;                        // events per warp; geo.range = per * kSortWarps
+
+    for (unsigned r = blockIdx.x; r < geo.nranges; r += gridDim.x) {
+        const size_t begin = (size_t)r * geo.range, end = min(n, begin + geo.range);
+        const size_t wb = min(end, begin + (size_t)warp * per);
+        unsigned cell[STEPS], m[STEPS];
+        double ev[STEPS], wv[STEPS];
+#pragma unroll
+        for (int k = 0; k < STEPS; ++k) {
+            const size_t j = wb + 32u * k + lane;
+            const bool in = j < end;
+            cell[k] = in ? (unsigned)__ldg(cellid + j) : (unsigned)kNoCell;
+            ev[k] = in ? __ldcs(E_true + j) : 0.0;
+            wv[k] = in ? __ldcs(w0 + j) : 0.0;
+        }
+        // phase A: events per (warp, cell)
+        for (int c = lane; c < nc; c += 32) wcnt[c] = 0u;
+        __syncwarp();
+#pragma unroll
+        for (int k = 0; k < STEPS; ++k) {
+            m[k] = __match_any_sync(0xffffffffu, cell[k]);
+            if (cell[k] != kNoCell && lane == 31u - (unsigned)__clz((int)m[k])) wcnt[cell[k]] += (unsigned)__popc(m[k]);
+            __syncwarp();
+        }
+        __syncthreads();
+        // per cell: exclusive prefix over the warps (in place), total into cbase
+        for (int c = threadIdx.x; c < nc; c += kSortThreads) {
+            unsigned run = 0;
+#pragma unroll
+            for (int w = 0; w < kSortWarps; ++w) {
+                const unsigned v = wcnt_all[(size_t)w * nc + c];
+                wcnt_all[(size_t)w * nc + c] = run;
+                run += v;
+            }
+            cbase[c] = run;
+        }
+        __syncthreads();
+        // exclusive scan of the cell totals (each thread a contiguous run of cells)
+        {
+            const int cper = (nc + kSortThreads - 1) / kSortThreads;
+            const int c0 = min(nc, (int)threadIdx.x * cper), c1 = min(nc, c0 + cper);
+            unsigned sum = 0;
+            for (int c = c0; c < c1; ++c) sum += cbase[c];
+            unsigned inc = sum;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned o = __shfl_up_sync(0xffffffffu, inc, d);
+                if (lane >= (unsigned)d) inc += o;
+            }
+            if (lane == 31) s_warp[warp] = inc;
+            __syncthreads();
+            if (warp == 0) {
+                const unsigned w = lane < (unsigned)kSortWarps ? s_warp[lane] : 0u;
+                unsigned winc = w;
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const unsigned o = __shfl_up_sync(0xffffffffu, winc, d);
+                    if (lane >= (unsigned)d) winc += o;
+                }
+                s_warp[lane] = winc - w;
+                if (lane == 31) s_warp[32] = winc;
+            }
+            __syncthreads();
+            unsigned run = s_warp[warp] + inc - sum;
+            for (int c = c0; c < c1; ++c) {
+                const unsigned v = cbase[c];
+                cbase[c] = run;
+                gbase[c] = __ldg(cell_begin + c) + __ldg(offsets + (size_t)c * geo.nranges + r) - run;
+                run += v;
+            }
+            if (threadIdx.x == 0) cbase[nc] = s_warp[32];
+        }
+        __syncthreads();
+        // phase B: every event to its place in the sorted chunk
+#pragma unroll
+        for (int k = 0; k < STEPS; ++k) {
+            if (cell[k] != kNoCell) {
+                const unsigned pos = cbase[cell[k]] + wcnt[cell[k]] + (unsigned)__popc(m[k] & lt_mask);
+                buf[pos] = make_double2(ev[k], wv[k]);
+                bcell[pos] = (unsigned short)cell[k];
+            }
+            __syncwarp();
+            if (cell[k] != kNoCell && lane == 31u - (unsigned)__clz((int)m[k])) wcnt[cell[k]] += (unsigned)__popc(m[k]);
+            __syncwarp();
+        }
+        __syncthreads();
+        // phase C: the sorted chunk leaves in order; neighbours in the chunk are neighbours in the sorted arrays
+        const unsigned kept = cbase[nc];
+        for (unsigned p = threadIdx.x; p < kept; p += kSortThreads) {
+            const double2 v = buf[p];
+            const unsigned dst = gbase[bcell[p]] + p;
+            sEt[dst] = v.x;
+            sW[dst] = v.y;
+        }
+        __syncthreads();
     }
 }
 

@@ -243,6 +243,15 @@ int osc_get_device(int *device /* HOST, out */);
  * the measured fp64 peak that roofline fractions are quoted against. */
 int osc_fp64_peak_probe(int iters, int blocks_per_sm, double *flops_per_launch, void *stream);
 
+/* Measurement helper, not part of the hot path: one launch of a register-resident loop of ONE instruction pattern
+ * (8 independent chains per thread, blocks_per_sm blocks of 256 threads on every SM), so that ncu's
+ * smsp__inst_executed / sm__cycles_elapsed, or CUDA events and the SM clock, give the issue cost of the pattern in
+ * cycles per warp instruction and SM sub-partition (profiles/r2_dfma_issue.md).
+ *   kind 0: DFMA with three distinct register operands;  1: DFMA, two registers + immediate;  2: DFMA, one register;
+ *        3: DMUL;  4: DADD;  5: kind 0 + two three-register FFMA per DFMA;  6: kind 0 + two IMAD per DFMA
+ * *fp64_inst_per_launch (HOST, out, may be NULL) receives the fp64 thread instructions of the launch. */
+int osc_fp64_issue_probe(int kind, int iters, int blocks_per_sm, double *fp64_inst_per_launch, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -28,7 +28,7 @@ EXPORTS = ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "os
            "osc_plan_create", "osc_plan_reweight_bin", "osc_plan_reweight_bin_batch", "osc_plan_destroy",
            "osc_neg2lnl", "osc_bin_centre_compare", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_reweight_bin_scales_host", "osc_last_error", "osc_launch_count",
            "osc_version", "osc_set_device", "osc_get_device", "osc_fp64_peak_probe", "osc_set_batch_path",
-           "osc_set_k2_tuning")
+           "osc_set_k2_tuning", "osc_fp64_issue_probe")
 
 
 class OscError(RuntimeError):
@@ -74,6 +74,7 @@ def lib() -> ctypes.CDLL:
     L.osc_set_device.argtypes = [i]
     L.osc_get_device.argtypes = [ctypes.POINTER(i)]
     L.osc_fp64_peak_probe.argtypes = [i, i, ctypes.POINTER(d), vp]
+    L.osc_fp64_issue_probe.argtypes = [i, i, i, ctypes.POINTER(d), vp]
     L.osc_set_batch_path.argtypes = [ctypes.c_char_p]
     L.osc_set_k2_tuning.argtypes = [i, i, i, i]
     for name in ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_scales",
@@ -81,7 +82,7 @@ def lib() -> ctypes.CDLL:
                  "osc_plan_create", "osc_plan_reweight_bin", "osc_plan_reweight_bin_batch", "osc_plan_destroy",
                  "osc_neg2lnl", "osc_bin_centre_compare", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_reweight_bin_scales_host", "osc_set_device",
                  "osc_get_device",
-                 "osc_fp64_peak_probe", "osc_set_batch_path", "osc_set_k2_tuning"):
+                 "osc_fp64_peak_probe", "osc_set_batch_path", "osc_set_k2_tuning", "osc_fp64_issue_probe"):
         getattr(L, name).restype = i
     L.osc_last_error.restype = ctypes.c_char_p
     L.osc_version.restype = ctypes.c_char_p
@@ -428,6 +429,13 @@ def osc_fp64_peak_probe(iters: int, blocks_per_sm: int = 4, stream=None) -> floa
     flops = ctypes.c_double(0.0)
     _check(lib().osc_fp64_peak_probe(int(iters), int(blocks_per_sm), ctypes.byref(flops), _stream(stream)))
     return flops.value
+
+
+def osc_fp64_issue_probe(kind: int, iters: int, blocks_per_sm: int = 4, stream=None) -> float:
+    """Enqueue one launch of issue-probe `kind` (include/osc.h); returns its fp64 thread-instruction count."""
+    cnt = ctypes.c_double(0.0)
+    _check(lib().osc_fp64_issue_probe(int(kind), int(iters), int(blocks_per_sm), ctypes.byref(cnt), _stream(stream)))
+    return cnt.value
 
 
 def osc_reweight_bin_scales_host(E_true: np.ndarray, E_reco: np.ndarray, w0: np.ndarray, channel: np.ndarray,

@@ -1428,4 +1428,33 @@ int osc_fp64_peak_probe(int iters, int blocks_per_sm, double* flops_per_launch, 
     return post_launch("osc_fp64_peak_probe");
 }
 
+int osc_fp64_issue_probe(int kind, int iters, int blocks_per_sm, double* fp64_inst_per_launch, void* stream)
+{
+    if (kind < 0 || kind > 6 || iters < 1 || blocks_per_sm < 1 || blocks_per_sm > 8)
+        return fail(OSC_ERR_INVALID_ARG, "bad probe arguments");
+    int sms = 0;
+    int rc = sm_count(&sms);
+    if (rc) return rc;
+    static double* buf = nullptr;             // in[24] (harmless values near 1), out[1]
+    if (!buf) {
+        CUDA_TRY(cudaMalloc((void**)&buf, 32 * sizeof(double)));
+        double h[32];
+        for (int k = 0; k < 32; ++k) h[k] = k < 8 ? 1.0 + 0.01 * k : (k < 16 ? 0.999999 - 1e-7 * k : 1e-9 * (k - 15));
+        CUDA_TRY(cudaMemcpy(buf, h, sizeof h, cudaMemcpyHostToDevice));
+    }
+    const int grid = sms * blocks_per_sm;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    switch (kind) {
+    case 0: issue_probe_kernel<0><<<grid, kBlock, 0, st>>>(buf, buf + 24, iters); break;
+    case 1: issue_probe_kernel<1><<<grid, kBlock, 0, st>>>(buf, buf + 24, iters); break;
+    case 2: issue_probe_kernel<2><<<grid, kBlock, 0, st>>>(buf, buf + 24, iters); break;
+    case 3: issue_probe_kernel<3><<<grid, kBlock, 0, st>>>(buf, buf + 24, iters); break;
+    case 4: issue_probe_kernel<4><<<grid, kBlock, 0, st>>>(buf, buf + 24, iters); break;
+    case 5: issue_probe_kernel<5><<<grid, kBlock, 0, st>>>(buf, buf + 24, iters); break;
+    default: issue_probe_kernel<6><<<grid, kBlock, 0, st>>>(buf, buf + 24, iters); break;
+    }
+    if (fp64_inst_per_launch) *fp64_inst_per_launch = 8.0 * (double)iters * (double)kBlock * (double)grid;
+    return post_launch("osc_fp64_issue_probe");
+}
+
 } // extern "C"

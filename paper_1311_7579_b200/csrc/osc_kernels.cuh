@@ -625,4 +625,51 @@ __global__ void __launch_bounds__(kBlock) dfma_probe_kernel(double* out, int ite
     if (s == 123.456) out[0] = s; // keeps the loop alive, practically never stores
 }
 
+// Issue-rate probes behind DESIGN.md 5.1 ("what bounds these kernels"): register-resident loops of one instruction
+// pattern, 8 independent chains per thread, so that ncu's smsp__inst_executed / sm__cycles_elapsed of a launch gives the
+// issue cost of the pattern in cycles per warp instruction and sub-partition.  y, z come from memory (opaque to the
+// compiler) and stay in registers.  KIND: 0 DFMA x = fma(y, z, x), three distinct register operands;
+// 1 DFMA x = fma(x, y, c), two registers and an immediate; 2 DFMA x = fma(x, m, c), one register (dfma_probe_kernel's
+// pattern); 3 DMUL x = x * y; 4 DADD x = x + y; 5 pattern 0 followed by two FFMA with three register operands each;
+// 6 pattern 0 followed by two IMAD.  Not part of the hot path.
+template <int KIND>
+__global__ void __launch_bounds__(kBlock) issue_probe_kernel(const double* __restrict__ in, double* out, int iters)
+{
+    double x[8], y[8], z[8];
+    float f[8], g[8];
+    int q[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        // thread-dependent values: warp-uniform ones would be kept in uniform registers, which is the cheap operand kind
+        x[k] = in[k] + threadIdx.x;
+        y[k] = in[8 + k] - 1e-9 * threadIdx.x;
+        z[k] = in[16 + k] + 1e-12 * threadIdx.x;
+        f[k] = (float)in[k] + 1e-3f * threadIdx.x;
+        g[k] = (float)in[8 + k] - 1e-6f * threadIdx.x;
+        q[k] = (int)in[16 + k] + threadIdx.x;
+    }
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            if (KIND == 0 || KIND == 5 || KIND == 6) x[k] = fma(y[k], z[k], x[k]);
+            if (KIND == 1) x[k] = fma(x[k], y[k], 0.5);
+            if (KIND == 2) x[k] = fma(x[k], 0.999999, 1e-9);
+            if (KIND == 3) x[k] = x[k] * y[k];
+            if (KIND == 4) x[k] = x[k] + y[k];
+            if (KIND == 5) {
+                f[k] = fmaf(g[k], f[(k + 1) & 7], f[k]);
+                g[k] = fmaf(f[k], g[(k + 3) & 7], g[k]);
+            }
+            if (KIND == 6) {
+                q[k] = q[k] * q[(k + 1) & 7] + q[(k + 2) & 7];
+                q[(k + 3) & 7] = q[k] * q[(k + 5) & 7] + q[(k + 3) & 7];
+            }
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += x[k] + (double)f[k] + (double)g[k] + (double)q[k];
+    if (s == 123.456) out[0] = s; // keeps the loop alive, practically never stores
+}
+
 } // namespace oscb

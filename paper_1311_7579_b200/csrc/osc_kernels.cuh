@@ -23,6 +23,8 @@ constexpr int kBlock = 256;          // threads per block of k1b and the small k
 constexpr int kBlockProbAll = 640;   // k1b above ~4e5 events: one block of 20 warps per SM, 96 registers per thread (us per call of
                                      // 1e7 events: 384 threads 230, 512 150.7, 640 148.8, 768 154.4, 896 156.5, 1024 160.0;
                                      // two blocks of 512: 158.1, four of 256: 163.4)
+constexpr int kProbAllAhead = 3;     // slots k1b loads its energies ahead of the arithmetic (us per call of 1e7 events:
+                                     // 1 slot 148.8, 2 slots 143.7, 3 slots 138.8, 4 slots 148.9, 6 slots 146.7)
 constexpr int kBlockProb = 768;      // k1 above ~5e5 events: ONE block of 24 warps per SM (as k2; 88.7 us against 95.0 us
                                      // per 1e7 events for four blocks of 256, whose warps finish at different times)
 
@@ -173,8 +175,7 @@ __device__ __forceinline__ void prob_nine(const ProbAllArgs& a, double E, double
 
 // VEC (E_true and every row of P_out 16-byte aligned, i.e. n even): slot i holds the adjacent events (2i, 2i + 1), one
 // 128-bit load and nine 128-bit streaming stores per slot; otherwise tile i / THREADS holds events j0 and j0 + THREADS
-// with scalar accesses.  The energies of the thread's next slot are loaded (pinned, see ld_stream_pinned) before the
-// arithmetic of the current one.  THREADS = kBlockProbAll: one block per SM, as k1 and k2 (the warps of co-resident blocks
+// with scalar accesses.  The energies are loaded (pinned, see ld_stream_pinned) kProbAllAhead slots ahead of the arithmetic.  THREADS = kBlockProbAll: one block per SM, as k1 and k2 (the warps of co-resident blocks
 // finish at different times); 256: four blocks per SM for sizes that would leave SMs idle otherwise.
 template <bool VEC, int THREADS>
 __global__ void __launch_bounds__(THREADS, THREADS >= 512 ? 1 : 4)
@@ -195,15 +196,29 @@ prob_all_kernel(const __grid_constant__ ProbAllArgs a, const double* __restrict_
             E1 = (j1 < n) ? ld_stream_pinned(E_true + j1) : 1.0;
         }
     };
+    // the energies are loaded kProbAllAhead slots ahead: the kernel runs at 0.8-0.9 of the HBM bandwidth, where a load
+    // queues behind the stores of everybody's previous slots (ncu, one slot ahead: 30 % of all warp samples sat on the
+    // first use of the prefetched energy, long scoreboard)
     size_t i = (size_t)blockIdx.x * THREADS + threadIdx.x;
-    double N0 = 1.0, N1 = 1.0;
-    if (i < nslots) load(i, N0, N1);
+    double Q[kProbAllAhead][2];
+#pragma unroll
+    for (int d = 0; d < kProbAllAhead; ++d) {
+        Q[d][0] = 1.0;
+        Q[d][1] = 1.0;
+        if (i + d * stride < nslots) load(i + d * stride, Q[d][0], Q[d][1]);
+    }
     while (i < nslots) {
         const size_t j0 = VEC ? 2 * i : (i / THREADS) * (2 * THREADS) + (i % THREADS);
         const size_t j1 = VEC ? j0 + 1 : j0 + THREADS;
-        const double E0 = N0, E1 = N1;
+        const double E0 = Q[0][0], E1 = Q[0][1];
+#pragma unroll
+        for (int d = 0; d + 1 < kProbAllAhead; ++d) {
+            Q[d][0] = Q[d + 1][0];
+            Q[d][1] = Q[d + 1][1];
+        }
         i += stride;
-        if (i < nslots) load(i, N0, N1);
+        if (i + (kProbAllAhead - 1) * stride < nslots)
+            load(i + (kProbAllAhead - 1) * stride, Q[kProbAllAhead - 1][0], Q[kProbAllAhead - 1][1]);
         double P0[9], P1[9];
         prob_nine(a, E0, P0);
         prob_nine(a, E1, P1);

@@ -46,9 +46,9 @@ CAPTURES: Dict[str, dict] = {
                files=_EVENT, what="osc_prob, 1e5 events, mu->mu and mu->e (configs[0]); mean of the two launches"),
     "k1b": dict(csv="r2_k1b_ops.csv", kernels=r"prob_all_kernel", calls=1, units=10_000_000, unit="event",
                 files=_EVENT, what="osc_prob_all, 1e7 events, 9 outputs (configs[1])"),
-    "k4": dict(csv="r2_k4_ops.csv", kernels=r"scan_", calls=1, units=1_000_000 * 1024, unit="(event, point)",
+    "k4": dict(csv="r2_k4_ops.csv", kernels=r"scan_|sort_", calls=1, units=1_000_000 * 1024, unit="(event, point)",
                files=_SCAN, what="osc_reweight_bin_batch, 1e6 events x 1024 grid points, all kernels of one call (configs[3])"),
-    "k5": dict(csv="r2_k5_ops.csv", kernels=r"scan_", calls=1, units=1_000_000 * 1024, unit="(event, point)",
+    "k5": dict(csv="r2_k5_ops.csv", kernels=r"scan_|sort_", calls=1, units=1_000_000 * 1024, unit="(event, point)",
                files=_SCAN, what="the same call forced through k5 (osc_set_batch_path), all kernels of one call"),
     "plan": dict(csv="r2_plan_ops.csv", kernels=r"scan_full_one_kernel", calls=1, units=10_000_000, unit="event",
                  files=_SCAN, what="osc_plan_reweight_bin, 1e7 pre-sorted events (main kernel)"),

@@ -223,6 +223,25 @@ CallScratch call_scratch(char* scratch)
     return c;
 }
 
+// Launch with the programmatic-stream-serialization attribute (programmatic dependent launch): the set-up of this launch
+// may overlap the tail of the kernel before it on the stream; the kernels call griddepcontrol.wait before they touch
+// global memory (osc_kernels.cuh, pdl_wait).  After a kernel that never triggers, the launch is ordered as usual.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), int grid, int block, size_t smem, cudaStream_t st, Args&&... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
 template <bool VEC, int THREADS, int SLOTS = kSlots>
 int launch_k2(int grid, size_t smem, cudaStream_t st, const BinArgs& args, const double* E_true, const double* E_reco,
               const double* w0, const int8_t* channel, size_t n, double energy_scale, const double* bin_edges,
@@ -235,20 +254,8 @@ int launch_k2(int grid, size_t smem, cudaStream_t st, const BinArgs& args, const
                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured.store(smem, std::memory_order_relaxed);
     }
-    // programmatic dependent launch: the set-up of this launch may overlap the tail of the kernel before it on the
-    // stream; the kernel waits (griddepcontrol.wait) before it touches global memory (osc_kernels.cuh, pdl_wait)
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)grid);
-    cfg.blockDim = dim3(THREADS);
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    CUDA_TRY(cudaLaunchKernelEx(&cfg, reweight_bin_kernel<VEC, THREADS, SLOTS>, args, E_true, E_reco, w0, channel, n,
-                                energy_scale, bin_edges, n_bins, n_sub, cs.ms, cs.table_cache, hist_out));
+    CUDA_TRY(launch_pdl(reweight_bin_kernel<VEC, THREADS, SLOTS>, grid, THREADS, smem, st, args, E_true, E_reco, w0, channel, n,
+                        energy_scale, bin_edges, n_bins, n_sub, cs.ms, cs.table_cache, hist_out));
     return post_launch("osc_reweight_bin");
 }
 
@@ -363,18 +370,8 @@ int launch_k2s(int grid, size_t smem, cudaStream_t st, const BinArgs& args, cons
                                       (int)smem));
         configured.store(smem, std::memory_order_relaxed);
     }
-    cudaLaunchConfig_t cfg = {};                      // programmatic dependent launch, as launch_k2
-    cfg.gridDim = dim3((unsigned)grid);
-    cfg.blockDim = dim3(256);
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    CUDA_TRY(cudaLaunchKernelEx(&cfg, reweight_bin_scales_kernel<VEC, 256, NS>, args, sc, E_true, E_reco, w0, channel, n,
-                                bin_edges, n_bins, n_sub, cs.ms, cs.table_cache, hist_out));
+    CUDA_TRY(launch_pdl(reweight_bin_scales_kernel<VEC, 256, NS>, grid, 256, smem, st, args, sc, E_true, E_reco, w0, channel, n,
+                        bin_edges, n_bins, n_sub, cs.ms, cs.table_cache, hist_out));
     return post_launch("osc_reweight_bin_scales");
 }
 
@@ -542,11 +539,11 @@ int osc_prob_all(const double* E_true, size_t n, int antinu, double* P_out, void
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const bool vec = aligned(E_true, 16) && aligned(P_out, 16) && n % 2 == 0;
     if (big) {
-        if (vec) prob_all_kernel<true, kT><<<grid, kT, 0, st>>>(a, E_true, n, P_out);
-        else prob_all_kernel<false, kT><<<grid, kT, 0, st>>>(a, E_true, n, P_out);
+        if (vec) CUDA_TRY(launch_pdl(prob_all_kernel<true, kT>, grid, kT, 0, st, a, E_true, n, P_out));
+        else CUDA_TRY(launch_pdl(prob_all_kernel<false, kT>, grid, kT, 0, st, a, E_true, n, P_out));
     } else {
-        if (vec) prob_all_kernel<true, kBlock><<<grid, kBlock, 0, st>>>(a, E_true, n, P_out);
-        else prob_all_kernel<false, kBlock><<<grid, kBlock, 0, st>>>(a, E_true, n, P_out);
+        if (vec) CUDA_TRY(launch_pdl(prob_all_kernel<true, kBlock>, grid, kBlock, 0, st, a, E_true, n, P_out));
+        else CUDA_TRY(launch_pdl(prob_all_kernel<false, kBlock>, grid, kBlock, 0, st, a, E_true, n, P_out));
     }
     return post_launch("osc_prob_all");
 }

@@ -227,8 +227,9 @@ constexpr int kMergeSegs = 8; // at most this many threads share the partials of
 // hist: [n_sub][nh] sub-histograms of this block in shared memory (n_sub >= kMergeSegs, nh even, hist 16-byte aligned;
 // the memory is reused as scratch by the last block).  Every block writes its sum to ms.partial; the block that arrives
 // last (ticket) adds the partials of all blocks in block order into out[nh].  One level: the critical path after the
-// slowest block is one fence, one atomic and the loads of the partials, which up to kMergeSegs threads per pair of cells
-// issue all at once.  Every sum has a fixed order (given the launch shape), so the result is a deterministic function
+// slowest block is one atomic and the loads of the partials, which up to kMergeSegs threads per pair of cells issue
+// twelve at a time (2.8 us for 237 kB through ONE SM; the two-level scheme of round 1 rebuilt on the same atomics and
+// paired loads -- ten group leaders, then one -- was 1 us SLOWER per call: two more barriers and a second ticket).  Every sum has a fixed order (given the launch shape), so the result is a deterministic function
 // of the inputs.  Ordering: the barrier orders the block's stores before thread 0's release-acquire atomic, which is
 // cumulative (the pattern of a grid-wide barrier).  Must be called by all threads of the block; returns true in the last block (all
 // threads), false elsewhere.

@@ -182,6 +182,8 @@ __global__ void __launch_bounds__(THREADS, THREADS >= 512 ? 1 : 4)
 prob_all_kernel(const __grid_constant__ ProbAllArgs a, const double* __restrict__ E_true, size_t n,
                 double* __restrict__ P_out)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     const size_t nslots = VEC ? (n + 1) / 2 : ((n + 2 * THREADS - 1) / (2 * THREADS)) * THREADS;
     const size_t stride = (size_t)gridDim.x * THREADS;
     auto load = [&](size_t i, double& E0, double& E1) {

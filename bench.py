@@ -101,6 +101,11 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append((time.time(), line.strip()))
 
+    def wait_first_row(self, timeout: float = 3.0):
+        t = time.time()
+        while self.proc is not None and not self.rows and time.time() - t < timeout:
+            time.sleep(0.01)
+
     def stop(self, t0: float = None, t1: float = None):
         t0 = self.t_start if t0 is None else t0
         t1 = time.time() if t1 is None else t1
@@ -288,10 +293,12 @@ class Ctx:
 def _time_steps(ctx: Ctx, step, steps: int, warm: int, flush: bool = False):
     """Per-step CUDA events on the launching stream (an L2 flush, if any, stays outside the timed intervals)."""
     torch = ctx.torch
+    sampler = ClockSampler(ctx.local)
     for i in range(warm):
         step(i)
+    sampler.wait_first_row()
+    step(warm)
     torch.cuda.synchronize()
-    sampler = ClockSampler(ctx.local)
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     l0 = ctx.osc.osc_launch_count()
     for i, (a, b) in enumerate(evs):
@@ -533,12 +540,18 @@ def main():
         barrier()
         return max_over_ranks(a.elapsed_time(b))
 
+    # the clock sampler starts BEFORE the warm-up and the timed region waits for its first row: the start-up of nvidia-smi
+    # (~0.2 s of driver queries) otherwise falls into the few milliseconds that are timed and costs 0.7 % of `value`
+    sampler = ClockSampler(local) if rank == 0 else None
     for _ in range(warm):
+        step()
+    if sampler is not None:
+        sampler.wait_first_row()
+    for _ in range(2):
         step()
     barrier()
 
     # ---- timed region: device-resident inputs -----------------------------------------------------------------
-    sampler = ClockSampler(local) if rank == 0 else None
     launches0 = osc.osc_launch_count()
     t_wall0 = time.time()
     ms = timed(step, args.steps)
@@ -558,6 +571,8 @@ def main():
 
     torch.cuda.synchronize()
     ks, ke = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for _ in range(3):             # the device has just idled through a host round trip: three untimed launches first
+        one_k2()
     ks.record(stream)
     for _ in range(reps):
         one_k2()

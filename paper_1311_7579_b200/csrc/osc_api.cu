@@ -214,11 +214,25 @@ struct CallScratch {
     unsigned char* table_cache;
 };
 
-CallScratch call_scratch(char* scratch)
+// One merge level while the partial sums of a launch are at most 512 kB (one SM reads them in the shadow of a few
+// microseconds), two levels above that (osc_hist.cuh, block_merge).
+int merge_groups(int grid, size_t nh)
+{
+    return (size_t)grid * nh * sizeof(double) <= (size_t)512 * 1024 ? 1 : (grid + kGroup - 1) / kGroup;
+}
+
+size_t merge_scratch_bytes(int grid, size_t nh)
+{
+    return kScratchHead + ((size_t)grid + (size_t)merge_groups(grid, nh)) * nh * sizeof(double);
+}
+
+CallScratch call_scratch(char* scratch, int grid, size_t nh)
 {
     CallScratch c;
     c.ms.counters = reinterpret_cast<unsigned int*>(scratch);
     c.ms.partial = reinterpret_cast<double*>(scratch + kScratchHead);
+    c.ms.gpartial = c.ms.partial + (size_t)grid * nh;
+    c.ms.ngroups = merge_groups(grid, nh);
     c.table_cache = reinterpret_cast<unsigned char*>(scratch + kCounterBytes);
     return c;
 }
@@ -325,8 +339,8 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     const int grid = (int)g;
 
     ScratchLease lease;
-    if ((rc = stream_scratch(kScratchHead + (size_t)grid * nh * sizeof(double), st, lease))) return rc;
-    const CallScratch ms = call_scratch(lease.p);
+    if ((rc = stream_scratch(merge_scratch_bytes(grid, nh), st, lease))) return rc;
+    const CallScratch ms = call_scratch(lease.p, grid, nh);
 
     const bool vec = aligned(E_true, 16) && aligned(E_reco, 16) && aligned(w0, 16) && aligned(channel, 2);
 #define OSC_K2_SINGLE(T)                                                                                               \
@@ -396,8 +410,8 @@ int launch_reweight_scales(const BinArgs& args, const double* E_true, const doub
     if (ntiles < g) g = ntiles;
     const int grid = (int)g;
     ScratchLease lease;
-    if ((rc = stream_scratch(kScratchHead + (size_t)grid * nht * sizeof(double), st, lease))) return rc;
-    const CallScratch ms = call_scratch(lease.p);
+    if ((rc = stream_scratch(merge_scratch_bytes(grid, nht), st, lease))) return rc;
+    const CallScratch ms = call_scratch(lease.p, grid, nht);
     ScaleArgs sc;
     for (int k = 0; k < kMaxScales; ++k) sc.s[k] = k < n_scales ? scales[k] : 1.0;
     const bool vec = aligned(E_true, 16) && aligned(E_reco, 16) && aligned(w0, 16) && aligned(channel, 2);
@@ -1246,8 +1260,8 @@ int osc_bin_centre_compare(const double* E_true, const double* w0, const int8_t*
         if (ntiles < g) g = ntiles;
         const int grid = (int)g;
         ScratchLease lease;
-        if ((rc = stream_scratch(kScratchHead + (size_t)grid * nh * sizeof(double), st, lease))) return rc;
-        const MergeScratch ms = call_scratch(lease.p).ms;
+        if ((rc = stream_scratch(merge_scratch_bytes(grid, (size_t)nh), st, lease))) return rc;
+        const MergeScratch ms = call_scratch(lease.p, grid, (size_t)nh).ms;
         if (two_slots) {
             if (smem > 48 * 1024)
                 CUDA_TRY(cudaFuncSetAttribute(unit_hist_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

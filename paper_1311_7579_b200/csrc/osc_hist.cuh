@@ -166,13 +166,17 @@ __device__ __forceinline__ void warp_hist_add2_single(const LaneHist& lh, int ce
     warp_hist_commit_single(p, rmax1, w0, w1);
 }
 
-// Scratch of one call: counters[1] | partial[grid][nh].  It lives in a buffer the library keeps per (device, stream);
-// calls on one stream are ordered, so they can share it.  The ticket counter is zero when a kernel starts and the block
-// that consumes it sets it back to zero.
+// Scratch of one call: counters[ngroups + 1] | partial[grid][nh] | gpartial[ngroups][nh].  It lives in a buffer the
+// library keeps per (device, stream); calls on one stream are ordered, so they can share it.  The ticket counters are zero
+// when a kernel starts and the blocks that consume them set them back to zero.  ngroups = 1: one-level merge.
 struct MergeScratch {
     double* partial;
+    double* gpartial;
     unsigned int* counters;
+    int ngroups;
 };
+
+constexpr int kGroup = 16; // blocks per first-level group of the two-level merge
 
 // src[0] + src[stride] + ... (count terms, added in that order), read through L2.  The loads of sixteen terms are
 // issued together before they are added: the merge is a chain of dependent L2 round trips otherwise, and it sits on
@@ -222,16 +226,70 @@ __device__ __forceinline__ double2 ordered_sum2_cg(const double2* src, int count
     return s;
 }
 
-constexpr int kMergeSegs = 8; // at most this many threads share the partials of one pair of cells in the final merge
+constexpr int kMergeSegs = 8; // at most this many threads share the partials of one pair of cells in a merge step
+
+// dst[nh] = src[0][nh] + src[1][nh] + ... + src[count - 1][nh], added in that order per cell (src rows nh apart, read through
+// L2; dst global).  A pair of cells is shared by up to kMergeSegs threads, each adds a contiguous range of rows with its
+// loads in flight together; the ranges are then added in order.  scratch: shared memory for nh * kMergeSegs doubles
+// (only used when a block has at least two threads per pair of cells).  Called by all threads of the block.
+__device__ __forceinline__ void merge_rows(const double* src, int count, int nh, double* __restrict__ dst, double* scratch)
+{
+    const int npair = nh / 2;
+    int nseg = (int)blockDim.x / npair;
+    nseg = nseg < 1 ? 1 : (nseg > kMergeSegs ? kMergeSegs : nseg);
+    if (nseg > count) nseg = count;
+    if (nseg <= 1 || (reinterpret_cast<size_t>(dst) & 15)) {
+        for (int i = threadIdx.x; i < nh; i += blockDim.x) __stcg(dst + i, ordered_sum_cg(src + i, count, nh));
+        return;
+    }
+    const double2* src2 = reinterpret_cast<const double2*>(src);
+    const int per = (count + nseg - 1) / nseg;
+    const int t = (int)threadIdx.x;
+    double2* seg_sum = reinterpret_cast<double2*>(scratch);
+    if (t < nseg * npair) {
+        const int seg = t / npair, i = t - seg * npair;
+        const int b0 = seg * per, b1 = min(count, b0 + per);
+        seg_sum[t] = b1 > b0 ? ordered_sum2_cg(src2 + (size_t)b0 * npair + i, b1 - b0, npair) : make_double2(0.0, 0.0);
+    }
+    __syncthreads();
+    if (t < npair) {
+        double2 s = seg_sum[t];
+        for (int k = 1; k < nseg; ++k) {
+            const double2 v = seg_sum[k * npair + t];
+            s.x += v.x;
+            s.y += v.y;
+        }
+        __stcg(reinterpret_cast<double2*>(dst) + t, s);
+    }
+}
+
+// One thread takes a ticket with release-acquire semantics after a block barrier: the block's stores (ordered before by the
+// barrier, cumulativity as in a grid-wide barrier) are visible to whoever sees the ticket, and the loads that follow see
+// the stores of every block that took an earlier one.  Returns (block-uniform) whether this block took the last of `total`
+// tickets; the counter is then set back to zero for the next kernel on the stream.
+__device__ __forceinline__ bool take_ticket(unsigned int* counter, unsigned total, unsigned int* s_ticket)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned ticket;
+        asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(ticket) : "l"(counter) : "memory");
+        if (ticket == total - 1u) *counter = 0u;
+        *s_ticket = ticket;
+    }
+    __syncthreads();
+    return *s_ticket == total - 1u;
+}
 
 // hist: [n_sub][nh] sub-histograms of this block in shared memory (n_sub >= kMergeSegs, nh even, hist 16-byte aligned;
-// the memory is reused as scratch by the last block).  Every block writes its sum to ms.partial; the block that arrives
-// last (ticket) adds the partials of all blocks in block order into out[nh].  One level: the critical path after the
-// slowest block is one atomic and the loads of the partials, which up to kMergeSegs threads per pair of cells issue
-// twelve at a time (2.8 us for 237 kB through ONE SM; the two-level scheme of round 1 rebuilt on the same atomics and
-// paired loads -- ten group leaders, then one -- was 1 us SLOWER per call: two more barriers and a second ticket).  Every sum has a fixed order (given the launch shape), so the result is a deterministic function
-// of the inputs.  Ordering: the barrier orders the block's stores before thread 0's release-acquire atomic, which is
-// cumulative (the pattern of a grid-wide barrier).  Must be called by all threads of the block; returns true in the last block (all
+// the memory is reused as scratch by the merging blocks).  Every block writes its sum to ms.partial.
+//   ms.ngroups == 1 (the host's choice while grid x nh partial sums are at most 512 kB): the block that arrives last
+//     (ticket) adds the partials of all blocks in block order into out[nh].  The critical path after the slowest block is
+//     one atomic and the loads of the partials -- 2.8 us for the 237 kB of 148 blocks x 200 cells through ONE SM; the
+//     two-level scheme below was 1 us slower there (a second ticket and two more barriers);
+//   otherwise: the last block of each group of kGroup adds the group's partials into ms.gpartial, and the last of those
+//     adds the groups into out -- with 296 blocks x 600 cells (three energy scales) one SM would read 1.4 MB (16 us).
+// One pass, no second launch.  Every sum has a fixed order (given the launch shape), so the result is a deterministic
+// function of the inputs.  Must be called by all threads of the block; returns true in the block that wrote `out` (all
 // threads), false elsewhere.
 __device__ __forceinline__ bool block_merge(double* hist, int n_sub, int nh, const MergeScratch& ms,
                                             double* __restrict__ out, unsigned int* s_ticket)
@@ -251,47 +309,18 @@ __device__ __forceinline__ bool block_merge(double* hist, int n_sub, int nh, con
         for (; w < n_sub; ++w) s0 += hist[(size_t)w * nh + i];
         __stcg(my_partial + i, (s0 + s1) + (s2 + s3));
     }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        // release: the block's partial (ordered before this by the barrier) is visible to whoever sees the ticket;
-        // acquire: the last block's loads below see every other block's partial
-        unsigned ticket;
-        asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(ticket) : "l"(ms.counters) : "memory");
-        if (ticket == gridDim.x - 1u) ms.counters[0] = 0u;  // last block: nobody else reads it again
-        *s_ticket = ticket;
-    }
-    __syncthreads();
-    if (*s_ticket != gridDim.x - 1u) return false;
-
-    const int grid = (int)gridDim.x;
-    const int npair = nh / 2;
-    int nseg = (int)blockDim.x / npair;
-    nseg = nseg < 1 ? 1 : (nseg > kMergeSegs ? kMergeSegs : nseg);
-    const double2* part2 = reinterpret_cast<const double2*>(ms.partial);
-    double2* out2 = reinterpret_cast<double2*>(out);
-    if (nseg == 1 || (reinterpret_cast<size_t>(out) & 15)) {
-        for (int i = threadIdx.x; i < nh; i += blockDim.x) out[i] = ordered_sum_cg(ms.partial + i, grid, nh);
+    if (ms.ngroups <= 1) {
+        if (!take_ticket(ms.counters, gridDim.x, s_ticket)) return false;
+        merge_rows(ms.partial, (int)gridDim.x, nh, out, hist);
         return true;
     }
-    // a pair of cells is shared by nseg threads, each adds a contiguous range of blocks; the ranges are then added in order
-    const int per = (grid + nseg - 1) / nseg;
-    const int t = (int)threadIdx.x;
-    double2* seg_sum = reinterpret_cast<double2*>(hist);
-    if (t < nseg * npair) {
-        const int seg = t / npair, i = t - seg * npair;
-        const int b0 = seg * per, b1 = min(grid, b0 + per);
-        seg_sum[t] = b1 > b0 ? ordered_sum2_cg(part2 + (size_t)b0 * npair + i, b1 - b0, npair) : make_double2(0.0, 0.0);
-    }
-    __syncthreads();
-    if (t < npair) {
-        double2 s = seg_sum[t];
-        for (int k = 1; k < nseg; ++k) {
-            const double2 v = seg_sum[k * npair + t];
-            s.x += v.x;
-            s.y += v.y;
-        }
-        out2[t] = s;
-    }
+    const int group = blockIdx.x / kGroup;
+    const int gfirst = group * kGroup;
+    const int gsize = min(kGroup, (int)gridDim.x - gfirst);
+    if (!take_ticket(ms.counters + 1 + group, (unsigned)gsize, s_ticket)) return false;
+    merge_rows(ms.partial + (size_t)gfirst * nh, gsize, nh, ms.gpartial + (size_t)group * nh, hist);
+    if (!take_ticket(ms.counters, (unsigned)ms.ngroups, s_ticket)) return false;
+    merge_rows(ms.gpartial, ms.ngroups, nh, out, hist);
     return true;
 }
 

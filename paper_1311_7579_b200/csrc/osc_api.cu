@@ -136,6 +136,24 @@ int check_bin_args(const double* E_true, const double* E_reco, const double* w0,
     return OSC_OK;
 }
 
+// The stream-ordered allocator returns freed memory to the driver at the next synchronisation unless the pool is told to
+// keep some: with the default threshold of zero every batched call would pay for fresh device allocations (hundreds of
+// microseconds on the host).  Once per device, the default pool is allowed to retain up to 512 MB.
+int keep_pool_memory()
+{
+    static std::atomic<bool> done[64];
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64 || done[dev].load(std::memory_order_relaxed)) return OSC_OK;
+    cudaMemPool_t pool = nullptr;
+    CUDA_TRY(cudaDeviceGetDefaultMemPool(&pool, dev));
+    unsigned long long current = 0, keep = 512ull << 20;
+    CUDA_TRY(cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &current));
+    if (current < keep) CUDA_TRY(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+    done[dev].store(true, std::memory_order_relaxed);
+    return OSC_OK;
+}
+
 // Stream-ordered scratch of one call; freed (stream-ordered) when it goes out of scope.
 struct Scratch {
     char* p = nullptr;
@@ -143,6 +161,8 @@ struct Scratch {
     int alloc(size_t bytes, cudaStream_t s)
     {
         st = s;
+        int rc = keep_pool_memory();
+        if (rc) return rc;
         CUDA_TRY(cudaMallocAsync((void**)&p, bytes, s));
         return OSC_OK;
     }

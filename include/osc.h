@@ -132,7 +132,9 @@ int osc_reweight_bin_scales(const double *E_true, const double *E_reco, const do
  *   - points that differ only in sin2_th23 and delta_cp share the matter eigen-problem.  When the list has
  *     at least 8 points per such group on average (a scan grid: "only theta23 and dm2_32
  *     float"), the events are sorted by histogram cell once and the eigen-solve is done once per (event,
- *     group); a point then costs 4 to 6 fused multiply-adds per event (kernel k4, csrc/osc_scan.cuh);
+ *     group); a point then costs 3 to 6 fused multiply-adds per event (k4, csrc/osc_scan.cuh: from 4e5 events
+ *     on one launch per sub-group of 32 points with the point monomials in the kernel parameters, below that
+ *     one launch with the event terms in shared memory);
  *   - otherwise every (event, point) pair gets the full closed form: from 4 points on (6 for more than
  *     2e6 events), on the events sorted by histogram cell, with the weights of a cell summed in registers
  *     (kernel k5); below that the sort does not pay and every point gets its own pass of
@@ -211,7 +213,8 @@ int osc_reweight_bin_scales_host(const double *E_true_host, const double *E_reco
 
 /* Measurement and test overrides (process-wide, thread-safe; they affect calls enqueued afterwards).
  *   osc_set_batch_path  path = "auto" (default: the library chooses, see osc_reweight_bin_batch), "k2", "k4" or "k5":
- *                       the code path of osc_reweight_bin_batch / osc_plan_reweight_bin_batch ("k2" does not apply to plans).
+ *                       the code path of osc_reweight_bin_batch / osc_plan_reweight_bin_batch ("k2" does not apply to plans);
+ *                       "k4s" / "k4c": k4 with its shared-memory kernel / its kernel-parameter kernel whatever the size.
  *   osc_set_k2_tuning   launch shape of osc_reweight_bin's kernel; 0 leaves a field to the library.
  *                       threads in {128, 256, 384, 512, 768}, slots in {1, 2} (sub-histograms per warp: one, or one per
  *                       event of the lane), n_sub in {1, 2, 4} (sub-histograms per slot), blocks_per_sm <= 16.

@@ -392,7 +392,7 @@ def _check_host_events(E_true, E_reco, w0, channel) -> None:
 
 
 def osc_set_batch_path(path: str) -> None:
-    """"auto" | "k2" | "k4" | "k5": code path of the batched calls (measurements and tests)."""
+    """"auto" | "k2" | "k4" | "k4s" | "k4c" | "k5": code path of the batched calls (measurements and tests)."""
     _check(lib().osc_set_batch_path(path.encode()))
 
 

@@ -6,9 +6,11 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
+#include <cmath>
 #include <cstring>
 #include <array>
 #include <complex>
+#include <limits>
 #include <map>
 #include <memory>
 #include <mutex>
@@ -34,7 +36,7 @@ std::atomic<unsigned long long> g_launches{0};
 
 // Measurement / test overrides (osc_set_batch_path, osc_set_k2_tuning); 0 = the library chooses.  Never read from
 // the environment: a stray variable must not change launch shapes in a fitter that calls the library 1e6 times.
-std::atomic<int> g_batch_path{0};                       // 0 auto, 2 k2, 4 k4, 5 k5
+std::atomic<int> g_batch_path{0};                       // 0 auto, 2 k2, 4 k4, 41 / 42 k4 with the slice / constant-bank kernel, 5 k5
 std::atomic<int> g_tune_threads{0}, g_tune_slots{0}, g_tune_nsub{0}, g_tune_bps{0};
 #ifndef OSC_SORT_CHUNK
 #define OSC_SORT_CHUNK 2048
@@ -681,6 +683,9 @@ GroupKey group_key(const osc_params& p)
 struct ScanPlan {
     std::vector<ScanGroup> groups;
     std::vector<ScanSub> subs;
+    std::vector<ScanConstArgs> consts;   // subs[s] as the parameter block of scan_const_kernel (when const_ok)
+    bool const_ok = false;               // every channel of every group is one of the two kinds that kernel is built for
+    std::vector<std::array<std::complex<double>, kChannels * kScanElems>> coef;   // c_k of every point and channel
 };
 
 // Index sets of the rows of W = R23 D: row e touches column 0 only, rows mu and tau columns 1 and 2.
@@ -693,6 +698,81 @@ int w_cols(int flavour, int out[2])
     out[0] = 1;
     out[1] = 2;
     return 2;
+}
+
+// Sub-group s of the plan as the parameter block of scan_const_kernel (osc_scan.cuh).  The rows of W have unit length,
+// which takes one term off each kind of channel:
+//   three entries (numu -> numu): coefficients a, b on two diagonal entries z_a, z_b of S' and c on an off-diagonal
+//     entry z_c, all real, a + b = 1:  |a z_a + b z_b + c z_c|^2 = |s + a u + c v|^2 with s = z_b, u = z_a - z_b, v = z_c
+//     = |s|^2 + a^2 |u|^2 + c^2 |v|^2 + 2a Re(s u*) + 2c Re(s v*) + 2ac Re(u v*);  u is the amplitude of the
+//     pseudo-entry el_a - el_b (every field of ScanElem enters the amplitude linearly, and its delta is 0);
+//   two entries (numu -> nue): |c0|^2 + |c1|^2 = 1:  |c0 z0 + c1 z1|^2
+//     = |z1|^2 + |c0|^2 (|z0|^2 - |z1|^2) + 2 Re(c0 c1*) Re(z0 z1*) - 2 Im(c0 c1*) Im(z0 z1*).
+// The first term of each does not depend on the point: the kernel sums it once per event.  false: a channel is of
+// neither kind (the caller keeps to scan_main_kernel, which takes any term list).
+bool make_const_args(const ScanPlan& plan, size_t s, ScanConstArgs& a)
+{
+    const ScanSub& sub = plan.subs[s];
+    const ScanGroup& g = plan.groups[(size_t)sub.group];
+    std::memset(&a, 0, sizeof a);
+    a.set = g.set;
+    for (int l = 0; l < kScanLanes; ++l) a.pt[l] = sub.pt[l];
+    const double UNIT = 8 * std::numeric_limits<double>::epsilon();
+    for (int c = 0; c < kChannels; ++c) {
+        const ScanChan& gc = g.ch[c];
+        ScanChan& ac = a.ch[c];
+        ac.sa = gc.sa;
+        ac.nk = gc.nk;
+        for (int k = 0; k < gc.nk; ++k)
+            if (gc.el[k].ee != 0.0) return false;
+        if (gc.nk == 3) {
+            int d[3], nd = 0, o = -1;
+            for (int k = 0; k < 3; ++k) {
+                if (gc.el[k].delta != 0.0) d[nd++] = k;
+                else o = k;
+            }
+            if (nd != 2 || o < 0) return false;
+            a.mm |= 1 << c;
+            ac.el[0] = gc.el[d[1]];                                         // s = z_b
+            ac.el[1].delta = 0.0;                                           // u = z_a - z_b
+            ac.el[1].ee = 0.0;
+            ac.el[1].Tr0 = gc.el[d[0]].Tr0 - gc.el[d[1]].Tr0;
+            ac.el[1].T2r0 = gc.el[d[0]].T2r0 - gc.el[d[1]].T2r0;
+            ac.el[1].T2r1 = gc.el[d[0]].T2r1 - gc.el[d[1]].T2r1;
+            ac.el[2] = gc.el[o];                                            // v = z_c
+            for (int l = 0; l < kScanLanes; ++l) {
+                if (sub.pt[l] < 0) continue;
+                const std::complex<double>* ck = &plan.coef[(size_t)sub.pt[l]][(size_t)c * kScanElems];
+                if (ck[0].imag() != 0.0 || ck[1].imag() != 0.0 || ck[2].imag() != 0.0) return false;
+                const double ca = ck[d[0]].real(), cb = ck[d[1]].real(), cc = ck[o].real();
+                if (std::fabs(ca + cb - 1.0) > UNIT) return false;
+                a.mono[c][0][l] = ca * ca;
+                a.mono[c][1][l] = cc * cc;
+                a.mono[c][2][l] = 2.0 * ca;
+                a.mono[c][3][l] = 2.0 * cc;
+                a.mono[c][4][l] = 2.0 * ca * cc;
+            }
+        } else if (gc.nk == 2) {
+            if (gc.el[0].delta != 0.0 || gc.el[1].delta != 0.0) return false;
+            ac.el[0] = gc.el[0];
+            ac.el[1] = gc.el[1];
+            for (int l = 0; l < kScanLanes; ++l) {
+                if (sub.pt[l] < 0) continue;
+                const std::complex<double>* ck = &plan.coef[(size_t)sub.pt[l]][(size_t)c * kScanElems];
+                if (std::fabs(std::norm(ck[0]) + std::norm(ck[1]) - 1.0) > UNIT) return false;
+                const std::complex<double> x = ck[0] * std::conj(ck[1]);
+                a.mono[c][0][l] = std::norm(ck[0]);
+                a.mono[c][1][l] = 2.0 * x.real();
+                a.mono[c][2][l] = -2.0 * x.imag();
+            }
+        } else {
+            return false;
+        }
+        for (int t = 0; t < kConstTerms; ++t)
+            for (int l = 0; l < kScanLanes; ++l)
+                if (a.mono[c][t][l] != 0.0) ac.tmask |= 1 << t;
+    }
+    return true;
 }
 
 void build_scan_plan(const osc_params* points, int n_points, ScanPlan& plan)
@@ -711,6 +791,7 @@ void build_scan_plan(const osc_params* points, int n_points, ScanPlan& plan)
     }
     plan.groups.assign(members.size(), ScanGroup());
     plan.subs.clear();
+    plan.coef.assign((size_t)n_points, {});
     for (size_t g = 0; g < members.size(); ++g) {
         // T' of the group: the precompute with theta23 = 0, delta = 0 gives U = R13 R12
         osc_params q = points[members[g][0]];
@@ -771,6 +852,7 @@ void build_scan_plan(const osc_params* points, int n_points, ScanPlan& plan)
                     ck[k] = W[fout][i] * std::conj(W[fin][j]);
                     if (i != j) ck[k] += W[fout][j] * std::conj(W[fin][i]);
                 }
+                for (int k = 0; k < kScanElems; ++k) plan.coef[(size_t)mem[q]][(size_t)c * kScanElems + k] = ck[k];
                 double* mo = &mono[q][(size_t)c * kScanTerms];
                 static const int PK[3] = {0, 0, 1}, PL[3] = {1, 2, 2};
                 for (int k = 0; k < 3; ++k) mo[k] = std::norm(ck[k]);
@@ -800,6 +882,9 @@ void build_scan_plan(const osc_params* points, int n_points, ScanPlan& plan)
             }
         }
     }
+    plan.consts.resize(plan.subs.size());
+    plan.const_ok = true;
+    for (size_t s = 0; s < plan.subs.size() && plan.const_ok; ++s) plan.const_ok = make_const_args(plan, s, plan.consts[s]);
 }
 
 // Events sorted by histogram cell and cut into pieces (osc_scan.cuh): what k4 and k5 work on.  The buffers belong
@@ -921,6 +1006,55 @@ int scan_sort(const SortedEvents& se, const double* E_true, const double* E_reco
     return post_launch("sort of the events: scatter");
 }
 
+int scan_merge(const double* partial, const SortedEvents& se, int n_points, double* hist_out, cudaStream_t st)
+{
+    if (n_points < 32)
+        scan_merge_few_kernel<<<se.geo.ncells, 256, 0, st>>>(partial, se.unit_begin, se.geo.ncells, n_points, hist_out);
+    else
+        scan_merge_kernel<<<dim3((unsigned)se.geo.ncells, (unsigned)((n_points + 255) / 256)), 256, 0, st>>>(
+            partial, se.unit_begin, se.geo.ncells, n_points, hist_out);
+    return post_launch("batched reweighting on sorted events (merge)");
+}
+
+// k4 with the tables in the kernel parameters (scan_const_kernel): unless osc_set_batch_path("k4s") asks for the
+// shared-memory slice kernel, whenever every channel is of one of the two kinds the kernel is built for.
+// A launch per sub-group costs at least 14 us however few events there are (the launches of a call overlap only with their
+// neighbours), so it is the choice from 4e5 events on (1024 points in 32 sub-groups, ms per call, slice kernel / this
+// one: 1e5 events 0.33 / 0.46, 3e5 0.40 / 0.47, 5e5 0.61 / 0.50, 1e6 1.12 / 0.75, 1e7 11.2 / 6.4).
+// osc_set_batch_path("k4s" | "k4c") forces one of the two.
+constexpr size_t kConstMinEvents = 400000;
+constexpr size_t kConstUnits = 4096;   // pieces per launch the events are cut into (pieces of 128 / 256 / 320 / 384 / 512
+                                       // events at 1e6: 0.845 / 0.747 / 0.752 / 0.780 / 0.782 ms per call)
+bool scan_uses_const(const ScanPlan& plan, size_t n)
+{
+    const int forced = g_batch_path.load();
+    if (forced == 41 || !plan.const_ok) return false;
+    return forced == 42 || n >= kConstMinEvents;
+}
+
+// One launch per sub-group, nothing uploaded.  The first launch is ordered after the sort as usual; the others carry
+// the programmatic-serialization attribute: they start while their predecessor drains and, because every block waits
+// for the predecessor before it exits, complete in order, so the merge behind them sees all of partial[][].
+int scan_run_const(const SortedEvents& se, const ScanPlan& plan, int n_points, double* hist_out, cudaStream_t st)
+{
+    int rc;
+    const ScanGeom& geo = se.geo;
+    Scratch sc;
+    if ((rc = sc.alloc(round_up((size_t)geo.max_units * n_points * sizeof(double), 256), st))) return rc;
+    double* partial = reinterpret_cast<double*>(sc.p);
+    const int grid = (int)((geo.max_units + kScanWarps - 1) / kScanWarps);
+    for (size_t s = 0; s < plan.consts.size(); ++s) {
+        if (s == 0)
+            scan_const_kernel<<<grid, 32 * kScanWarps, 0, st>>>(plan.consts[s], se.sEt, se.sW, se.cell_begin, se.unit_begin,
+                                                               se.unit_cell, geo, se.n_bins, n_points, partial);
+        else
+            CUDA_TRY(launch_pdl(scan_const_kernel, grid, 32 * kScanWarps, 0, st, plan.consts[s], se.sEt, se.sW, se.cell_begin,
+                                se.unit_begin, se.unit_cell, geo, se.n_bins, n_points, partial));
+        if ((rc = post_launch("batched reweighting on sorted events (k4, tables in the kernel parameters)"))) return rc;
+    }
+    return scan_merge(partial, se, n_points, hist_out, st);
+}
+
 // The point kernels on sorted events: k4 (plan != nullptr: sub-groups of a scan grid) or k5 (full != nullptr: one
 // parameter block per point, every point its own eigen-problem), then the ordered merge of the pieces of every cell.
 int scan_run(const SortedEvents& se, const ScanPlan* plan, const std::vector<BinArgs>* full, int n_points,
@@ -928,6 +1062,9 @@ int scan_run(const SortedEvents& se, const ScanPlan* plan, const std::vector<Bin
 {
     int rc;
     ScanGeom geo = se.geo;
+    if (plan && g_batch_path.load() == 42 && !plan->const_ok)
+        return fail(OSC_ERR_INVALID_ARG, "osc_set_batch_path(\"k4c\"): a channel of this point list is of neither kind scan_const_kernel is built for");
+    if (plan && scan_uses_const(*plan, se.n)) return scan_run_const(se, *plan, n_points, hist_out, st);
     geo.nsubs = plan ? (int)plan->subs.size() : n_points;      // items a warp walks per piece: sub-groups or points
     int slots = geo.nsubs < 8 ? geo.nsubs : 8;
     geo.subs_per_slot = (geo.nsubs + slots - 1) / slots;
@@ -978,12 +1115,7 @@ int scan_run(const SortedEvents& se, const ScanPlan* plan, const std::vector<Bin
         }
         if ((rc = post_launch("batched reweighting on sorted events (k5, one eigen-problem per point)"))) return rc;
     }
-    if (n_points < 32)
-        scan_merge_few_kernel<<<geo.ncells, 256, 0, st>>>(partial, se.unit_begin, geo.ncells, n_points, hist_out);
-    else
-        scan_merge_kernel<<<dim3((unsigned)geo.ncells, (unsigned)((n_points + 255) / 256)), 256, 0, st>>>(
-            partial, se.unit_begin, geo.ncells, n_points, hist_out);
-    return post_launch("batched reweighting on sorted events (merge)");
+    return scan_merge(partial, se, n_points, hist_out, st);
 }
 
 // One batched call: sort into a stream-ordered scratch, then run.
@@ -995,6 +1127,7 @@ int launch_batch_scan(const ScanPlan* plan, const std::vector<BinArgs>* full, in
     const int nsubs = plan ? (int)plan->subs.size() : n_points;
     const int slots = nsubs < 8 ? nsubs : 8;
     size_t piece = round_up(n * (size_t)slots / 16384 + 1, 64);
+    if (plan && scan_uses_const(*plan, n)) piece = round_up(n / kConstUnits + 1, 64);   // a launch per sub-group: its own grid
     if (piece < 128) piece = 128;
     if (piece > (plan ? 8192u : 512u)) piece = plan ? 8192 : 512;   // k5 stages the piece in shared memory
     SortedEvents se;
@@ -1088,7 +1221,7 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
         ScanPlan plan;
         build_scan_plan(points, n_points, plan);
         bool use_scan = (size_t)n_points >= 8 * plan.subs.size();
-        if (forced == 4) use_scan = true;
+        if (forced == 4 || forced == 41 || forced == 42) use_scan = true;
         if (forced == 2 || forced == 5) use_scan = false;
         if (use_scan)
             return launch_batch_scan(&plan, nullptr, n_points, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
@@ -1204,7 +1337,7 @@ int osc_plan_reweight_bin_batch(const osc_plan* plan, const osc_params* points, 
     build_scan_plan(points, n_points, sp);
     bool use_scan = (size_t)n_points >= 8 * sp.subs.size();
     const int forced = g_batch_path.load();
-    if (forced == 4) use_scan = true;
+    if (forced == 4 || forced == 41 || forced == 42) use_scan = true;
     if (forced == 5) use_scan = false;
     if (use_scan) return scan_run(pl->se, &sp, nullptr, n_points, hist_out, st);
     std::vector<BinArgs> blocks((size_t)n_points);
@@ -1405,8 +1538,10 @@ int osc_set_batch_path(const char* path)
     if (!std::strcmp(path, "auto")) v = 0;
     if (!std::strcmp(path, "k2")) v = 2;
     if (!std::strcmp(path, "k4")) v = 4;
+    if (!std::strcmp(path, "k4s")) v = 41;
+    if (!std::strcmp(path, "k4c")) v = 42;
     if (!std::strcmp(path, "k5")) v = 5;
-    if (v < 0) return fail(OSC_ERR_INVALID_ARG, "osc_set_batch_path: \"%s\" is not auto, k2, k4 or k5", path);
+    if (v < 0) return fail(OSC_ERR_INVALID_ARG, "osc_set_batch_path: \"%s\" is not auto, k2, k4, k4s, k4c or k5", path);
     g_batch_path.store(v);
     return OSC_OK;
 }

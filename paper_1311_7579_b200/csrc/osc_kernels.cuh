@@ -58,14 +58,6 @@ __device__ __forceinline__ unsigned lanemask_lt()
     return m;
 }
 
-// Programmatic dependent launch (PTX griddepcontrol): the fused kernels are launched with the programmatic-stream-
-// serialization attribute, so a launch may be set up -- blocks scheduled, shared memory initialised -- while the kernel
-// before it on the stream is still draining; pdl_wait() returns once that kernel has completed and its memory is
-// visible, and nothing before it may touch global memory.  Without the attribute, or after a kernel that never
-// triggers, both are no-ops and the launch is ordered as usual.
-__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
-__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-
 // p[0 .. count) = 0.0 with 16-byte stores (p 16-byte aligned); called by all threads of the block.
 __device__ __forceinline__ void zero_shared(double* p, int count)
 {

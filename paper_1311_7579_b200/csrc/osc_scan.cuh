@@ -69,6 +69,25 @@ struct ScanSub {
     double mono[kChannels][kScanTerms][kScanLanes];
 };
 
+// One sub-group as the parameter block of scan_const_kernel: it travels as a __grid_constant__ kernel parameter, so
+// the monomials reach the fused multiply-adds of phase B through the constant bank.  A channel is of one of two kinds
+// (osc_api.cu, make_const_args, for the algebra):
+//   "three entries" (mm bit set; numu -> numu)  el[] = s, u, v;  w0 |s + a u + c v|^2 = w0 |s|^2 + sum_t q_t m_t with
+//       q = w0 {|u|^2, |v|^2, Re(s u*), Re(s v*), Re(u v*)},  m = {a^2, c^2, 2a, 2c, 2ac}
+//   "two entries" (numu -> nue)  el[] = z0, z1;  w0 |c0 z0 + c1 z1|^2 = w0 |z1|^2 + sum_t q_t m_t with
+//       q = w0 {|z0|^2 - |z1|^2, Re(z0 z1*), Im(z0 z1*)},  m = {|c0|^2, 2 Re(c0 c1*), -2 Im(c0 c1*)}
+// el[0] of a three-entry channel is a diagonal entry (delta = 1), every other el[] has delta = 0, and no entry is (e, e).
+// mono[channel][t][lane]; bit t of ch[channel].tmask: some lane has a non-zero m_t.
+constexpr int kConstTerms = 5;
+struct ScanConstArgs {
+    OscSet set;
+    int mm;                    // bit c: channel c is of kind "three entries"
+    int pad;
+    ScanChan ch[kChannels];
+    int pt[kScanLanes];
+    double mono[kChannels][kConstTerms][kScanLanes];
+};
+
 struct ScanGeom {
     size_t range;              // events per warp range of the sort passes (multiple of 32)
     unsigned nranges;
@@ -587,6 +606,169 @@ scan_main_kernel(const ScanGroup* __restrict__ groups, const ScanSub* __restrict
         }
         if (pt >= 0) partial[(size_t)u * npoints + pt] = (acc[0] + acc[1]) + (acc[2] + acc[3]);
     }
+}
+
+// ------------------------------------------------------------------------------------------------
+// k4 main kernel, second form: ONE sub-group per launch, its tables in the kernel parameters (ScanConstArgs).
+// Lane = event in both phases: phase A leaves the terms q_t of the lane's event in registers, phase B adds
+// q_t m_t[point] to 32 accumulators (one per point of the sub-group) with the monomials as constant-bank operands.
+// Why: a DFMA with three distinct register operands issues every 3 cycles on sm_100a, any other every 2
+// (profiles/r2_dfma_issue.md); lane = point needs acc += q * m with q from a shared-memory broadcast load and m in a
+// register (three registers plus a load per fused multiply-add), lane = event needs acc += q * c[bank][offset] (two
+// registers, no load).  The 32 accumulators of a lane are transposed through shared memory once per piece: lane p
+// sums the p-th accumulator of lanes 0..31 in that order, so partial[piece][point] is a deterministic function of
+// the inputs.  The launches of the sub-groups of a call do not depend on one another: each triggers its successor at
+// once (griddepcontrol.launch_dependents) and waits for its predecessor only before it exits, so the blocks of
+// the next sub-group fill the SMs as the current one drains and the launches complete in order.
+// Shared memory: red[kScanWarps][32][kRedStride]
+// ------------------------------------------------------------------------------------------------
+constexpr int kRedStride = 34;        // doubles per row of the transposition buffer: 16-byte rows, conflict-free
+
+// Events per lane and step, blocks per SM (configs[3], 1e6 events x 1024 points, ms per call): 1 event, 4 blocks 0.852;
+// 2 events, 4 blocks (128 registers, 250 bytes of spills) 0.747; 2 events, 3 blocks (168 registers) 0.807; 3 events,
+// 3 blocks 0.883.  A pair of monomials loaded once (LDCU.128) serves kConstEv fused multiply-adds per point.
+constexpr int kConstEv = 2;
+constexpr int kConstBlocksPerSM = 4;
+
+// Entry of S' with delta = 0, ee = 0 (an off-diagonal entry, or the difference of two diagonal ones), and with
+// delta = 1, ee = 0: scan_amp with the flags folded in.
+__device__ __forceinline__ void scan_amp_off(const OscEig& e, double A, const ScanElem& el, double& zr, double& zi)
+{
+    const double T2r = fma(A, el.T2r1, el.T2r0);
+    const double N0r = fma(-e.sum12, el.Tr0, T2r);
+    const double N2r = fma(-e.sum01, el.Tr0, T2r);
+    const double kn = e.kap2 * N2r;
+    zr = -(kn * e.s02);
+    zi = fma(kn, e.c02, -(e.kap0 * N0r));
+}
+__device__ __forceinline__ void scan_amp_diag(const OscEig& e, double A, const ScanElem& el, double& zr, double& zi)
+{
+    const double T2r = fma(A, el.T2r1, el.T2r0);
+    const double N0r = e.prod12 + fma(-e.sum12, el.Tr0, T2r);
+    const double N2r = e.prod01 + fma(-e.sum01, el.Tr0, T2r);
+    const double kn = e.kap2 * N2r;
+    zr = fma(-kn, e.s02, e.c1h);
+    zi = fma(kn, e.c02, fma(-e.kap0, N0r, e.s1h));
+}
+
+template <int CH, bool MM>
+__device__ __forceinline__ void scan_const_piece(const ScanConstArgs& P, const double* __restrict__ sEt,
+                                                 const double* __restrict__ sW, unsigned begin, unsigned end,
+                                                 unsigned lane, double (&acc)[kScanLanes], double& cst)
+{
+    constexpr int NT = MM ? 5 : 3;
+    const ScanChan& c = P.ch[CH];
+    const int tm = c.tmask;
+    unsigned e = begin + lane;
+    double E[kConstEv], w[kConstEv];
+#pragma unroll
+    for (int k = 0; k < kConstEv; ++k) {
+        E[k] = e + 32 * k < end ? __ldg(sEt + e + 32 * k) : 1.0;
+        w[k] = e + 32 * k < end ? __ldg(sW + e + 32 * k) : 0.0;
+    }
+#pragma unroll 1
+    for (unsigned s0 = begin; s0 < end; s0 += 32 * kConstEv) {
+        e += 32 * kConstEv;
+        double En[kConstEv], wn[kConstEv];
+#pragma unroll
+        for (int k = 0; k < kConstEv; ++k) {
+            En[k] = e + 32 * k < end ? __ldg(sEt + e + 32 * k) : 1.0;
+            wn[k] = e + 32 * k < end ? __ldg(sW + e + 32 * k) : 0.0;
+        }
+        // ---- phase A: S' entries of the lane's events, then the terms --------------------------------------
+        double q[kConstEv][NT];
+#pragma unroll
+        for (int k = 0; k < kConstEv; ++k) {
+            const double A = c.sa * E[k];
+            OscEig g;
+            eig_solve(P.set, A, rcp_pos(E[k]), g);
+            if (MM) {
+                double sr, si, ur, ui, vr, vi;
+                scan_amp_diag(g, A, c.el[0], sr, si);
+                scan_amp_off(g, A, c.el[1], ur, ui);
+                scan_amp_off(g, A, c.el[2], vr, vi);
+                cst = fma(w[k], fma(sr, sr, si * si), cst);
+                q[k][0] = w[k] * fma(ur, ur, ui * ui);
+                q[k][1] = w[k] * fma(vr, vr, vi * vi);
+                q[k][2] = w[k] * fma(sr, ur, si * ui);
+                q[k][3] = w[k] * fma(sr, vr, si * vi);
+                q[k][4] = w[k] * fma(ur, vr, ui * vi);
+            } else {
+                double zr0, zi0, zr1, zi1;
+                scan_amp_off(g, A, c.el[0], zr0, zi0);
+                scan_amp_off(g, A, c.el[1], zr1, zi1);
+                const double n1 = fma(zr1, zr1, zi1 * zi1);
+                cst = fma(w[k], n1, cst);
+                q[k][0] = w[k] * (fma(zr0, zr0, zi0 * zi0) - n1);
+                q[k][1] = w[k] * fma(zr0, zr1, zi0 * zi1);
+                q[k][2] = w[k] * fma(zi0, zr1, -(zr0 * zi1));
+            }
+        }
+        // ---- phase B: 32 points, the monomials from the kernel parameters ----------------------------------
+#pragma unroll
+        for (int t = 0; t < NT; ++t) {
+            if (tm & (1 << t)) {
+#pragma unroll
+                for (int p = 0; p < kScanLanes; ++p) {
+                    const double m = P.mono[CH][t][p];
+#pragma unroll
+                    for (int k = 0; k < kConstEv; ++k) acc[p] = fma(q[k][t], m, acc[p]);
+                }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < kConstEv; ++k) {
+            E[k] = En[k];
+            w[k] = wn[k];
+        }
+    }
+}
+
+__global__ void __launch_bounds__(32 * kScanWarps, kConstBlocksPerSM)
+scan_const_kernel(const __grid_constant__ ScanConstArgs P, const double* __restrict__ sEt, const double* __restrict__ sW,
+                  const unsigned int* __restrict__ cell_begin, const unsigned int* __restrict__ unit_begin,
+                  const unsigned short* __restrict__ unit_cell, ScanGeom geo, int nb, int npoints,
+                  double* __restrict__ partial)
+{
+    __shared__ __align__(16) double s_red[kScanWarps][kScanLanes * kRedStride];
+    pdl_launch_dependents();
+    const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const unsigned u = blockIdx.x * kScanWarps + warp;
+    if (u < __ldg(unit_begin + geo.ncells)) {
+        const int cell = (int)__ldg(unit_cell + u);
+        const unsigned cb = __ldg(cell_begin + cell), ce = __ldg(cell_begin + cell + 1);
+        const unsigned begin = cb + (u - __ldg(unit_begin + cell)) * geo.piece;
+        const unsigned end = min(ce, begin + geo.piece);
+        const int ch = cell / nb;
+        double acc[kScanLanes];
+#pragma unroll
+        for (int p = 0; p < kScanLanes; ++p) acc[p] = 0.0;
+        double cst = 0.0;                                       // the term every point shares
+        const bool mm = (P.mm >> ch) & 1;
+        switch (ch) {
+        case 0: if (mm) scan_const_piece<0, true>(P, sEt, sW, begin, end, lane, acc, cst); else scan_const_piece<0, false>(P, sEt, sW, begin, end, lane, acc, cst); break;
+        case 1: if (mm) scan_const_piece<1, true>(P, sEt, sW, begin, end, lane, acc, cst); else scan_const_piece<1, false>(P, sEt, sW, begin, end, lane, acc, cst); break;
+        case 2: if (mm) scan_const_piece<2, true>(P, sEt, sW, begin, end, lane, acc, cst); else scan_const_piece<2, false>(P, sEt, sW, begin, end, lane, acc, cst); break;
+        default: if (mm) scan_const_piece<3, true>(P, sEt, sW, begin, end, lane, acc, cst); else scan_const_piece<3, false>(P, sEt, sW, begin, end, lane, acc, cst); break;
+        }
+        // transposition: row = lane of the event, column = point; lane p then adds column p from the top
+        double* r = s_red[warp];
+#pragma unroll
+        for (int p = 0; p < kScanLanes; p += 2)
+            *reinterpret_cast<double2*>(r + lane * kRedStride + p) = make_double2(acc[p], acc[p + 1]);
+        __syncwarp();
+        double s[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+        for (int l = 0; l < kScanLanes; l += 4) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) s[k] += r[(l + k) * kRedStride + lane];
+        }
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) cst += __shfl_xor_sync(0xffffffffu, cst, off);
+        const int pt = P.pt[lane];
+        if (pt >= 0) partial[(size_t)u * npoints + pt] = ((s[0] + s[1]) + (s[2] + s[3])) + cst;
+    }
+    pdl_wait();
 }
 
 // ------------------------------------------------------------------------------------------------

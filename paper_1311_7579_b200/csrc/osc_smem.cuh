@@ -58,4 +58,12 @@ __device__ __forceinline__ void sts_f64_volatile(uint32_t a, double v)
     asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory");
 }
 
+// Programmatic dependent launch (PTX griddepcontrol): the fused kernels are launched with the programmatic-stream-
+// serialization attribute, so a launch may be set up -- blocks scheduled, shared memory initialised -- while the kernel
+// before it on the stream is still draining; pdl_wait() returns once that kernel has completed and its memory is
+// visible, and nothing before it may touch global memory.  Without the attribute, or after a kernel that never
+// triggers, both are no-ops and the launch is ordered as usual.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 } // namespace oscb

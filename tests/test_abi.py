@@ -191,6 +191,9 @@ def test_setters_validate():
     L = binding.lib()
     assert L.osc_set_batch_path(b"k7") == INVALID and b"k7" in L.osc_last_error()
     assert L.osc_set_batch_path(b"k5") == OK and L.osc_set_batch_path(b"auto") == OK
+    for path in (b"k2", b"k4", b"k4s", b"k4c"):
+        assert L.osc_set_batch_path(path) == OK
+    assert L.osc_set_batch_path(b"auto") == OK
     assert L.osc_set_k2_tuning(700, 0, 0, 0) == INVALID
     assert L.osc_set_k2_tuning(0, 3, 0, 0) == INVALID
     assert L.osc_set_k2_tuning(0, 0, 3, 0) == INVALID

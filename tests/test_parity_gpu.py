@@ -430,8 +430,13 @@ def test_batch_point_count_edge_cases(osc):
 # ------------------------------------------------------------------------------------------------
 # k4, the factorised path of the batched call (points that differ only in theta23 / delta_cp share the
 # eigen-problem).  osc_set_batch_path forces one path or the other (include/osc.h), so both are checked against the
-# oracle on the same inputs, and against each other.
+# oracle on the same inputs, and against each other.  k4 has two main kernels: "k4s" (shared-memory slice, lane = point)
+# and "k4c" (one launch per sub-group, monomials in the kernel parameters, lane = event); "k4" lets the library choose
+# (k4c from 4e5 events on).
 # ------------------------------------------------------------------------------------------------
+K4_PATHS = ["k4s", "k4c"]
+
+
 class batch_path:
     def __init__(self, which):
         self.which = which
@@ -472,26 +477,31 @@ def test_k4_ragged_groups_vs_oracle(osc):
     edges = wl.bin_edges()
     d = [dev(a) for a in (et, er, w0, ch)]
     ref = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 1.03, edges)
-    with batch_path("k4"):
-        got4 = host(osc.osc_reweight_bin_batch(pts, *d, 1.03, dev(edges)))
+    got4 = {}
+    for path in K4_PATHS:
+        with batch_path(path):
+            got4[path] = host(osc.osc_reweight_bin_batch(pts, *d, 1.03, dev(edges)))
     with batch_path("k2"):
         got3 = host(osc.osc_reweight_bin_batch(pts, *d, 1.03, dev(edges)))
     with batch_path("k5"):
         got5 = host(osc.osc_reweight_bin_batch(pts, *d, 1.03, dev(edges)))
-    assert_hist_close(got4, ref, "k4 ragged groups")
+    for path in K4_PATHS:
+        assert_hist_close(got4[path], ref, f"{path} ragged groups")
+        assert np.array_equal(got4[path] == 0.0, got3 == 0.0)
     assert_hist_close(got3, ref, "k2-per-point ragged groups")
     assert_hist_close(got5, ref, "k5 ragged groups")
-    assert np.array_equal(got4 == 0.0, got3 == 0.0) and np.array_equal(got5 == 0.0, got3 == 0.0)
+    assert np.array_equal(got5 == 0.0, got3 == 0.0)
 
 
-def test_k4_equals_k3_on_the_grid_with_more_events(osc):
+@pytest.mark.parametrize("k4", K4_PATHS)
+def test_k4_equals_k3_on_the_grid_with_more_events(osc, k4):
     pts = wl.scan_points()[:96]          # three dm2_32 groups of 32 points
     n = 200_000 + 33
     et, er, w0, ch = wl.events(n, seed=23)
     edges = wl.bin_edges()
     d = [dev(a) for a in (et, er, w0, ch)]
     de = dev(edges)
-    with batch_path("k4"):
+    with batch_path(k4):
         a = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, de))
         b = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, de))
     with batch_path("k2"):
@@ -509,7 +519,7 @@ def test_k4_equals_k3_on_the_grid_with_more_events(osc):
     assert_hist_close(a[pick], ref, "k4 vs oracle")
 
 
-@pytest.mark.parametrize("path", ["k4", "k5"])
+@pytest.mark.parametrize("path", K4_PATHS + ["k5"])
 @pytest.mark.parametrize("n", [0, 1, 31, 64, 65, 129, 1000])
 @pytest.mark.parametrize("nb,kind", [(1, "uniform"), (7, "random"), (50, "uniform")])
 def test_k4_small_and_ragged_sizes(osc, n, nb, kind, path):
@@ -528,7 +538,7 @@ def test_k4_small_and_ragged_sizes(osc, n, nb, kind, path):
     assert_hist_close(got, ref, f"{path} n={n} nb={nb}")
 
 
-@pytest.mark.parametrize("path", ["k2", "k4", "k5"])
+@pytest.mark.parametrize("path", ["k2"] + K4_PATHS + ["k5"])
 def test_batch_paths_with_many_bins(osc, path):
     """350 bins x 4 channels = 1400 cells: the per-warp counters of the sort passes and the cell search of the piece
     kernels at a size well beyond configs[3]'s 200 cells; "k2" is one pass of the single-set kernel per point."""
@@ -549,13 +559,13 @@ def test_batch_sorted_paths_with_768_bins(osc):
     edges = wl.bin_edges(768, 5.0)
     pts = [wl.table1(sin2_th23=0.3 + 0.04 * k, dm2_32=2.2e-3 + 1e-5 * (k // 5)) for k in range(10)]
     ref = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 1.0, edges)
-    for path in ("k4", "k5"):
+    for path in K4_PATHS + ["k5"]:
         with batch_path(path):
             got = host(osc.osc_reweight_bin_batch(pts, dev(et), dev(er), dev(w0), dev(ch), 1.0, dev(edges)))
         assert_hist_close(got, ref, f"{path} with 768 bins")
 
 
-@pytest.mark.parametrize("path", ["k4", "k5"])
+@pytest.mark.parametrize("path", K4_PATHS + ["k5"])
 def test_batch_sorted_paths_on_corner_parameters(osc, path):
     """The degenerate and extreme parameter sets of test_corner_parameters through the sorted batched kernels: every
     corner as its own group (k5), and every corner with four (theta23, delta) variations (k4)."""
@@ -565,7 +575,7 @@ def test_batch_sorted_paths_on_corner_parameters(osc, path):
     pts = []
     for c in CORNERS:
         base = wl.table1(**c)
-        for k in range(4 if path == "k4" else 1):
+        for k in range(4 if path in K4_PATHS else 1):
             pts.append(dict(base, sin2_th23=base["sin2_th23"] if k == 0 else 0.2 + 0.2 * k,
                             delta_cp=base["delta_cp"] if k == 0 else -2.5 + 1.7 * k))
     with batch_path(path):
@@ -574,12 +584,13 @@ def test_batch_sorted_paths_on_corner_parameters(osc, path):
     assert_hist_close(got, ref, f"{path} on corner parameters")
 
 
-def test_k4_all_events_dropped(osc):
+@pytest.mark.parametrize("k4", K4_PATHS)
+def test_k4_all_events_dropped(osc, k4):
     n = 500
     et, er, w0, ch = wl.events(n, seed=25)
     er[:] = 99.0
     pts = [wl.table1(sin2_th23=0.4), wl.table1(sin2_th23=0.6)]
-    with batch_path("k4"):
+    with batch_path(k4):
         got = host(osc.osc_reweight_bin_batch(pts, dev(et), dev(er), dev(w0), dev(ch), 1.0, dev(wl.bin_edges())))
     assert got.shape == (2, 4, 50) and float(np.abs(got).sum()) == 0.0
 
@@ -683,6 +694,11 @@ def test_plan_batch_grid_and_unrelated_points(osc):
         assert_hist_close(got, ref, f"plan batch {name}")
         direct = host(osc.osc_reweight_bin_batch(pts, *d, 1.0, dev(edges)))
         np.testing.assert_allclose(got, direct, rtol=1e-12, atol=0.0)
+        if name == "grid":                             # both main kernels of k4 on the plan's pieces
+            for path in K4_PATHS:
+                with batch_path(path):
+                    forced = host(osc.osc_plan_reweight_bin_batch(plan, pts))
+                assert_hist_close(forced, ref, f"plan batch grid, {path}")
 
 
 def test_outputs_stay_inside_their_buffers(osc):

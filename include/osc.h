@@ -199,7 +199,10 @@ int osc_bin_index(const double *E_true, const double *E_reco, const int8_t *chan
 
 /* Same as the osc_prob / osc_reweight_bin pair but with HOST buffers: copies the inputs to the device,
  * runs the kernels, copies the result back and synchronises.  This is the flow of the paper's Listing 1
- * and what bench.py times as "e2e". */
+ * and what bench.py times as "e2e".  The reweight calls send more than 2^20 events in up to 8
+ * chunks and run the kernel on one chunk while the next is on the bus; the per-chunk histograms are added in chunk
+ * order, so the result is still a deterministic function of the inputs (equal to the device call to rounding).
+ * Pinned host arrays make the copies asynchronous; pageable ones work, without the overlap. */
 int osc_prob_host(const double *E_true_host, size_t n, int flavour_in, int flavour_out, int antinu,
                   double *P_out_host);
 int osc_reweight_bin_host(const double *E_true_host, const double *E_reco_host, const double *w0_host,

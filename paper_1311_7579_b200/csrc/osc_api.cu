@@ -19,6 +19,7 @@
 #include <vector>
 
 #include "../../include/osc.h"
+#include "osc_host.cuh"
 #include "osc_kernels.cuh"
 #include "osc_like.cuh"
 #include "osc_scan.cuh"
@@ -395,6 +396,11 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
                                        n_bins, n_sub_t, ms, hist_out);
 }
 
+// Threads per block of k2s, 512 / kScalesThreads blocks per SM (126 registers either way).  1e7 events x 3 scales:
+// 256 x 2 blocks 242.5 us, 512 x 1 block 268.3 us (k2 itself is the other way round: its one block of 768 threads wins).
+constexpr int kScalesThreads = 256;
+constexpr int kScalesBlocksPerSM = 512 / kScalesThreads;
+
 template <bool VEC, int NS>
 int launch_k2s(int grid, size_t smem, cudaStream_t st, const BinArgs& args, const ScaleArgs& sc, const double* E_true,
                const double* E_reco, const double* w0, const int8_t* channel, size_t n, const double* bin_edges,
@@ -402,11 +408,11 @@ int launch_k2s(int grid, size_t smem, cudaStream_t st, const BinArgs& args, cons
 {
     static std::atomic<size_t> configured{0};
     if (configured.load(std::memory_order_relaxed) < smem) {
-        CUDA_TRY(cudaFuncSetAttribute(reweight_bin_scales_kernel<VEC, 256, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        CUDA_TRY(cudaFuncSetAttribute(reweight_bin_scales_kernel<VEC, kScalesThreads, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)smem));
         configured.store(smem, std::memory_order_relaxed);
     }
-    CUDA_TRY(launch_pdl(reweight_bin_scales_kernel<VEC, 256, NS>, grid, 256, smem, st, args, sc, E_true, E_reco, w0, channel, n,
+    CUDA_TRY(launch_pdl(reweight_bin_scales_kernel<VEC, kScalesThreads, NS>, grid, kScalesThreads, smem, st, args, sc, E_true, E_reco, w0, channel, n,
                         bin_edges, n_bins, n_sub, cs.ms, cs.table_cache, hist_out));
     return post_launch("osc_reweight_bin_scales");
 }
@@ -419,16 +425,16 @@ int launch_reweight_scales(const BinArgs& args, const double* E_true, const doub
 {
     const size_t nht = (size_t)n_scales * kChannels * n_bins;
     const size_t fixed = sizeof(double) * kBinArgsDoubles + bin_table_bytes(n_bins);
-    const size_t sub1 = sizeof(double) * 8 * kSlots * nht;              // 8 warps
-    if (2 * (fixed + sub1 + 1024) > kSmemBudget) return 1;
-    const int n_sub = 2 * (fixed + 2 * sub1 + 1024) <= kSmemBudget ? 2 : 1;
+    const size_t sub1 = sizeof(double) * (kScalesThreads / 32) * kSlots * nht;
+    if (kScalesBlocksPerSM * (fixed + sub1 + 1024) > kSmemBudget) return 1;
+    const int n_sub = kScalesBlocksPerSM * (fixed + 2 * sub1 + 1024) <= kSmemBudget ? 2 : 1;
     const size_t smem = fixed + n_sub * sub1;
     int sms = 0;
     int rc = sm_count(&sms);
     if (rc) return rc;
-    const size_t ntiles = (n + 511) / 512;
+    const size_t ntiles = (n + 2 * kScalesThreads - 1) / (2 * kScalesThreads);
     if (ntiles > 0xFFFFFFFFull) return fail(OSC_ERR_INVALID_ARG, "n = %zu events is more than one call takes (2^32 tiles)", n);
-    size_t g = (size_t)sms * 2;
+    size_t g = (size_t)sms * kScalesBlocksPerSM;
     if (ntiles < g) g = ntiles;
     const int grid = (int)g;
     ScratchLease lease;
@@ -451,14 +457,22 @@ int launch_reweight_scales(const BinArgs& args, const double* E_true, const doub
 }
 
 // Device staging buffers of the *_host entry points (grown on demand, reused between calls).
+constexpr int kHostChunks = 8;                 // chunks a host call's events cross PCIe in, at most
+constexpr size_t kHostChunkMin = 1u << 20;     // events per chunk, at least (a kernel launch per chunk: 7 us of fixed cost)
 struct HostPath {
     std::mutex mu;
-    cudaStream_t stream = nullptr;
+    cudaStream_t stream = nullptr;             // kernels, small copies
+    cudaStream_t copy_stream = nullptr;        // the event arrays, chunk after chunk
+    cudaEvent_t chunk_ready[kHostChunks] = {};
     char* buf = nullptr;
     size_t cap = 0;
     int ensure(size_t bytes)
     {
         if (!stream) CUDA_TRY(cudaStreamCreateWithFlags(&stream, cudaStreamNonBlocking));
+        if (!copy_stream) {
+            CUDA_TRY(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
+            for (int c = 0; c < kHostChunks; ++c) CUDA_TRY(cudaEventCreateWithFlags(&chunk_ready[c], cudaEventDisableTiming));
+        }
         if (bytes > cap) {
             if (buf) CUDA_TRY(cudaFree(buf));
             buf = nullptr;
@@ -1006,6 +1020,33 @@ int scan_sort(const SortedEvents& se, const double* E_true, const double* E_reco
     return post_launch("sort of the events: scatter");
 }
 
+// The plan of the last point list, kept: a scan is typically repeated over the same grid (other events, another energy
+// scale, the next step of a fit), and building the plan is 0.2 ms of host time for 1024 points -- a quarter of what the
+// GPU then needs for 1e6 events.  Compared bytewise (a list that differs only in padding bytes is rebuilt, never reused
+// wrongly); thread-safe; the plan is immutable once built.
+struct PlanCache {
+    std::mutex mu;
+    std::vector<unsigned char> key;
+    std::shared_ptr<const ScanPlan> plan;
+};
+PlanCache g_plan_cache;
+
+std::shared_ptr<const ScanPlan> scan_plan_for(const osc_params* points, int n_points)
+{
+    const size_t bytes = (size_t)n_points * sizeof(osc_params);
+    {
+        std::lock_guard<std::mutex> lk(g_plan_cache.mu);
+        if (g_plan_cache.plan && g_plan_cache.key.size() == bytes && !std::memcmp(g_plan_cache.key.data(), points, bytes))
+            return g_plan_cache.plan;
+    }
+    auto fresh = std::make_shared<ScanPlan>();
+    build_scan_plan(points, n_points, *fresh);
+    std::lock_guard<std::mutex> lk(g_plan_cache.mu);
+    g_plan_cache.key.assign(reinterpret_cast<const unsigned char*>(points), reinterpret_cast<const unsigned char*>(points) + bytes);
+    g_plan_cache.plan = fresh;
+    return fresh;
+}
+
 int scan_merge(const double* partial, const SortedEvents& se, int n_points, double* hist_out, cudaStream_t st)
 {
     if (n_points < 32)
@@ -1218,8 +1259,8 @@ int osc_reweight_bin_batch(const osc_params* points, int n_points, const double*
     // osc_set_batch_path overrides the choice (tests exercise all paths on the same inputs).
     const int forced = g_batch_path.load();
     {
-        ScanPlan plan;
-        build_scan_plan(points, n_points, plan);
+        const std::shared_ptr<const ScanPlan> held = scan_plan_for(points, n_points);
+        const ScanPlan& plan = *held;
         bool use_scan = (size_t)n_points >= 8 * plan.subs.size();
         if (forced == 4 || forced == 41 || forced == 42) use_scan = true;
         if (forced == 2 || forced == 5) use_scan = false;
@@ -1333,8 +1374,8 @@ int osc_plan_reweight_bin_batch(const osc_plan* plan, const osc_params* points, 
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     // same choice between the factorised kernel k4 and the one-eigen-problem-per-point kernel k5 as in
     // osc_reweight_bin_batch; the sort is already paid for, so there is no k2 branch
-    ScanPlan sp;
-    build_scan_plan(points, n_points, sp);
+    const std::shared_ptr<const ScanPlan> held = scan_plan_for(points, n_points);
+    const ScanPlan& sp = *held;
     bool use_scan = (size_t)n_points >= 8 * sp.subs.size();
     const int forced = g_batch_path.load();
     if (forced == 4 || forced == 41 || forced == 42) use_scan = true;
@@ -1496,10 +1537,15 @@ int osc_reweight_bin_scales_host(const double* E_true_host, const double* E_reco
     HostPath& g_host = *hp;
     std::lock_guard<std::mutex> lk(g_host.mu);
     const size_t nh = (size_t)kChannels * n_bins;
+    const size_t nout = (size_t)n_scales * nh;
+    // chunks of an even number of events (the 16-byte loads of the kernels), at most kHostChunks of at least kHostChunkMin
+    size_t chunk = std::max<size_t>(kHostChunkMin, (n + kHostChunks - 1) / kHostChunks);
+    chunk += chunk & 1;
+    const int n_chunks = n ? (int)((n + chunk - 1) / chunk) : 1;
     const size_t b8 = round_up(n * sizeof(double), 256);
     const size_t b1 = round_up(n, 256);
     const size_t be = round_up((size_t)(n_bins + 1) * sizeof(double), 256);
-    const size_t bh = round_up((size_t)n_scales * nh * sizeof(double), 256);
+    const size_t bh = round_up((size_t)(n_chunks + 1) * nout * sizeof(double), 256);
     if ((rc = g_host.ensure(3 * b8 + b1 + be + bh + 256))) return rc;
     char* p = g_host.buf;
     double* dEt = reinterpret_cast<double*>(p);
@@ -1507,18 +1553,42 @@ int osc_reweight_bin_scales_host(const double* E_true_host, const double* E_reco
     double* dW = reinterpret_cast<double*>(p + 2 * b8);
     int8_t* dC = reinterpret_cast<int8_t*>(p + 3 * b8);
     double* dEdges = reinterpret_cast<double*>(p + 3 * b8 + b1);
-    double* dH = reinterpret_cast<double*>(p + 3 * b8 + b1 + be);
-    cudaStream_t st = g_host.stream;
-    if (n) {
-        CUDA_TRY(cudaMemcpyAsync(dEt, E_true_host, n * sizeof(double), cudaMemcpyHostToDevice, st));
-        CUDA_TRY(cudaMemcpyAsync(dEr, E_reco_host, n * sizeof(double), cudaMemcpyHostToDevice, st));
-        CUDA_TRY(cudaMemcpyAsync(dW, w0_host, n * sizeof(double), cudaMemcpyHostToDevice, st));
-        CUDA_TRY(cudaMemcpyAsync(dC, channel_host, n, cudaMemcpyHostToDevice, st));
-    }
+    double* dH = reinterpret_cast<double*>(p + 3 * b8 + b1 + be);       // [0]: the result, [1 + c]: chunk c
+    cudaStream_t st = g_host.stream, cs = g_host.copy_stream;
     CUDA_TRY(cudaMemcpyAsync(dEdges, bin_edges_host, (size_t)(n_bins + 1) * sizeof(double), cudaMemcpyHostToDevice, st));
-    rc = osc_reweight_bin_scales(dEt, dEr, dW, dC, n, energy_scales, n_scales, dEdges, n_bins, dH, st);
-    if (rc) return rc;
-    CUDA_TRY(cudaMemcpyAsync(hist_out_host, dH, (size_t)n_scales * nh * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (n_chunks == 1) {
+        if (n) {
+            CUDA_TRY(cudaMemcpyAsync(dEt, E_true_host, n * sizeof(double), cudaMemcpyHostToDevice, st));
+            CUDA_TRY(cudaMemcpyAsync(dEr, E_reco_host, n * sizeof(double), cudaMemcpyHostToDevice, st));
+            CUDA_TRY(cudaMemcpyAsync(dW, w0_host, n * sizeof(double), cudaMemcpyHostToDevice, st));
+            CUDA_TRY(cudaMemcpyAsync(dC, channel_host, n, cudaMemcpyHostToDevice, st));
+        }
+        if ((rc = osc_reweight_bin_scales(dEt, dEr, dW, dC, n, energy_scales, n_scales, dEdges, n_bins, dH, st))) return rc;
+    } else {
+        // the copy stream runs ahead of the kernels by whole chunks; a chunk's kernel waits for its four arrays only
+        for (int c = 0; c < n_chunks; ++c) {
+            const size_t o = (size_t)c * chunk, m = std::min(chunk, n - o);
+            CUDA_TRY(cudaMemcpyAsync(dEt + o, E_true_host + o, m * sizeof(double), cudaMemcpyHostToDevice, cs));
+            CUDA_TRY(cudaMemcpyAsync(dEr + o, E_reco_host + o, m * sizeof(double), cudaMemcpyHostToDevice, cs));
+            CUDA_TRY(cudaMemcpyAsync(dW + o, w0_host + o, m * sizeof(double), cudaMemcpyHostToDevice, cs));
+            CUDA_TRY(cudaMemcpyAsync(dC + o, channel_host + o, m, cudaMemcpyHostToDevice, cs));
+            CUDA_TRY(cudaEventRecord(g_host.chunk_ready[c], cs));
+            CUDA_TRY(cudaStreamWaitEvent(st, g_host.chunk_ready[c], 0));
+            if ((rc = osc_reweight_bin_scales(dEt + o, dEr + o, dW + o, dC + o, m, energy_scales, n_scales, dEdges, n_bins,
+                                              dH + (size_t)(1 + c) * nout, st)))
+                break;
+        }
+        if (!rc) {
+            chunk_sum_kernel<<<(unsigned)((nout + 255) / 256), 256, 0, st>>>(dH + nout, n_chunks, nout, dH);
+            rc = post_launch("osc_reweight_bin_scales_host (sum over the chunks)");
+        }
+        if (rc) {                                       // leave both streams idle before the buffers are used again
+            cudaStreamSynchronize(cs);
+            cudaStreamSynchronize(st);
+            return rc;
+        }
+    }
+    CUDA_TRY(cudaMemcpyAsync(hist_out_host, dH, nout * sizeof(double), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     return OSC_OK;
 }

@@ -584,6 +584,33 @@ def test_batch_sorted_paths_on_corner_parameters(osc, path):
     assert_hist_close(got, ref, f"{path} on corner parameters")
 
 
+def test_batch_keeps_the_plan_of_the_last_point_list_only_while_it_is_the_same(osc):
+    """The library keeps the host-side plan of the last point list (compared bytewise): a repeated list must give the same
+    histograms, a list of the same length that differs in one number must give its own."""
+    n = 20_000 + 3
+    et, er, w0, ch = wl.events(n, seed=29)
+    edges = wl.bin_edges()
+    d = [dev(a) for a in (et, er, w0, ch)]
+    de = dev(edges)
+    a_pts = [wl.table1(sin2_th23=0.35 + 0.01 * k, delta_cp=-1.0 + 0.1 * k) for k in range(16)]
+    b_pts = [dict(q) for q in a_pts]
+    b_pts[7]["delta_cp"] = 2.5                        # same group structure, one monomial set differs
+    c_pts = [dict(q) for q in a_pts]
+    c_pts[3]["dm2_32"] = 2.7e-3                       # one point leaves the group
+    for path in K4_PATHS + ["k5"]:
+        with batch_path(path):
+            a1 = host(osc.osc_reweight_bin_batch(a_pts, *d, 1.0, de))
+            b1 = host(osc.osc_reweight_bin_batch(b_pts, *d, 1.0, de))
+            a2 = host(osc.osc_reweight_bin_batch(a_pts, *d, 1.0, de))
+            a3 = host(osc.osc_reweight_bin_batch(a_pts, *d, 1.0, de))
+            c1 = host(osc.osc_reweight_bin_batch(c_pts, *d, 1.0, de))
+        assert np.array_equal(a1, a2) and np.array_equal(a2, a3), path
+        for name, pts, got in (("a", a_pts, a1), ("b", b_pts, b1), ("c", c_pts, c1)):
+            ref = oracle.reweight_bin_batch([oracle.Params(**q) for q in pts], et, er, w0, ch, 1.0, edges)
+            assert_hist_close(got, ref, f"{path}, list {name}")
+        assert not np.array_equal(a1[7], b1[7]) and np.array_equal(a1[6], b1[6])
+
+
 @pytest.mark.parametrize("k4", K4_PATHS)
 def test_k4_all_events_dropped(osc, k4):
     n = 500
@@ -893,6 +920,25 @@ def test_host_entry_points(osc):
     assert hs.shape == (3, 4, 50)
     for k, s in enumerate(wl.ENERGY_SCALES):
         assert_hist_close(hs[k], oracle.reweight_bin(op, et, er, w0, ch, s, edges), f"osc_reweight_bin_scales_host {s}")
+
+
+def test_host_entry_points_in_chunks(osc):
+    """Above 2^20 events the host calls send the events in chunks and run the kernel on chunk c while chunk c + 1 is on
+    the bus (three chunks here, the last one ragged and odd); the per-chunk histograms are added in chunk order."""
+    n = 3_000_001
+    et, er, w0, ch = wl.events(n, seed=15)
+    et[2_000_000] = float("nan"); ch[1_048_576] = 5; er[1_048_575] = -1.0       # dropped events at the chunk borders
+    edges = wl.bin_edges()
+    op = set_params(osc, wl.table1(delta_cp=0.7))
+    hs = osc.osc_reweight_bin_scales_host(et, er, w0, ch, wl.ENERGY_SCALES, edges)
+    again = osc.osc_reweight_bin_scales_host(et, er, w0, ch, wl.ENERGY_SCALES, edges)
+    assert np.array_equal(hs, again), "the chunked host call is not bit-reproducible"
+    d = [dev(a) for a in (et, er, w0, ch)]
+    on_device = host(osc.osc_reweight_bin_scales(*d, wl.ENERGY_SCALES, dev(edges)))
+    np.testing.assert_allclose(hs, on_device, rtol=1e-12, atol=0.0)
+    assert_hist_close(hs[2], oracle.reweight_bin(op, et, er, w0, ch, wl.ENERGY_SCALES[2], edges), "chunked host call")
+    one = osc.osc_reweight_bin_host(et, er, w0, ch, wl.ENERGY_SCALES[0], edges)
+    np.testing.assert_allclose(one, hs[0], rtol=1e-12, atol=0.0)
 
 
 # ------------------------------------------------------------------------------------------------

@@ -132,7 +132,7 @@ int osc_reweight_bin_scales(const double *E_true, const double *E_reco, const do
  *   - points that differ only in sin2_th23 and delta_cp share the matter eigen-problem.  When the list has
  *     at least 8 points per such group on average (a scan grid: "only theta23 and dm2_32
  *     float"), the events are sorted by histogram cell once and the eigen-solve is done once per (event,
- *     group); a point then costs 3 to 6 fused multiply-adds per event (k4, csrc/osc_scan.cuh: from 4e5 events
+ *     group); a point then costs 3 to 6 fused multiply-adds per event (k4, csrc/osc_scan.cuh: from 1e5 events
  *     on one launch per sub-group of 32 points with the point monomials in the kernel parameters, below that
  *     one launch with the event terms in shared memory);
  *   - otherwise every (event, point) pair gets the full closed form: from 4 points on (6 for more than

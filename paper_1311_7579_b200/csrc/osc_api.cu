@@ -1059,11 +1059,13 @@ int scan_merge(const double* partial, const SortedEvents& se, int n_points, doub
 
 // k4 with the tables in the kernel parameters (scan_const_kernel): unless osc_set_batch_path("k4s") asks for the
 // shared-memory slice kernel, whenever every channel is of one of the two kinds the kernel is built for.
-// A launch per sub-group costs at least 14 us however few events there are (the launches of a call overlap only with their
-// neighbours), so it is the choice from 4e5 events on (1024 points in 32 sub-groups, ms per call, slice kernel / this
-// one: 1e5 events 0.33 / 0.46, 3e5 0.40 / 0.47, 5e5 0.61 / 0.50, 1e6 1.12 / 0.75, 1e7 11.2 / 6.4).
-// osc_set_batch_path("k4s" | "k4c") forces one of the two.
-constexpr size_t kConstMinEvents = 400000;
+// A launch per sub-group is 32 launches for 1024 points, about 5 us of host time each with 5.8 kB of parameters: below 1e5
+// events the call is bound by that and the single launch of the slice kernel is ahead (1024 points in 32 sub-groups, plan
+// of the point list kept, ms per call, slice kernel / this one: 1e4 events 0.084 / 0.217, 3e4 0.113 / 0.135, 1e5 0.178 /
+// 0.177, 2e5 0.285 / 0.251, 4e5 0.491 / 0.392, 1e6 1.110 / 0.733, 3e6 3.159 / 1.950).  Dealing the launches round to eight
+// side streams that fork from and join the caller's stream costs more host time than it saves (0.28 ms per call up to
+// 2e5 events).  osc_set_batch_path("k4s" | "k4c") forces one of the two kernels.
+constexpr size_t kConstMinEvents = 100000;
 constexpr size_t kConstUnits = 4096;   // pieces per launch the events are cut into (pieces of 128 / 256 / 320 / 384 / 512
                                        // events at 1e6: 0.845 / 0.747 / 0.752 / 0.780 / 0.782 ms per call)
 bool scan_uses_const(const ScanPlan& plan, size_t n)

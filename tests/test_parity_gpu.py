@@ -432,7 +432,7 @@ def test_batch_point_count_edge_cases(osc):
 # eigen-problem).  osc_set_batch_path forces one path or the other (include/osc.h), so both are checked against the
 # oracle on the same inputs, and against each other.  k4 has two main kernels: "k4s" (shared-memory slice, lane = point)
 # and "k4c" (one launch per sub-group, monomials in the kernel parameters, lane = event); "k4" lets the library choose
-# (k4c from 4e5 events on).
+# (k4c from 1e5 events on).
 # ------------------------------------------------------------------------------------------------
 K4_PATHS = ["k4s", "k4c"]
 

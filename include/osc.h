@@ -122,6 +122,21 @@ int osc_reweight_bin_scales(const double *E_true, const double *E_reco, const do
                             size_t n, const double *energy_scales, int n_scales, const double *bin_edges,
                             int n_bins, double *hist_out, void *stream);
 
+/* osc_reweight_bin for callers that cannot allocate (code under CUDA stream capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): same arguments, same result (to rounding; bit-identical where osc_reweight_bin picks the
+ * same launch shape), but the kernel's scratch -- ticket counters, bin-table cache, per-block partial histograms -- is a
+ * static device array inside the library instead of the per-stream buffer osc_reweight_bin allocates on first use.
+ * This call and everything below it call no cudaMalloc / cudaMallocAsync / cudaFree and no allocating library routine.
+ *   limit      n_bins <= 128 (OSC_ERR_INVALID_ARG above, state unchanged); any n as for osc_reweight_bin
+ *   cost       the array is 1 130 496 bytes; every GPU that loads the library holds it until the process exits
+ *   sharing    ALL calls on a device share the array, whatever their stream: calls that overlap on the GPU (different
+ *              streams, or graphs replayed concurrently) RACE on it and give wrong histograms; calls on one stream are
+ *              ordered and safe.  The array keeps the last call's contents; the call zeroes the counters it needs.
+ * Inputs and outputs are the caller's, as for osc_reweight_bin; hist_out is OVERWRITTEN. */
+int osc_reweight_bin_static(const double *E_true, const double *E_reco, const double *w0, const int8_t *channel,
+                            size_t n, double energy_scale, const double *bin_edges, int n_bins, double *hist_out,
+                            void *stream);
+
 /* Batched parameter sets (row a4; BASELINE.json configs[3]): slice p of hist_out equals
  * osc_reweight_bin run with points[p] (to rounding: the order of the additions differs).  Independent of
  * the state set by osc_set_params.

@@ -28,7 +28,7 @@ EXPORTS = ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "os
            "osc_plan_create", "osc_plan_reweight_bin", "osc_plan_reweight_bin_batch", "osc_plan_destroy",
            "osc_neg2lnl", "osc_bin_centre_compare", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_reweight_bin_scales_host", "osc_last_error", "osc_launch_count",
            "osc_version", "osc_set_device", "osc_get_device", "osc_fp64_peak_probe", "osc_set_batch_path",
-           "osc_set_k2_tuning", "osc_fp64_issue_probe")
+           "osc_set_k2_tuning", "osc_fp64_issue_probe", "osc_reweight_bin_static")
 
 
 class OscError(RuntimeError):
@@ -77,12 +77,14 @@ def lib() -> ctypes.CDLL:
     L.osc_fp64_issue_probe.argtypes = [i, i, i, ctypes.POINTER(d), vp]
     L.osc_set_batch_path.argtypes = [ctypes.c_char_p]
     L.osc_set_k2_tuning.argtypes = [i, i, i, i]
+    L.osc_reweight_bin_static.argtypes = [_dp, _dp, _dp, _dp, sz, d, _dp, i, _dp, vp]
     for name in ("osc_set_params", "osc_prob", "osc_prob_all", "osc_reweight_bin", "osc_reweight_bin_scales",
                  "osc_reweight_bin_batch",
                  "osc_plan_create", "osc_plan_reweight_bin", "osc_plan_reweight_bin_batch", "osc_plan_destroy",
                  "osc_neg2lnl", "osc_bin_centre_compare", "osc_bin_index", "osc_prob_host", "osc_reweight_bin_host", "osc_reweight_bin_scales_host", "osc_set_device",
                  "osc_get_device",
-                 "osc_fp64_peak_probe", "osc_set_batch_path", "osc_set_k2_tuning", "osc_fp64_issue_probe"):
+                 "osc_fp64_peak_probe", "osc_set_batch_path", "osc_set_k2_tuning", "osc_fp64_issue_probe",
+                 "osc_reweight_bin_static"):
         getattr(L, name).restype = i
     L.osc_last_error.restype = ctypes.c_char_p
     L.osc_version.restype = ctypes.c_char_p
@@ -208,6 +210,21 @@ def osc_reweight_bin(E_true, E_reco, w0, channel, energy_scale: float, bin_edges
         raise ValueError("hist_out must hold N_CHANNELS * n_bins values")
     _check(lib().osc_reweight_bin(pt, pr, pw, pc, n, float(energy_scale), _dev(bin_edges, torch.float64, "bin_edges"),
                                   nb, _dev(hist_out, torch.float64, "hist_out"), _stream(stream)))
+    return hist_out
+
+
+def osc_reweight_bin_static(E_true, E_reco, w0, channel, energy_scale: float, bin_edges, hist_out, stream=None):
+    """osc_reweight_bin without any allocation in the library (scratch in a static device array, at most 128 bins);
+    the caller passes hist_out: this wrapper allocates nothing either."""
+    import torch
+
+    nb = _n_bins(bin_edges)
+    n, pt, pr, pw, pc = _event_ptrs(E_true, E_reco, w0, channel)
+    if hist_out.numel() != N_CHANNELS * nb:
+        raise ValueError("hist_out must hold N_CHANNELS * n_bins values")
+    _check(lib().osc_reweight_bin_static(pt, pr, pw, pc, n, float(energy_scale),
+                                         _dev(bin_edges, torch.float64, "bin_edges"), nb,
+                                         _dev(hist_out, torch.float64, "hist_out"), _stream(stream)))
     return hist_out
 
 

@@ -613,6 +613,97 @@ int osc_reweight_bin(const double* E_true, const double* E_reco, const double* w
                            static_cast<cudaStream_t>(stream));
 }
 
+// ------------------------------------------------------------------------------------------------
+// osc_reweight_bin_static: osc_reweight_bin for callers that must not allocate (stream capture, serving loops,
+// harnesses that forbid cudaMalloc).  The scratch of k2 -- ticket counters, bin-table cache, block partials -- lives in
+// a file-scope __device__ array instead of the per-stream scratch the library otherwise allocates on first use.  Every
+// GPU that loads the library holds the array (1.08 MB) until the process exits; every call shares it.
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int kStaticMaxBins = 128;    // the binnings k2 takes with its widest block (768 threads, two slots per warp)
+constexpr int kStaticMaxGrid = 256;    // blocks: one per SM, clamped
+constexpr size_t kStaticScratchBytes =
+    kScratchHead + (size_t)(kStaticMaxGrid + (kStaticMaxGrid + kGroup - 1) / kGroup) * kChannels * kStaticMaxBins * sizeof(double);
+
+} // namespace
+
+// In host code this name is a host-side stand-in for the symbol, not a device address: the address the kernels get is
+// taken with cudaGetSymbolAddress below.  Zero-initialised when the module is loaded.
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+namespace {
+
+// Device address of g_static_scratch on the current device (taken once per device, with that device current).
+int static_scratch(char** out)
+{
+    static std::atomic<char*> ptr[64];
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return fail(OSC_ERR_CUDA, "device index %d out of range", dev);
+    char* p = ptr[dev].load(std::memory_order_acquire);
+    if (!p) {
+        void* q = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&q, g_static_scratch);
+        if (e != cudaSuccess || !q)
+            return fail(OSC_ERR_CUDA, "cudaGetSymbolAddress(g_static_scratch) on device %d: %s", dev, cudaGetErrorString(e));
+        p = static_cast<char*>(q);
+        ptr[dev].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return OSC_OK;
+}
+
+} // namespace
+
+int osc_reweight_bin_static(const double* E_true, const double* E_reco, const double* w0, const int8_t* channel, size_t n,
+                            double energy_scale, const double* bin_edges, int n_bins, double* hist_out, void* stream)
+{
+    int rc = check_bin_args(E_true, E_reco, w0, channel, n, energy_scale, bin_edges, n_bins, hist_out);
+    if (rc) return rc;
+    if (n_bins > kStaticMaxBins)
+        return fail(OSC_ERR_INVALID_ARG, "osc_reweight_bin_static: n_bins = %d is more than the %d bins its static scratch "
+                                         "(%zu bytes per GPU) is laid out for; use osc_reweight_bin", n_bins, kStaticMaxBins,
+                    kStaticScratchBytes);
+    if (n > 0 && !w0) return fail(OSC_ERR_INVALID_ARG, "null w0 with n > 0");
+    if (!aligned(hist_out, 8)) return fail(OSC_ERR_ALIGNMENT, "hist_out not 8-byte aligned");
+    HostSet h;
+    if ((rc = snapshot(h))) return rc;
+    BinArgs args;
+    make_bin_args(h, args);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t nh = (size_t)kChannels * n_bins;
+    if (n == 0) {
+        CUDA_TRY(cudaMemsetAsync(hist_out, 0, nh * sizeof(double), st));
+        return OSC_OK;
+    }
+    constexpr int THREADS = 768;
+    const size_t smem = k2_smem_bytes(n_bins, THREADS, 1);
+    if (smem + 1024 > kSmemBudget)
+        return fail(OSC_ERR_INVALID_ARG, "internal: %d bins do not fit the 768-thread layout of k2", n_bins);
+    int sms = 0;
+    if ((rc = sm_count(&sms))) return rc;
+    const size_t ntiles = (n + 2 * THREADS - 1) / (2 * (size_t)THREADS);
+    if (ntiles > 0xFFFFFFFFull) return fail(OSC_ERR_INVALID_ARG, "n = %zu events is more than one call takes (2^32 tiles)", n);
+    size_t g = std::min<size_t>((size_t)sms, (size_t)kStaticMaxGrid);
+    if (ntiles < g) g = ntiles;
+    const int grid = (int)g;
+    if (merge_scratch_bytes(grid, nh) > kStaticScratchBytes)
+        return fail(OSC_ERR_INVALID_ARG, "internal: static scratch too small for %d blocks x %zu cells", grid, nh);
+    char* scratch = nullptr;
+    if ((rc = static_scratch(&scratch))) return rc;
+    // the array keeps what the last call left: the ticket counters must start at zero (a call that failed on the device
+    // may have left them set); the bin-table cache is validated against the edges by the kernel, the partials are
+    // written before they are read
+    CUDA_TRY(cudaMemsetAsync(scratch, 0, kCounterBytes, st));
+    const CallScratch cs = call_scratch(scratch, grid, nh);
+    const bool vec = aligned(E_true, 16) && aligned(E_reco, 16) && aligned(w0, 16) && aligned(channel, 2);
+    return vec ? launch_k2<true, THREADS>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
+                                          n_bins, 1, cs, hist_out)
+               : launch_k2<false, THREADS>(grid, smem, st, args, E_true, E_reco, w0, channel, n, energy_scale, bin_edges,
+                                           n_bins, 1, cs, hist_out);
+}
+
 namespace {
 
 // Pinned staging for host-built tables that a batched call uploads: a small ring of page-locked buffers, each

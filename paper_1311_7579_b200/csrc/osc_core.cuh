@@ -34,7 +34,7 @@ struct OscEig {
 };
 
 // Rows a2a-a2d: eigenvalues, gap phases and the two sinc-like factors for matter term A at 1/E.
-__device__ __forceinline__ void eig_solve(const OscSet& ps, double A, double invE, OscEig& o)
+__device__ __forceinline__ void eig_solve(const OscSet& ps, double A, double invE, OscEig& o, const PolyTop& top)
 {
     const double SQ3 = 1.7320508075688772;
     const double HALF_SQ3 = 0.8660254037844386;
@@ -86,14 +86,19 @@ __device__ __forceinline__ void eig_solve(const OscSet& ps, double A, double inv
     // a2d gap phases in quarter turns: g R xq23 / E (signed with R)
     double RX = R * (ps.xq23 * invE);
     double s1, c1c, s12, c12;
-    sincos_quarter_mul(ga, RX, s1, c1c);
-    sincos_quarter_mul(gb, RX, s12, c12);
+    sincos_quarter_mul(ga, RX, s1, c1c, top);
+    sincos_quarter_mul(gb, RX, s12, c12, top);
     o.s1h = s1;
     o.c1h = c1c;
     o.c02 = fma(c1c, c12, -(s1 * s12));
     o.s02 = fma(s1, c12, c1c * s12);
     o.kap0 = s1 * ka;
     o.kap2 = s12 * kb;
+}
+
+__device__ __forceinline__ void eig_solve(const OscSet& ps, double A, double invE, OscEig& o)
+{
+    eig_solve(ps, A, invE, o, poly_top());
 }
 
 // Rows a2e-a2f: |Z_{beta alpha}|^2 for one transition.

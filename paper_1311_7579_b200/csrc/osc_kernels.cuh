@@ -313,6 +313,37 @@ __device__ __forceinline__ bool locate_one(const BinView& bt, double energy_scal
     return ok;
 }
 
+// Loop-invariant constants of the closed form that the event loops of k2 and k2s keep in registers.  ptxas does not keep
+// them on its own: set.dd and set.k1 (c1 = fma(A, k1, dd): two constants in one DFMA) and the four leading polynomial
+// coefficients (PolyTop, osc_math.cuh) are re-loaded with LDC.64 in every iteration, and the DFMAs that consume them
+// wait on the short scoreboard -- 16 % of the warp-state samples of k2s.  Read through a volatile shared-memory load
+// (the block's copy of BinArgs at `pb`; its pad word is 0.0) the values cannot be rematerialised from the constant
+// bank, so they stay in registers.  Measured per 1e7 events: k2 124.6 -> 118.5 us (551 instead of 627 instructions per
+// pair of events), k2s (three scales) 242 -> 198 us; only dd, k1: 121.5 / 213 us; only the coefficients: 123 us.
+// k2 at 200 / 400 / 500 bins: 130.8 -> 121.0, 156.4 -> 139.3, 168.1 -> 165.2 us.  The one shape that loses is k2's
+// 256 threads with one sub-histogram per warp (binnings above ~570 bins: 228 -> 238 us at 768 bins), which keeps the
+// constants where ptxas puts them (PIN = false).
+struct LoopConsts {
+    OscSet set;
+    PolyTop top;
+};
+template <bool PIN = true>
+__device__ __forceinline__ LoopConsts pin_loop_consts(const BinArgs& a, uint32_t pb)
+{
+    LoopConsts c;
+    c.set = a.set;
+    c.top = poly_top();
+    if (!PIN) return c;
+    c.set.dd = lds_f64_volatile(pb + 8u * 2u);
+    c.set.k1 = lds_f64_volatile(pb + 8u * 3u);
+    const double zero = lds_f64_volatile(pb + 8u * 5u);
+    c.top.c4 += zero;
+    c.top.c5 += zero;
+    c.top.c10 += zero;
+    c.top.c11 += zero;
+    return c;
+}
+
 // Two events of one thread as they come from global memory (VEC: events 2i, 2i+1 by 128-bit loads).  The two channel
 // bytes stay packed (low byte: first event) until they are used, so that nothing waits on the load where it is issued.
 struct EventPair {
@@ -358,6 +389,7 @@ __device__ __forceinline__ void k2_loop(const BinArgs& a, const double* __restri
                                         const BinView& bt, uint32_t pb, const LaneHist& lh, unsigned lt_mask,
                                         unsigned ntiles, unsigned t, EventPair cur)
 {
+    const LoopConsts lc = pin_loop_consts<!(THREADS == 256 && SLOTS == 1)>(a, pb);
     while (t < ntiles) {
         int cell0, cell1;
         unsigned c0, c1;
@@ -374,8 +406,8 @@ __device__ __forceinline__ void k2_loop(const BinArgs& a, const double* __restri
         const OscTrans tr1 = load_trans(pb, (int)c1);
         const double A0 = tr0.sa * Es0, A1 = tr1.sa * Es1;  // a2a
         OscEig e0, e1;
-        eig_solve(a.set, A0, rcp_pos(Es0), e0);             // a2b-a2d
-        eig_solve(a.set, A1, rcp_pos(Es1), e1);
+        eig_solve(lc.set, A0, rcp_pos(Es0), e0, lc.top);    // a2b-a2d
+        eig_solve(lc.set, A1, rcp_pos(Es1), e1, lc.top);
         int rmax1 = 0;
         if (SLOTS == 2) warp_hist_rank(plan, lt_mask);
         else warp_hist_rank_single(plan, lt_mask, rmax1);
@@ -473,6 +505,7 @@ __device__ __forceinline__ void k2s_loop(const BinArgs& a, const double* __restr
                                          unsigned ntiles, unsigned t, EventPair cur)
 {
     const int nh = kChannels * bt.nb;
+    const LoopConsts lc = pin_loop_consts(a, pb);
     while (t < ntiles) {
         const unsigned ch0 = cur.chp & 0xFFu, ch1 = cur.chp >> 8;
         const bool ok0 = energy_ok(cur.Et0) && ch0 < (unsigned)kChannels;
@@ -495,8 +528,8 @@ __device__ __forceinline__ void k2s_loop(const BinArgs& a, const double* __restr
         const OscTrans tr1 = load_trans(pb, (int)c1);
         const double A0 = tr0.sa * Es0, A1 = tr1.sa * Es1;  // a2a
         OscEig e0, e1;
-        eig_solve(a.set, A0, rcp_pos(Es0), e0);             // a2b-a2d
-        eig_solve(a.set, A1, rcp_pos(Es1), e1);
+        eig_solve(lc.set, A0, rcp_pos(Es0), e0, lc.top);    // a2b-a2d
+        eig_solve(lc.set, A1, rcp_pos(Es1), e1, lc.top);
 #pragma unroll
         for (int k = 0; k < NS; ++k) warp_hist_rank(plan[k], lt_mask);
         const double w_0 = __dmul_rn(wp0, assemble(e0, A0, tr0));   // a2e-a2f, a3a

@@ -83,8 +83,17 @@ __device__ __forceinline__ double floor_hi_word(double v, int hi_floor)
     return __hiloint2double(max(__double2hiint(v), hi_floor), __double2loint(v));
 }
 
+// The four coefficients that start the two polynomials: fma(c12, z, c11) and fma(c5, z, c4) have TWO constant
+// operands, a DFMA takes one from a uniform register, so ptxas loads the other into a register with LDC -- inside the
+// event loop, and the DFMA then waits for it on the short scoreboard.  A kernel whose loop has the registers keeps the
+// four in registers (pin_loop_consts in osc_kernels.cuh); everyone else passes poly_top() and gets the code as before.
+struct PolyTop {
+    double c4, c5, c10, c11;
+};
+__device__ __forceinline__ PolyTop poly_top() { return PolyTop{kPoly[4], kPoly[5], kPoly[10], kPoly[11]}; }
+
 // sin and cos of (pi/2) * a * b for |a b| < 2^31.
-__device__ __forceinline__ void sincos_quarter_mul(double a, double b, double& s, double& c)
+__device__ __forceinline__ void sincos_quarter_mul(double a, double b, double& s, double& c, const PolyTop& top)
 {
     const double MAGIC = kPoly[13];          // adding 1.5 * 2^52 rounds to the nearest integer
     double kd = fma(a, b, MAGIC);
@@ -92,9 +101,9 @@ __device__ __forceinline__ void sincos_quarter_mul(double a, double b, double& s
     kd -= MAGIC;
     const double f = fma(a, b, -kd);         // exact product minus integer: |f| <= 1/2 (+ 1 ulp of a b)
     const double z = f * f;
-    double pc = fma(kPoly[12], z, kPoly[11]);
-    double ps = fma(kPoly[5], z, kPoly[4]);
-    pc = fma(pc, z, kPoly[10]);
+    double pc = fma(kPoly[12], z, top.c11);
+    double ps = fma(top.c5, z, top.c4);
+    pc = fma(pc, z, top.c10);
     ps = fma(ps, z, kPoly[3]);
     pc = fma(pc, z, kPoly[9]);
     ps = fma(ps, z, kPoly[2]);
@@ -110,6 +119,10 @@ __device__ __forceinline__ void sincos_quarter_mul(double a, double b, double& s
     const double cc = odd ? ps : pc;
     s = flip_sign_if(ss, (k & 2) << 30);
     c = flip_sign_if(cc, ((k + 1) & 2) << 30);
+}
+__device__ __forceinline__ void sincos_quarter_mul(double a, double b, double& s, double& c)
+{
+    sincos_quarter_mul(a, b, s, c, poly_top());
 }
 
 // t = cos(acos(U/2)/3) in [sqrt(3)/2, 1] for U in [0, 2], i.e. the largest root of 8 t^3 - 6 t = U,

@@ -97,3 +97,28 @@ def test_static_scratch_call_sizes_and_limits(osc):
     assert "128" in str(ei.value) and "osc_reweight_bin_static" in str(ei.value)
     torch.cuda.synchronize()
     assert float((big - 5.0).abs().sum()) == 0.0
+
+
+def test_static_scratch_call_under_stream_capture(osc):
+    """What the entry point is for: the call is captured into a CUDA graph (a cudaMalloc inside the capture would
+    invalidate it) and replayed on new contents of the same buffers."""
+    n, edges = 200_000, wl.bin_edges()
+    osc.osc_set_params(**wl.table1())
+    d = [dev(a) for a in wl.events(n, seed=74)]
+    de = dev(edges)
+    out = torch.zeros((osc.N_CHANNELS, len(edges) - 1), dtype=torch.float64, device="cuda")
+    osc.osc_reweight_bin_static(*d, 1.0, de, out)              # set-up outside the capture: symbol address, attributes
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    with torch.cuda.graph(g, stream=side):
+        osc.osc_reweight_bin_static(*d, 1.0, de, out, stream=torch.cuda.current_stream())
+    for seed in (75, 76):
+        fresh = wl.events(n, seed=seed)
+        for t_dev, a in zip(d, fresh):
+            t_dev.copy_(torch.from_numpy(np.ascontiguousarray(a)))
+        out.fill_(-1.0)
+        g.replay()
+        torch.cuda.synchronize()
+        ref = osc.osc_reweight_bin(*d, 1.0, de).cpu().numpy()
+        np.testing.assert_allclose(out.cpu().numpy(), ref, rtol=RTOL, atol=0.0)

@@ -396,9 +396,12 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
                                        n_bins, n_sub_t, ms, hist_out);
 }
 
-// Threads per block of k2s, 512 / kScalesThreads blocks per SM (126 registers either way).  1e7 events x 3 scales:
-// 256 x 2 blocks 242.5 us, 512 x 1 block 268.3 us (k2 itself is the other way round: its one block of 768 threads wins).
-constexpr int kScalesThreads = 256;
+// Threads per block of k2s, 512 / kScalesThreads blocks per SM (126-128 registers either way).  1e7 events x 3 scales, in
+// the order the kernel changed: as round 2 began 2 x 256 threads 242.5 us, 1 x 512 268.3 us; with the loop constants in
+// registers 198.0 / 193.9; with gridDim.x in a register as well 190.0 / 182.2 (1e8 events: 1753 / 1694 us, 1e6: 32.8 /
+// 30.4) -- once the warps no longer wait for constants, one block (half the partial sums to merge, all warps the same age)
+// is ahead, as it is for k2.  2 x 320 and 1 x 640 threads (96 registers): 198.1 / 195.4 us.
+constexpr int kScalesThreads = 512;
 constexpr int kScalesBlocksPerSM = 512 / kScalesThreads;
 
 template <bool VEC, int NS>

@@ -506,6 +506,9 @@ __device__ __forceinline__ void k2s_loop(const BinArgs& a, const double* __restr
 {
     const int nh = kChannels * bt.nb;
     const LoopConsts lc = pin_loop_consts(a, pb);
+    // gridDim.x in a register: ptxas otherwise re-loads it with LDC right before `t += gridDim.x`, and the add then waits
+    // for it on the short scoreboard -- 11 % of the warp-state samples of this kernel (profiles/r2_k2s_full.md)
+    const unsigned stride = pin_u32(gridDim.x);
     while (t < ntiles) {
         const unsigned ch0 = cur.chp & 0xFFu, ch1 = cur.chp >> 8;
         const bool ok0 = energy_ok(cur.Et0) && ch0 < (unsigned)kChannels;
@@ -522,7 +525,7 @@ __device__ __forceinline__ void k2s_loop(const BinArgs& a, const double* __restr
             warp_hist_match(plan[k], lh, cell0, cell1);
         }
         const double wp0 = cur.wp0, wp1 = cur.wp1;
-        t += gridDim.x;
+        t += stride;
         if (t < ntiles) cur = load_pair<VEC, THREADS>(E_true, E_reco, w0, channel, n, t);
         const OscTrans tr0 = load_trans(pb, (int)c0);
         const OscTrans tr1 = load_trans(pb, (int)c1);

@@ -390,6 +390,9 @@ __device__ __forceinline__ void k2_loop(const BinArgs& a, const double* __restri
                                         unsigned ntiles, unsigned t, EventPair cur)
 {
     const LoopConsts lc = pin_loop_consts<!(THREADS == 256 && SLOTS == 1)>(a, pb);
+    // the tile stride: the 768-thread shape gets it through a uniform register; the others re-load gridDim.x with an LDC
+    // in every iteration and wait for it (as k2s did), unless it is pinned in a register
+    const unsigned stride = THREADS == 768 ? gridDim.x : pin_u32(gridDim.x);
     while (t < ntiles) {
         int cell0, cell1;
         unsigned c0, c1;
@@ -400,7 +403,7 @@ __device__ __forceinline__ void k2_loop(const BinArgs& a, const double* __restri
         warp_hist_match_pred(plan, lh, ok0, cell0, ok1, cell1);
         const double wp0 = cur.wp0, wp1 = cur.wp1;
         // prefetch: E_true, E_reco and channel of the current pair are dead from here on
-        t += gridDim.x;
+        t += stride;
         if (t < ntiles) cur = load_pair<VEC, THREADS>(E_true, E_reco, w0, channel, n, t);
         const OscTrans tr0 = load_trans(pb, (int)c0);
         const OscTrans tr1 = load_trans(pb, (int)c1);

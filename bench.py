@@ -670,6 +670,15 @@ def main():
             dist.destroy_process_group()
         return
 
+    # ---- the two legs reported beside `value`: their own roofline objects (whole step of this rank: one launch of k2s;
+    # three launches of the plan kernel plus their merges) -----------------------------------------------------------
+    fused["roofline"] = ctx.roofline("k2s", n / (fused["ms_per_step"] * 1e-3), BYTES_PER_EVENT, clocks,
+                                     note="whole step = one launch; a unit is an event weighted once and binned at three "
+                                          "energy scales")
+    planned["roofline"] = ctx.roofline("plan", n * len(SCALES) / (planned["ms_per_step"] * 1e-3), 16.0, clocks,
+                                       note="whole step = three launches of the plan kernel and three merges; counts are of "
+                                            "the main kernel; 16 B per event (sorted E_true, w0)")
+
     # ---- roofline of the dominant kernel ------------------------------------------------------------------------
     roofline = ctx.roofline("k2", n / (k_ms * 1e-3), BYTES_PER_EVENT, clocks)
     c2 = opcounts.counts("k2", ctx.counts)

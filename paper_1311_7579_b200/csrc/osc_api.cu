@@ -309,12 +309,16 @@ int launch_reweight(const BinArgs& args, const double* E_true, const double* E_r
     int sms = 0;
     int rc = sm_count(&sms);
     if (rc) return rc;
-    // ONE block per SM, as many warps as the sub-histograms leave room for (1e7 events, B200):
-    //   up to ~140 bins   768 threads, a sub-histogram per (warp, event of the lane)   129-138 us
-    //   up to ~213 bins   512 threads, same layout (118 registers, 5 % fewer instructions)   138-140 us
-    //   up to ~425 bins   512 threads, ONE sub-histogram per warp (SLOTS = 1, lane_hist_single)   139-155 us
-    //   up to ~570 bins   384 threads, one sub-histogram per warp   170-174 us
-    //   up to 768 bins    256 threads, one sub-histogram per warp   245-251 us
+    // ONE block per SM, as many warps as the sub-histograms leave room for (us per 1e7 events on a B200, end of round 2;
+    // in brackets: round 1):
+    //   up to ~140 bins   768 threads, a sub-histogram per (warp, event of the lane)   118-121 (129-138)
+    //   up to ~213 bins   512 threads, same layout (122 registers, 5 % fewer instructions)   118-119 (138-140)
+    //   up to ~425 bins   512 threads, ONE sub-histogram per warp (SLOTS = 1, lane_hist_single)   118-142 (139-155)
+    //   up to ~570 bins   384 threads, one sub-histogram per warp   159-160 (170-174)
+    //   up to 768 bins    256 threads, one sub-histogram per warp   224-228 (245-251)
+    // (1 and 10 bins: 137 and 126 us -- every lane of a warp hits the same few cells.  The step from 118 us at 250 bins to
+    // 133 us at 300 is not the launch shape: above ~280 uniform bins some cells of the 2048-cell look-up table straddle two
+    // edges and the bin search takes its two-step form.)
     // Warp counts that are not a multiple of four per scheduler lose (576, 640, 704 threads: 145, 135, 138 us against
     // 129).  Why one block: co-resident blocks do not run at the same speed -- the warp schedulers favour the warps
     // that arrived first: with three blocks of 256 and equal shares of 44 tiles the first block of an SM needed
